@@ -1,0 +1,130 @@
+/*
+ * wcras.h -- C ABI of libwcras: RAS-preconditioned mixed-precision nested BiCGStab for the
+ * Wilson-clover Dirac equation D phi = eta on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arXiv:1011.3318 (Osaki & Ishikawa, "Domain Decomposition method on GPU cluster").  Citations
+ * below are PAPER.md:<line> (section / equation / algorithm) or BASELINE.json:north_star where the paper
+ * gives no formula.  The readings Q1..Q20 are listed in DESIGN.md.
+ *
+ * Conventions common to every call
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host memory.  The caller
+ *     owns every buffer it passes; the library never frees or keeps a caller pointer after the call
+ *     returns (wcras_create copies the gauge field into its own layouts, so it may be freed afterwards).
+ *   - Canonical layouts at the boundary: site index i = x + Lx*(y + Ly*(z + Lz*t)), mu = 0..3 = x,y,z,t.
+ *       gauge  [V][4][3][3][2]  fp64, (U psi)_a = sum_b U[a][b] psi_b, {re,im} innermost
+ *       spinor [V][4][3][2]     spin, colour, {re,im}; fp32 or fp64 as stated per call
+ *     The internal coalesced SoA layouts (north_star (a)) are private to the library.
+ *   - All work is enqueued on the CUDA stream given to wcras_create.  wcras_solve* and wcras_time_kernel
+ *     synchronise that stream before returning; the apply_* calls do not.
+ *   - in/out buffers of one call must not alias.
+ *   - Return value: WCRAS_OK (0) or a negative code; wcras_last_error gives a message.  No exceptions,
+ *     no exit(), nothing is printed.  There is no CPU fallback: without a CUDA device every call that
+ *     computes returns WCRAS_CUDA_ERROR.
+ */
+#ifndef WCRAS_H
+#define WCRAS_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wcras_ctx wcras_ctx; /* opaque; owns all internal device copies and workspace */
+
+enum {
+    WCRAS_OK = 0,
+    WCRAS_INVALID_ARG = -1,   /* null pointer, dims < 2, b does not divide L, b+2s > L in a split direction, prec not 32/64 */
+    WCRAS_UNSUPPORTED = -2,   /* requested tier cannot hold this domain shape */
+    WCRAS_CUDA_ERROR = -3,    /* CUDA runtime error (message in wcras_last_error) */
+    WCRAS_BREAKDOWN = -4,     /* BiCGStab rho or omega underflow after one restart (reading Q13) */
+    WCRAS_NOT_CONVERGED = -5  /* iteration caps hit; phi is still written and info filled */
+};
+
+/* Filled by wcras_solve*.  Counts follow the paper's "Dv operation count" (Table 1). */
+typedef struct {
+    int outer_iters;    /* fp64 outer BiCGStab iterations (a half-step exit counts as one) */
+    int inner_iters;    /* fp32 inner BiCGStab iterations, summed over all inner solves */
+    int inner_solves;   /* number of inner solves (= preconditioner calls of the outer solver) */
+    int dv_fp32;        /* full-lattice fp32 D applications (Krylov + inside K_RAS, Alg.1 line 9) */
+    int dv_fp64;        /* full-lattice fp64 D applications */
+    int block_dv;       /* block-solver sweeps: MR iterations x K_RAS cycles, each over all domains */
+    int ras_applies;    /* K_RAS applications */
+    int status;         /* same as the return value */
+    double rel_resid_recur; /* |r|/|eta| from the outer recurrence at exit */
+    double rel_resid_true;  /* |eta - D phi|/|eta| recomputed in fp64 (PAPER.md:109 stopping condition) */
+    double ms_total;        /* device time of the whole solve (CUDA events on the stream) */
+    double ms_dslash;       /* sum over fp32 full-lattice D launches } only when wcras_set_timing(ctx,1); */
+    double ms_blocksolve;   /* sum over block-solver launches        } T_Dv^calc / T_dominv^calc of       */
+    double ms_blas;         /* BLAS-1 and conversions                } PAPER.md:103                       */
+    double ms_dslash64;     /* sum over fp64 full-lattice D launches }                                    */
+} wcras_info;
+
+/* create(lattice dims, kappa, c_sw, gauge field)  -- north_star ABI list; PAPER.md:27-31 (Eq. 1.1), :109.
+ * dims[mu] >= 2 (V*36 < 2^31).  gauge_dev: device, canonical layout, fp64, 72*V doubles.
+ * Builds the internal SoA fp64 + fp32 link copies and the clover term A(x) = 1 - (c_sw kappa/2) sum_{mu<nu}
+ * sigma_mu_nu F_mu_nu (clover-leaf F, readings Q3-Q5) as two packed 6x6 Hermitian chiral blocks per site,
+ * in fp64 and rounded to fp32.  cuda_stream: a cudaStream_t (NULL = legacy default stream). */
+int wcras_create(wcras_ctx** out, const int dims[4], double kappa, double csw, const double* gauge_dev,
+                 void* cuda_stream);
+int wcras_destroy(wcras_ctx* ctx);
+
+/* w = D v on the full periodic lattice (north_star (b)).  prec = 32: in/out are float,
+ * prec = 64: double; canonical spinor layout, 24*V reals each, device. */
+int wcras_apply_D(wcras_ctx* ctx, int prec, const void* in_dev, void* out_dev);
+
+/* ras_precondition(domain shape, overlap, block iterations)  -- north_star ABI list; PAPER.md:83 (the three
+ * RAS parameters d, N_dominv, NRAS), :101 (d = 2s), :45 (Omega_i, Omega'_i).
+ * domain[mu] must divide dims[mu]; overlap_s = s >= 0 is the extension per side in every direction with
+ * domain[mu] < dims[mu] (needs domain[mu] + 2s <= dims[mu]); block_iters = N_dominv >= 1 MR iterations;
+ * nras = NRAS >= 1.  Allocates the per-domain workspace and picks the block-solver tier. */
+int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, int block_iters, int nras);
+
+/* Block-solver tier: 0 = automatic (fused on-chip solver when the extended domain fits, else generic),
+ * 1 = generic global-memory tier, 2 = fused tier (WCRAS_UNSUPPORTED at the next wcras_ras_precondition if
+ * the shape does not fit).  Call before wcras_ras_precondition. */
+int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
+
+/* out = P'^T D_Omega' P' in : the principal sub-matrix of D on the extended domain Omega'_index of the
+ * current decomposition ("restriction of D ... with the Dirichlet boundary condition"; reading
+ * Q7), on full-lattice canonical vectors; out = 0 outside Omega'.  domain_index = -1 applies all domains at
+ * once (block-diagonal operator) and is allowed only for overlap 0. */
+int wcras_apply_D_restricted(wcras_ctx* ctx, int prec, int domain_index, const void* in_dev, void* out_dev);
+
+/* v = K_RAS r : Algorithm 1 = Eq. 2.1 with N_dominv MR iterations as the
+ * block solve.  fp32, canonical layout, device. */
+int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev);
+
+/* Solver parameters (reading Q13): inner relative tolerance (default 1e-5), iteration caps (1000 / 50),
+ * use_ras = 0 runs the inner solver without preconditioner ("No prec." column of Table 1). */
+int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int outer_maxit, int use_ras);
+
+/* Per-kernel-class CUDA-event timing inside wcras_solve (fills ms_dslash / ms_blocksolve / ms_blas). */
+int wcras_set_timing(wcras_ctx* ctx, int enable);
+
+/* solve(eta, tolerance) -> phi  -- north_star ABI list; PAPER.md:89 (mixed-precision nested BiCGStab: fp64
+ * outer solver, fp32 inner solver as its preconditioner), Eq. 2.2 (inner solver on
+ * D K_RAS chi = b), :109 (stop at |eta - D phi|/|eta| < tol, true residual recomputed in fp64).
+ * eta_dev / phi_dev: device, canonical fp64, 24*V doubles.  info: host struct, may be NULL. */
+int wcras_solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info);
+
+/* Same, with HOST buffers: copies eta to the device, solves, copies phi back (end-to-end entry point). */
+int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, double tol, wcras_info* info);
+
+/* Export the packed clover term for checking: out_dev = [V][2][36] doubles (packing: 6 real diagonal
+ * entries, then the 15 strictly-lower entries (i>j, k = i(i-1)/2 + j) as {re,im}). */
+int wcras_export_clover(wcras_ctx* ctx, double* out_dev);
+
+/* Time one kernel class in its native layout on internal scratch fields: reps back-to-back launches
+ * bracketed by CUDA events on the library's stream; returns the mean milliseconds per launch.
+ * which: 0 = fp32 D, 1 = fp64 D, 2 = one K_RAS block-solve launch (all domains, current RAS parameters),
+ *        3 = fused BLAS update (x += a p + w s ; r = s - w t ; <rt,r>, |r|^2). */
+int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch);
+
+/* How many kernels of this library have been launched on ctx since creation (for bench.py's gpu_launches). */
+long long wcras_launch_count(const wcras_ctx* ctx);
+
+const char* wcras_last_error(const wcras_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WCRAS_H */

@@ -1,0 +1,303 @@
+// ras.cu -- steps A2-A5: the RAS preconditioner K_RAS (Alg. 1 :59-79, Eq. 2.1 :49-52).
+//
+// Domains (Q8): blocks of shape b tile the lattice, domain index lexicographic
+// (x fastest); Omega'_i = block enlarged by s sites per side in every direction with b_mu < L_mu.
+// Block solve (Q9): N_dominv MR iterations on D_Omega' v = P_Omega' r from v = 0, where
+// D_Omega' is the principal sub-matrix of D on Omega' (hops leaving Omega' dropped; wrap-around hops that stay
+// inside are kept, Q7).
+//
+// Tier 1 (this file, "generic"): domain-local vectors rho, q, v live in global memory as [domain][6][nloc]
+// float4; one launch per MR half-step: (a) q = D_Omega' rho with the domain-local dots <q,rho>, <q,q>
+// (block reduce + fp64 atomics per domain), (b) v += alpha rho, rho -= alpha q.  The projection P_Omega'
+// (Alg.1 line 4) is fused into the first sweep (it reads the full-lattice r directly) and the restriction
+// R_Omega (line 6) + sum (line 8) + phi += v (line 9) into the last update.  Works for every shape/overlap.
+// Tier 2 (ras_fused.cu): one CTA per domain, everything on chip.
+#include "blas.cuh"
+
+namespace wc {
+
+struct DomGeom {
+    int b[4], ext[4], nblk[4], split[4];
+    int s, nloc, nd;
+};
+
+__device__ __forceinline__ void domain_start(const Geom& g, const DomGeom& dg, int d, int start[4]) {
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        const int bc = d % dg.nblk[mu];
+        d /= dg.nblk[mu];
+        int st = bc * dg.b[mu] - (dg.split[mu] ? dg.s : 0);
+        if (st < 0) st += g.L[mu];
+        start[mu] = st;
+    }
+}
+
+// q = D_Omega' rho for local site k of domain d; FIRST: rho is the full-lattice r (projection fused)
+template <bool FIRST>
+__global__ void __launch_bounds__(128) mr_dslash_kernel(Geom g, DomGeom dg, Fields<float> f, float kappa, const float4* __restrict__ rglob,
+                                                        const float4* __restrict__ rho, float4* __restrict__ q, double* __restrict__ scal) {
+    const int d = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc[3] = {0, 0, 0};
+    if (k < dg.nloc) {
+        int start[4], c[4], x[4];
+        domain_start(g, dg, d, start);
+        {
+            int kk = k;
+            c[0] = kk % dg.ext[0]; kk /= dg.ext[0];
+            c[1] = kk % dg.ext[1]; kk /= dg.ext[1];
+            c[2] = kk % dg.ext[2];
+            c[3] = kk / dg.ext[2];
+        }
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            x[mu] = start[mu] + c[mu];
+            if (x[mu] >= g.L[mu]) x[mu] -= g.L[mu];
+        }
+        const size_t V = g.V;
+        const int i = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + g.L[2] * x[3]));
+        const int gs[4] = {1, g.L[0], g.L[0] * g.L[1], g.L[0] * g.L[1] * g.L[2]};
+        const int ls[4] = {1, dg.ext[0], dg.ext[0] * dg.ext[1], dg.ext[0] * dg.ext[1] * dg.ext[2]};
+        const float4* vin = FIRST ? rglob : rho + (size_t)d * 6 * dg.nloc;
+        const size_t vstride = FIRST ? V : (size_t)dg.nloc;
+        float hop[24];
+#pragma unroll
+        for (int n = 0; n < 24; n++) hop[n] = 0;
+#define WC_MR_DIR(MU)                                                                                         \
+    {                                                                                                         \
+        const bool full = dg.ext[MU] == g.L[MU];                                                              \
+        const bool kf = full || c[MU] + 1 < dg.ext[MU];                                                       \
+        const bool kb = full || c[MU] > 0;                                                                    \
+        const int gjb = x[MU] == 0 ? i + (g.L[MU] - 1) * gs[MU] : i - gs[MU];                                 \
+        float u[18], sn[24];                                                                                  \
+        if (kf) {                                                                                             \
+            const int gjf = x[MU] + 1 == g.L[MU] ? i - (g.L[MU] - 1) * gs[MU] : i + gs[MU];                   \
+            const int ljf = c[MU] + 1 == dg.ext[MU] ? k - (dg.ext[MU] - 1) * ls[MU] : k + ls[MU];             \
+            load_link(f, V, i, MU, u);                                                                        \
+            load_spinor(vin, vstride, FIRST ? gjf : ljf, sn);                                                 \
+            hop_fwd<float, MU>(u, sn, hop);                                                                   \
+        }                                                                                                     \
+        if (kb) {                                                                                             \
+            const int ljb = c[MU] == 0 ? k + (dg.ext[MU] - 1) * ls[MU] : k - ls[MU];                          \
+            load_link(f, V, gjb, MU, u);                                                                      \
+            load_spinor(vin, vstride, FIRST ? gjb : ljb, sn);                                                 \
+            hop_bwd<float, MU>(u, sn, hop);                                                                   \
+        }                                                                                                     \
+    }
+        WC_MR_DIR(0) WC_MR_DIR(1) WC_MR_DIR(2) WC_MR_DIR(3)
+#undef WC_MR_DIR
+        float sc[24], out[24];
+        {
+            float cl[72];
+            load_spinor(vin, vstride, FIRST ? i : k, sc);
+            load_clover(f, V, i, cl);
+            clover_apply<float>(cl, sc, out);
+        }
+#pragma unroll
+        for (int n = 0; n < 24; n++) out[n] -= kappa * hop[n];
+        store_spinor(q + (size_t)d * 6 * dg.nloc, dg.nloc, k, out);
+#pragma unroll
+        for (int n = 0; n < 12; n++) {  // <q,rho> = sum conj(q) rho ; <q,q>
+            const float qr = out[2 * n], qi = out[2 * n + 1], rr = sc[2 * n], ri = sc[2 * n + 1];
+            acc[0] += (double)(qr * rr + qi * ri);
+            acc[1] += (double)(qr * ri - qi * rr);
+            acc[2] += (double)(qr * qr + qi * qi);
+        }
+    }
+    __shared__ double sm[3][4];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int n = 0; n < 3; n++) {
+        const double s = warp_sum(acc[n]);
+        if (lane == 0) sm[n][w] = s;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double s = 0;
+        for (int ww = 0; ww < (int)(blockDim.x >> 5); ww++) s += sm[threadIdx.x][ww];
+        atomicAdd(&scal[(size_t)d * 4 + threadIdx.x], s);
+    }
+}
+
+// v += alpha rho, rho -= alpha q; FIRST: rho_old = P r, v = alpha rho_old; LAST: no rho update and the
+// restriction R_Omega: bulk sites go to the full-lattice vout (ACCUM: vout += v, Alg.1 line 9 phi += v)
+template <bool FIRST, bool LAST, bool ACCUM>
+__global__ void __launch_bounds__(128) mr_update_kernel(Geom g, DomGeom dg, const float4* __restrict__ rglob, float4* __restrict__ rho,
+                                                        const float4* __restrict__ q, float4* __restrict__ v, float4* __restrict__ vout,
+                                                        const double* __restrict__ scal) {
+    const int d = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= dg.nloc) return;
+    const double qr = scal[(size_t)d * 4], qi = scal[(size_t)d * 4 + 1], qq = scal[(size_t)d * 4 + 2];
+    // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9)
+    const float ar = qq > 0 ? (float)(qr / qq) : 0.f, ai = qq > 0 ? (float)(qi / qq) : 0.f;
+    int start[4], c[4], x[4];
+    domain_start(g, dg, d, start);
+    {
+        int kk = k;
+        c[0] = kk % dg.ext[0]; kk /= dg.ext[0];
+        c[1] = kk % dg.ext[1]; kk /= dg.ext[1];
+        c[2] = kk % dg.ext[2];
+        c[3] = kk / dg.ext[2];
+    }
+    bool bulk = true;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        x[mu] = start[mu] + c[mu];
+        if (x[mu] >= g.L[mu]) x[mu] -= g.L[mu];
+        if (dg.split[mu]) bulk = bulk && c[mu] >= dg.s && c[mu] < dg.s + dg.b[mu];
+    }
+    const size_t i = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + (size_t)g.L[2] * x[3]));
+    const size_t base = (size_t)d * 6 * dg.nloc + k;
+#pragma unroll
+    for (int ch = 0; ch < 6; ch++) {
+        const size_t li = base + (size_t)ch * dg.nloc;
+        const float4 rv = FIRST ? rglob[(size_t)ch * g.V + i] : rho[li];
+        float4 vv = FIRST ? make_float4(0.f, 0.f, 0.f, 0.f) : v[li];
+        vv.x += ar * rv.x - ai * rv.y; vv.y += ar * rv.y + ai * rv.x;
+        vv.z += ar * rv.z - ai * rv.w; vv.w += ar * rv.w + ai * rv.z;
+        if (!LAST) {
+            const float4 qv = q[li];
+            float4 rn;
+            rn.x = rv.x - (ar * qv.x - ai * qv.y); rn.y = rv.y - (ar * qv.y + ai * qv.x);
+            rn.z = rv.z - (ar * qv.z - ai * qv.w); rn.w = rv.w - (ar * qv.w + ai * qv.z);
+            rho[li] = rn;
+            v[li] = vv;
+        } else if (bulk) {
+            const size_t gi = (size_t)ch * g.V + i;
+            if (ACCUM) {
+                const float4 o = vout[gi];
+                vv.x += o.x; vv.y += o.y; vv.z += o.z; vv.w += o.w;
+            }
+            vout[gi] = vv;
+        }
+    }
+}
+
+static DomGeom make_domgeom(const wcras_ctx* ctx) {
+    DomGeom dg;
+    for (int mu = 0; mu < 4; mu++) {
+        dg.b[mu] = ctx->ras.b[mu]; dg.ext[mu] = ctx->ras.ext[mu]; dg.nblk[mu] = ctx->ras.nblk[mu];
+        dg.split[mu] = ctx->ras.b[mu] < ctx->geom.L[mu];
+    }
+    dg.s = ctx->ras.s; dg.nloc = ctx->ras.nloc; dg.nd = ctx->ras.nd;
+    return dg;
+}
+
+__global__ void __launch_bounds__(RED_THREADS) k_add_f(size_t n, float4* __restrict__ x, const float4* __restrict__ y) {
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
+        float4 a = x[k];
+        const float4 b = y[k];
+        a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+        x[k] = a;
+    }
+}
+int add_f(wcras_ctx* ctx, float4* x, const float4* y) {
+    k_add_f<<<RED_BLOCKS, RED_THREADS, 0, ctx->stream>>>((size_t)6 * ctx->geom.V, x, y);
+    ctx->launches++;
+    WC_CHECK_LAUNCH();
+    return WCRAS_OK;
+}
+
+int ras_fused_supported(const wcras_ctx* ctx, const int b[4], const int ext[4], int s);
+int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+
+int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
+    RasConfig rc;
+    if (s < 0 || niter < 1 || nras < 1) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: need s>=0, block_iters>=1, nras>=1"); return WCRAS_INVALID_ARG; }
+    rc.nd = 1; rc.nloc = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        const int L = ctx->geom.L[mu], b = domain[mu];
+        if (b < 1 || L % b) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain[%d]=%d does not divide %d", mu, b, L); return WCRAS_INVALID_ARG; }
+        rc.b[mu] = b; rc.nblk[mu] = L / b;
+        rc.ext[mu] = b < L ? b + 2 * s : L;
+        if (rc.ext[mu] > L) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain[%d]+2*overlap=%d exceeds %d", mu, rc.ext[mu], L); return WCRAS_INVALID_ARG; }
+        rc.nd *= rc.nblk[mu]; rc.nloc *= rc.ext[mu];
+    }
+    rc.s = s; rc.niter = niter; rc.nras = nras; rc.set = true;
+    const bool fused_ok = ras_fused_supported(ctx, rc.b, rc.ext, s) != 0;
+    if (ctx->tier_request == 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
+    rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
+    if (int e = ensure_workspace(ctx)) return e;
+    // per-domain workspace of the generic tier (kept even when the fused tier is active: cheap to hold)
+    if (ctx->mr_rho) {
+        WC_CUDA(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal);
+        ctx->mr_rho = ctx->mr_q = ctx->mr_v = nullptr; ctx->mr_scal = nullptr;
+    }
+    if (rc.tier == 1) {
+        const size_t nb = sizeof(float4) * 6 * (size_t)rc.nd * rc.nloc;
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_rho, nb));
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_q, nb));
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_v, nb));
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * niter));
+    }
+    ctx->ras = rc;
+    return WCRAS_OK;
+}
+
+// vout (+)= sum_i R_i MR_niter(D_Omega'_i, P_Omega'_i r)
+static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
+    const RasConfig& rc = ctx->ras;
+    const DomGeom dg = make_domgeom(ctx);
+    const int TH = 128;
+    const dim3 grid((rc.nloc + TH - 1) / TH, rc.nd);
+    WC_CUDA(cudaMemsetAsync(ctx->mr_scal, 0, sizeof(double) * 4 * (size_t)rc.nd * rc.niter, ctx->stream));
+    const Fields<float> f = ctx->fields<float>();
+    const float kappa = (float)ctx->kappa;
+    for (int it = 0; it < rc.niter; it++) {
+        double* scal = ctx->mr_scal + (size_t)it * rc.nd * 4;
+        const bool first = it == 0, last = it == rc.niter - 1;
+        if (first) mr_dslash_kernel<true><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);
+        else mr_dslash_kernel<false><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);
+#define WC_UPD(F, L, A) mr_update_kernel<F, L, A><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, r, ctx->mr_rho, ctx->mr_q, ctx->mr_v, vout, scal)
+        if (first && last) { if (accum) WC_UPD(true, true, true); else WC_UPD(true, true, false); }
+        else if (first) WC_UPD(true, false, false);
+        else if (last) { if (accum) WC_UPD(false, true, true); else WC_UPD(false, true, false); }
+        else WC_UPD(false, false, false);
+#undef WC_UPD
+        ctx->launches += 2;
+    }
+    WC_CHECK_LAUNCH();
+    return WCRAS_OK;
+}
+
+static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
+    TimedRegion tr(ctx, TC_BLOCK);
+    ctx->block_dv += ctx->ras.niter;
+    if (ctx->ras.tier == 2) return ras_fused_block_solve(ctx, r, vout, accum);
+    return generic_block_solve(ctx, r, vout, accum);
+}
+
+int ras_block_solve(wcras_ctx* ctx, const float4* r, float4* v) { return block_solve(ctx, r, v, false); }
+
+// v = K_RAS r  (Alg. 1).  phi = 0, r_0 = r; for j < NRAS: v_j = S r_j; phi += v_j; r_{j+1} = r_j - D v_j
+// (the last residual update is dead and skipped, Q12).
+int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
+    const RasConfig& rc = ctx->ras;
+    if (!rc.set) { snprintf(ctx->err, sizeof ctx->err, "ras_apply: call wcras_ras_precondition first"); return WCRAS_INVALID_ARG; }
+    ctx->ras_applies++;
+    if (rc.nras == 1) return block_solve(ctx, r, v, false);
+    float4* rw = ctx->ras32[0];
+    float4* vj = ctx->ras32[1];
+    const float4* rcur = r;
+    for (int j = 0; j < rc.nras; j++) {
+        // v_j is needed on its own for r -= D v_j, so only the last cycle accumulates straight into phi
+        const bool lastc = j == rc.nras - 1;
+        if (j == 0) {
+            if (int e = block_solve(ctx, rcur, v, false)) return e;
+            if (!lastc) if (int e = dslash<float>(ctx, v, rw, rcur)) return e;  // rw = r - D v_0
+        } else if (lastc) {
+            if (int e = block_solve(ctx, rcur, v, true)) return e;  // phi += v_j fused
+        } else {
+            if (int e = block_solve(ctx, rcur, vj, false)) return e;
+            if (int e = dslash<float>(ctx, vj, rw, rcur)) return e;  // in-place: rw = rw - D v_j
+            TimedRegion tr(ctx, TC_BLAS);
+            if (int e = add_f(ctx, v, vj)) return e;  // phi += v_j
+        }
+        rcur = rw;
+    }
+    return WCRAS_OK;
+}
+
+}  // namespace wc

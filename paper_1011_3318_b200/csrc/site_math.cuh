@@ -1,0 +1,170 @@
+// site_math.cuh -- per-site arithmetic of the Wilson-clover operator, in registers.
+//
+// Everything here works on small fixed-size arrays that the kernels keep in registers:
+//   spinor      T s[24]   index (spin*3 + colour)*2 + {re,im}
+//   half spinor T h[12]   index (hs*3   + colour)*2 + {re,im}, hs = 0,1
+//   link        T u[18]   index (row*3  + col)*2    + {re,im}, (U psi)_a = sum_b U[a][b] psi_b
+//   clover      T c[72]   two chiral 6x6 Hermitian blocks of 36 reals: 6 real diagonal entries, then the
+//                         15 strictly-lower entries (i>j, k = i(i-1)/2 + j) as {re,im}; block 0 acts on
+//                         spins 0,1 and block 1 on spins 2,3 (component index within a block = spin*3+colour)
+//
+// Operator (BASELINE.json:north_star; PAPER.md:27-31 only names it):
+//   (D psi)(x) = A(x) psi(x) - kappa sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu) + (1+gamma_mu) U_mu(x-mu)^dag psi(x-mu) ]
+// gamma matrices: Hermitian chiral basis, gamma_k = sigma_2 (x) sigma_k, gamma_t = sigma_1 (x) 1 (Q2).
+// In this basis (1 -+ gamma_mu) has rank 2 and rows 2,3 are +-1 or +-i times rows 0,1 of the projected
+// spinor, so only a half spinor (2 spin x 3 colour) is multiplied by the link ("projected-spinor hopping
+// term", north_star (b)).
+#pragma once
+
+#if defined(__CUDACC__)
+#define WC_HD __host__ __device__ __forceinline__
+#else
+#define WC_HD inline
+#endif
+
+namespace wc {
+
+// h = upper two rows of (1 + SIGN*gamma_MU) s
+template <typename T, int MU, int SIGN>
+WC_HD void project(const T* __restrict__ s, T* __restrict__ h) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const T s0r = s[2 * c], s0i = s[2 * c + 1];
+        const T s1r = s[6 + 2 * c], s1i = s[6 + 2 * c + 1];
+        const T s2r = s[12 + 2 * c], s2i = s[12 + 2 * c + 1];
+        const T s3r = s[18 + 2 * c], s3i = s[18 + 2 * c + 1];
+        T h0r, h0i, h1r, h1i;
+        if (MU == 0) {  // (gamma_x s)_0 = -i s3, (gamma_x s)_1 = -i s2
+            if (SIGN < 0) { h0r = s0r - s3i; h0i = s0i + s3r; h1r = s1r - s2i; h1i = s1i + s2r; }   // s0 + i s3, s1 + i s2
+            else          { h0r = s0r + s3i; h0i = s0i - s3r; h1r = s1r + s2i; h1i = s1i - s2r; }   // s0 - i s3, s1 - i s2
+        } else if (MU == 1) {  // (gamma_y s)_0 = -s3, (gamma_y s)_1 = s2
+            if (SIGN < 0) { h0r = s0r + s3r; h0i = s0i + s3i; h1r = s1r - s2r; h1i = s1i - s2i; }
+            else          { h0r = s0r - s3r; h0i = s0i - s3i; h1r = s1r + s2r; h1i = s1i + s2i; }
+        } else if (MU == 2) {  // (gamma_z s)_0 = -i s2, (gamma_z s)_1 = i s3
+            if (SIGN < 0) { h0r = s0r - s2i; h0i = s0i + s2r; h1r = s1r + s3i; h1i = s1i - s3r; }   // s0 + i s2, s1 - i s3
+            else          { h0r = s0r + s2i; h0i = s0i - s2r; h1r = s1r - s3i; h1i = s1i + s3r; }   // s0 - i s2, s1 + i s3
+        } else {  // (gamma_t s)_0 = s2, (gamma_t s)_1 = s3
+            if (SIGN < 0) { h0r = s0r - s2r; h0i = s0i - s2i; h1r = s1r - s3r; h1i = s1i - s3i; }
+            else          { h0r = s0r + s2r; h0i = s0i + s2i; h1r = s1r + s3r; h1i = s1i + s3i; }
+        }
+        h[2 * c] = h0r; h[2 * c + 1] = h0i;
+        h[6 + 2 * c] = h1r; h[6 + 2 * c + 1] = h1i;
+    }
+}
+
+// acc += full spinor whose upper rows are g and whose rows 2,3 follow from (1 + SIGN*gamma_MU)
+template <typename T, int MU, int SIGN>
+WC_HD void reconstruct_add(const T* __restrict__ g, T* __restrict__ acc) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const T g0r = g[2 * c], g0i = g[2 * c + 1];
+        const T g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
+        acc[2 * c] += g0r; acc[2 * c + 1] += g0i;
+        acc[6 + 2 * c] += g1r; acc[6 + 2 * c + 1] += g1i;
+        T* a2 = acc + 12 + 2 * c;
+        T* a3 = acc + 18 + 2 * c;
+        if (MU == 0) {
+            if (SIGN < 0) { a2[0] += g1i; a2[1] -= g1r; a3[0] += g0i; a3[1] -= g0r; }   // r2 = -i g1, r3 = -i g0
+            else          { a2[0] -= g1i; a2[1] += g1r; a3[0] -= g0i; a3[1] += g0r; }   // r2 =  i g1, r3 =  i g0
+        } else if (MU == 1) {
+            if (SIGN < 0) { a2[0] -= g1r; a2[1] -= g1i; a3[0] += g0r; a3[1] += g0i; }   // r2 = -g1, r3 = g0
+            else          { a2[0] += g1r; a2[1] += g1i; a3[0] -= g0r; a3[1] -= g0i; }   // r2 = g1, r3 = -g0
+        } else if (MU == 2) {
+            if (SIGN < 0) { a2[0] += g0i; a2[1] -= g0r; a3[0] -= g1i; a3[1] += g1r; }   // r2 = -i g0, r3 = i g1
+            else          { a2[0] -= g0i; a2[1] += g0r; a3[0] += g1i; a3[1] -= g1r; }   // r2 = i g0, r3 = -i g1
+        } else {
+            if (SIGN < 0) { a2[0] -= g0r; a2[1] -= g0i; a3[0] -= g1r; a3[1] -= g1i; }   // r2 = -g0, r3 = -g1
+            else          { a2[0] += g0r; a2[1] += g0i; a3[0] += g1r; a3[1] += g1i; }
+        }
+    }
+}
+
+// g = U h  (both half-spin components)
+template <typename T>
+WC_HD void su3_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restrict__ g) {
+#pragma unroll
+    for (int hs = 0; hs < 2; hs++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const T ur = u[(a * 3 + b) * 2], ui = u[(a * 3 + b) * 2 + 1];
+                const T hr = h[(hs * 3 + b) * 2], hi = h[(hs * 3 + b) * 2 + 1];
+                re += ur * hr - ui * hi;
+                im += ur * hi + ui * hr;
+            }
+            g[(hs * 3 + a) * 2] = re;
+            g[(hs * 3 + a) * 2 + 1] = im;
+        }
+}
+
+// g = U^dagger h
+template <typename T>
+WC_HD void su3_adj_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restrict__ g) {
+#pragma unroll
+    for (int hs = 0; hs < 2; hs++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            T re = 0, im = 0;
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                const T ur = u[(b * 3 + a) * 2], ui = -u[(b * 3 + a) * 2 + 1];
+                const T hr = h[(hs * 3 + b) * 2], hi = h[(hs * 3 + b) * 2 + 1];
+                re += ur * hr - ui * hi;
+                im += ur * hi + ui * hr;
+            }
+            g[(hs * 3 + a) * 2] = re;
+            g[(hs * 3 + a) * 2 + 1] = im;
+        }
+}
+
+// hop += (1 - gamma_MU) U psi_fwd      (forward hop; u = U_MU(x), sf = psi(x+MU))
+template <typename T, int MU>
+WC_HD void hop_fwd(const T* __restrict__ u, const T* __restrict__ sf, T* __restrict__ hop) {
+    T h[12], g[12];
+    project<T, MU, -1>(sf, h);
+    su3_mul<T>(u, h, g);
+    reconstruct_add<T, MU, -1>(g, hop);
+}
+
+// hop += (1 + gamma_MU) U^dag psi_bwd  (backward hop; u = U_MU(x-MU), sb = psi(x-MU))
+template <typename T, int MU>
+WC_HD void hop_bwd(const T* __restrict__ u, const T* __restrict__ sb, T* __restrict__ hop) {
+    T h[12], g[12];
+    project<T, MU, +1>(sb, h);
+    su3_adj_mul<T>(u, h, g);
+    reconstruct_add<T, MU, +1>(g, hop);
+}
+
+// out[12 reals of one chirality] = B x, B = packed Hermitian 6x6 (36 reals), x = 6 complex
+template <typename T>
+WC_HD void herm6_mul(const T* __restrict__ b, const T* __restrict__ x, T* __restrict__ out) {
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+        T re = b[i] * x[2 * i], im = b[i] * x[2 * i + 1];
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            if (j < i) {  // A_ij, stored
+                const int k = 6 + 2 * (i * (i - 1) / 2 + j);
+                re += b[k] * x[2 * j] - b[k + 1] * x[2 * j + 1];
+                im += b[k] * x[2 * j + 1] + b[k + 1] * x[2 * j];
+            } else if (j > i) {  // A_ij = conj(A_ji)
+                const int k = 6 + 2 * (j * (j - 1) / 2 + i);
+                re += b[k] * x[2 * j] + b[k + 1] * x[2 * j + 1];
+                im += b[k] * x[2 * j + 1] - b[k + 1] * x[2 * j];
+            }
+        }
+        out[2 * i] = re;
+        out[2 * i + 1] = im;
+    }
+}
+
+// out = A(x) s
+template <typename T>
+WC_HD void clover_apply(const T* __restrict__ cl, const T* __restrict__ s, T* __restrict__ out) {
+    herm6_mul<T>(cl, s, out);
+    herm6_mul<T>(cl + 36, s + 12, out + 12);
+}
+
+}  // namespace wc

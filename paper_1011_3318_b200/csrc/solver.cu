@@ -1,0 +1,522 @@
+// solver.cu -- steps A6 (inner fp32 BiCGStab on D K_RAS chi = b, Eq. 2.2) and A7 (outer fp64
+// "flexible" BiCGStab whose preconditioner is the inner solve), with the fused BLAS-1 kernels
+// of north_star (d).  Recurrences (reading Q13), identical for both precisions:
+//   x=0, r=b, rt=r, rho=alpha=omega=1, v=p=0; loop:
+//   rho'=<rt,r>; beta=(rho'/rho)(alpha/omega); p=r+beta(p-omega v); ph=K p; v=D ph; alpha=rho'/<rt,v>;
+//   s=r-alpha v; [outer only: stop if |s|/|b|<tol with x+=alpha ph]; sh=K s; t=D sh; omega=<t,s>/<t,t>;
+//   x+=alpha ph+omega sh; r=s-omega t; stop when |r|/|b|<tol.
+#include <cmath>
+
+#include "blas.cuh"
+
+namespace wc {
+
+template <typename T> struct cpx { T r, i; };
+
+template <typename T> __device__ __forceinline__ void unpack(const float4& v, cpx<T>* c) { c[0] = {v.x, v.y}; c[1] = {v.z, v.w}; }
+template <typename T> __device__ __forceinline__ void unpack(const double2& v, cpx<T>* c) { c[0] = {v.x, v.y}; }
+__device__ __forceinline__ float4 pack(const cpx<float>* c, float4*) { return make_float4(c[0].r, c[0].i, c[1].r, c[1].i); }
+__device__ __forceinline__ double2 pack(const cpx<double>* c, double2*) { return make_double2(c[0].r, c[0].i); }
+
+template <typename T> __device__ __forceinline__ cpx<T> operator+(cpx<T> a, cpx<T> b) { return {a.r + b.r, a.i + b.i}; }
+template <typename T> __device__ __forceinline__ cpx<T> operator-(cpx<T> a, cpx<T> b) { return {a.r - b.r, a.i - b.i}; }
+template <typename T> __device__ __forceinline__ cpx<T> operator*(cpx<T> a, cpx<T> b) {
+    return {a.r * b.r - a.i * b.i, a.r * b.i + a.i * b.r};
+}
+// acc += conj(a) * b in fp64
+template <typename T> __device__ __forceinline__ void dot_acc(cpx<T> a, cpx<T> b, double& re, double& im) {
+    re += (double)a.r * (double)b.r + (double)a.i * (double)b.i;
+    im += (double)a.r * (double)b.i - (double)a.i * (double)b.r;
+}
+template <typename T> __device__ __forceinline__ cpx<T> ld_scalar(const double* s) { return {(T)s[0], (T)s[1]}; }
+
+#define GRID_STRIDE(idx, n) for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (n); idx += (size_t)gridDim.x * blockDim.x)
+
+// r = b, rt = b, x = 0, p = v = 0; bb = |b|^2; scalars reset
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __restrict__ b, Vec* r, Vec* rt, Vec* x, Vec* p, Vec* v,
+                                                      Scalars* sc, double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    double acc[1] = {0};
+    Vec zero;
+    memset(&zero, 0, sizeof zero);
+    GRID_STRIDE(k, n) {
+        const Vec bv = b[k];
+        cpx<T> c[N];
+        unpack<T>(bv, c);
+#pragma unroll
+        for (int j = 0; j < N; j++) acc[0] += (double)c[j].r * c[j].r + (double)c[j].i * c[j].i;
+        r[k] = bv; rt[k] = bv; x[k] = zero; p[k] = zero; v[k] = zero;
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) {
+        sc->bb = tot[0]; sc->rr = tot[0]; sc->ss = tot[0];
+        sc->rho[0] = tot[0]; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
+        sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+    }
+}
+
+// restart: rt = r, p = v = 0, rho = <r,r>, rho_old = alpha = omega = 1
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_restart(size_t n, const Vec* __restrict__ r, Vec* rt, Vec* p, Vec* v, Scalars* sc,
+                                                         double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    double acc[1] = {0};
+    Vec zero;
+    memset(&zero, 0, sizeof zero);
+    GRID_STRIDE(k, n) {
+        const Vec rv = r[k];
+        cpx<T> c[N];
+        unpack<T>(rv, c);
+#pragma unroll
+        for (int j = 0; j < N; j++) acc[0] += (double)c[j].r * c[j].r + (double)c[j].i * c[j].i;
+        rt[k] = rv; p[k] = zero; v[k] = zero;
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) {
+        sc->rr = tot[0];
+        sc->rho[0] = tot[0]; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
+        sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+    }
+}
+
+// p = r + beta (p - omega v), beta = (rho/rho_old)(alpha/omega)
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* __restrict__ r, Vec* __restrict__ p,
+                                                          const Vec* __restrict__ v, const Scalars* __restrict__ sc) {
+    constexpr int N = Cx<Vec>::N;
+    const cd b = cmul(cdiv({sc->rho[0], sc->rho[1]}, {sc->rho_old[0], sc->rho_old[1]}),
+                      cdiv({sc->alpha[0], sc->alpha[1]}, {sc->omega[0], sc->omega[1]}));
+    const cpx<T> beta = {(T)b.r, (T)b.i}, omega = ld_scalar<T>(sc->omega);
+    GRID_STRIDE(k, n) {
+        cpx<T> rc[N], pc[N], vc[N];
+        unpack<T>(r[k], rc); unpack<T>(p[k], pc); unpack<T>(v[k], vc);
+#pragma unroll
+        for (int j = 0; j < N; j++) pc[j] = rc[j] + beta * (pc[j] - omega * vc[j]);
+        p[k] = pack(pc, (Vec*)nullptr);
+    }
+}
+
+// rtv = <rt, v>; alpha = rho / rtv
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_dot_rtv(size_t n, const Vec* __restrict__ rt, const Vec* __restrict__ v, Scalars* sc,
+                                                         double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    double acc[2] = {0, 0};
+    GRID_STRIDE(k, n) {
+        cpx<T> a[N], b[N];
+        unpack<T>(rt[k], a); unpack<T>(v[k], b);
+#pragma unroll
+        for (int j = 0; j < N; j++) dot_acc(a[j], b[j], acc[0], acc[1]);
+    }
+    double tot[2];
+    if (grid_reduce<2>(acc, partials, ticket, tot)) {
+        sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
+        const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
+        sc->alpha[0] = a.r; sc->alpha[1] = a.i;
+    }
+}
+
+// s = r - alpha v; ss = |s|^2
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_update_s(size_t n, const Vec* __restrict__ r, const Vec* __restrict__ v,
+                                                          Vec* __restrict__ s, Scalars* sc, double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    const cpx<T> alpha = ld_scalar<T>(sc->alpha);
+    double acc[1] = {0};
+    GRID_STRIDE(k, n) {
+        cpx<T> rc[N], vc[N];
+        unpack<T>(r[k], rc); unpack<T>(v[k], vc);
+#pragma unroll
+        for (int j = 0; j < N; j++) {
+            rc[j] = rc[j] - alpha * vc[j];
+            acc[0] += (double)rc[j].r * rc[j].r + (double)rc[j].i * rc[j].i;
+        }
+        s[k] = pack(rc, (Vec*)nullptr);
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) sc->ss = tot[0];
+}
+
+// ts = <t,s>, tt = <t,t>; omega = ts/tt (0 if tt = 0)
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_dot_ts(size_t n, const Vec* __restrict__ t, const Vec* __restrict__ s, Scalars* sc,
+                                                        double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    double acc[3] = {0, 0, 0};
+    GRID_STRIDE(k, n) {
+        cpx<T> a[N], b[N];
+        unpack<T>(t[k], a); unpack<T>(s[k], b);
+#pragma unroll
+        for (int j = 0; j < N; j++) {
+            dot_acc(a[j], b[j], acc[0], acc[1]);
+            acc[2] += (double)a[j].r * a[j].r + (double)a[j].i * a[j].i;
+        }
+    }
+    double tot[3];
+    if (grid_reduce<3>(acc, partials, ticket, tot)) {
+        sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
+        sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
+        sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
+    }
+}
+
+// x += alpha ph + omega sh; r = s - omega t; rho_old = rho; rho = <rt,r>; rr = |r|^2
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_update_xr(size_t n, Vec* __restrict__ x, const Vec* __restrict__ ph,
+                                                           const Vec* __restrict__ sh, const Vec* __restrict__ s,
+                                                           const Vec* __restrict__ t, const Vec* __restrict__ rt, Vec* __restrict__ r,
+                                                           Scalars* sc, double* partials, unsigned* ticket) {
+    constexpr int N = Cx<Vec>::N;
+    const cpx<T> alpha = ld_scalar<T>(sc->alpha), omega = ld_scalar<T>(sc->omega);
+    double acc[3] = {0, 0, 0};
+    GRID_STRIDE(k, n) {
+        cpx<T> xc[N], pc[N], hc[N], sc_[N], tc[N], rc[N];
+        unpack<T>(x[k], xc); unpack<T>(ph[k], pc); unpack<T>(sh[k], hc);
+        unpack<T>(s[k], sc_); unpack<T>(t[k], tc); unpack<T>(rt[k], rc);
+#pragma unroll
+        for (int j = 0; j < N; j++) {
+            xc[j] = xc[j] + alpha * pc[j] + omega * hc[j];
+            sc_[j] = sc_[j] - omega * tc[j];
+            dot_acc(rc[j], sc_[j], acc[0], acc[1]);
+            acc[2] += (double)sc_[j].r * sc_[j].r + (double)sc_[j].i * sc_[j].i;
+        }
+        x[k] = pack(xc, (Vec*)nullptr);
+        r[k] = pack(sc_, (Vec*)nullptr);
+    }
+    double tot[3];
+    if (grid_reduce<3>(acc, partials, ticket, tot)) {
+        sc->rho_old[0] = sc->rho[0]; sc->rho_old[1] = sc->rho[1];
+        sc->rho[0] = tot[0]; sc->rho[1] = tot[1];
+        sc->rr = tot[2];
+    }
+}
+
+// x += alpha ph (half-step exit)
+template <typename T, typename Vec>
+__global__ void __launch_bounds__(RED_THREADS) k_axpy_alpha(size_t n, Vec* __restrict__ x, const Vec* __restrict__ ph,
+                                                            const Scalars* __restrict__ sc) {
+    constexpr int N = Cx<Vec>::N;
+    const cpx<T> alpha = ld_scalar<T>(sc->alpha);
+    GRID_STRIDE(k, n) {
+        cpx<T> xc[N], pc[N];
+        unpack<T>(x[k], xc); unpack<T>(ph[k], pc);
+#pragma unroll
+        for (int j = 0; j < N; j++) xc[j] = xc[j] + alpha * pc[j];
+        x[k] = pack(xc, (Vec*)nullptr);
+    }
+}
+
+// nrm = |a|^2 (fp64 vectors)
+__global__ void __launch_bounds__(RED_THREADS) k_norm2_d(size_t n, const double2* __restrict__ a, Scalars* sc, double* partials,
+                                                         unsigned* ticket) {
+    double acc[1] = {0};
+    GRID_STRIDE(k, n) {
+        const double2 v = a[k];
+        acc[0] += v.x * v.x + v.y * v.y;
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) sc->nrm = tot[0];
+}
+
+// out32 = in64 / sqrt(nrm).  fp32 SoA chunk c4 of site i (float4 [6][V]) holds the complex components 2*c4 and
+// 2*c4+1, which live in fp64 SoA chunks 2*c4 and 2*c4+1 of the same site (double2 [12][V]).
+__global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, const double2* __restrict__ in, float4* __restrict__ out,
+                                                                const Scalars* __restrict__ sc) {
+    const double inv = sc->nrm > 0 ? rsqrt(sc->nrm) : 0.0;
+    GRID_STRIDE(k, 6 * V) {
+        const size_t c4 = k / V, i = k - c4 * V;
+        const double2 a = in[(2 * c4) * V + i], b = in[(2 * c4 + 1) * V + i];
+        out[k] = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
+    }
+}
+// out64 = in32 * sqrt(nrm)
+__global__ void __launch_bounds__(RED_THREADS) k_f2d_scaled(size_t V, const float4* __restrict__ in, double2* __restrict__ out,
+                                                            const Scalars* __restrict__ sc) {
+    const double sc_ = sqrt(sc->nrm);
+    GRID_STRIDE(k, 6 * V) {
+        const size_t c4 = k / V, i = k - c4 * V;
+        const float4 a = in[k];
+        out[(2 * c4) * V + i] = make_double2(a.x * sc_, a.y * sc_);
+        out[(2 * c4 + 1) * V + i] = make_double2(a.z * sc_, a.w * sc_);
+    }
+}
+// x += dx (fp64)
+__global__ void __launch_bounds__(RED_THREADS) k_add_d(size_t n, double2* __restrict__ x, const double2* __restrict__ dx) {
+    GRID_STRIDE(k, n) {
+        double2 a = x[k];
+        const double2 b = dx[k];
+        a.x += b.x; a.y += b.y;
+        x[k] = a;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------
+static int read_scalars(wcras_ctx* ctx, const Scalars* sc) {
+    WC_CUDA(cudaMemcpyAsync(ctx->sc_host, sc, sizeof(Scalars), cudaMemcpyDeviceToHost, ctx->stream));
+    WC_CUDA(cudaStreamSynchronize(ctx->stream));
+    return WCRAS_OK;
+}
+
+#define LAUNCH(kern, ...)                                                        \
+    do {                                                                         \
+        kern<<<RED_BLOCKS, RED_THREADS, 0, ctx->stream>>>(__VA_ARGS__);          \
+        ctx->launches++;                                                         \
+    } while (0)
+
+template <typename T> struct Work {
+    typedef typename VecOf<T>::type Vec;
+    Vec *r, *rt, *p, *v, *s, *t, *ph, *sh;
+    Scalars* sc;
+    size_t n;
+};
+
+// BiCGStab driver.  K(in,out) applies the preconditioner (ignored when k_identity).  status: 0 converged,
+// WCRAS_NOT_CONVERGED, WCRAS_BREAKDOWN, or a CUDA error.
+template <typename T, typename KFunc>
+static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b, typename VecOf<T>::type* x, double tol, int maxit,
+                    bool half_exit, bool k_identity, KFunc K, int* iters, double* relres) {
+    typedef typename VecOf<T>::type Vec;
+    const size_t n = w.n;
+    double* part = ctx->partials;
+    unsigned* tk = ctx->ticket;
+    {
+        TimedRegion tr(ctx, TC_BLAS);
+        LAUNCH((k_init<T, Vec>), n, b, w.r, w.rt, x, w.p, w.v, w.sc, part, tk);
+    }
+    if (int rc = read_scalars(ctx, w.sc)) return rc;
+    const double bb = ctx->sc_host->bb;
+    *iters = 0;
+    *relres = 0;
+    if (bb == 0.0) return WCRAS_OK;
+    Vec* ph = k_identity ? w.p : w.ph;
+    Vec* sh = k_identity ? w.s : w.sh;
+    const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
+    int it = 0, restarts = 0, status = WCRAS_NOT_CONVERGED;
+    double rr = bb;
+    while (it < maxit) {
+        const Scalars& h = *ctx->sc_host;
+        if (hypot(h.rho[0], h.rho[1]) < tiny * bb || (it > 0 && hypot(h.omega[0], h.omega[1]) < tiny)) {
+            if (restarts++) { status = WCRAS_BREAKDOWN; break; }
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH((k_restart<T, Vec>), n, w.r, w.rt, w.p, w.v, w.sc, part, tk);
+        }
+        {
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH((k_update_p<T, Vec>), n, w.r, w.p, w.v, w.sc);
+        }
+        if (!k_identity) if (int rc = K(w.p, ph)) return rc;
+        if (int rc = dslash<T>(ctx, ph, w.v)) return rc;
+        {
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH((k_dot_rtv<T, Vec>), n, w.rt, w.v, w.sc, part, tk);
+            LAUNCH((k_update_s<T, Vec>), n, w.r, w.v, w.s, w.sc, part, tk);
+        }
+        if (half_exit) {
+            if (int rc = read_scalars(ctx, w.sc)) return rc;
+            if (std::sqrt(ctx->sc_host->ss / bb) < tol) {
+                TimedRegion tr(ctx, TC_BLAS);
+                LAUNCH((k_axpy_alpha<T, Vec>), n, x, ph, w.sc);
+                rr = ctx->sc_host->ss;
+                it++;
+                status = WCRAS_OK;
+                break;
+            }
+        }
+        if (!k_identity) if (int rc = K(w.s, sh)) return rc;
+        if (int rc = dslash<T>(ctx, sh, w.t)) return rc;
+        {
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH((k_dot_ts<T, Vec>), n, w.t, w.s, w.sc, part, tk);
+            LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, w.rt, w.r, w.sc, part, tk);
+        }
+        it++;
+        if (int rc = read_scalars(ctx, w.sc)) return rc;
+        rr = ctx->sc_host->rr;
+        if (!(rr == rr)) { status = WCRAS_BREAKDOWN; break; }  // NaN
+        if (std::sqrt(rr / bb) < tol) { status = WCRAS_OK; break; }
+    }
+    WC_CHECK_LAUNCH();
+    *iters = it;
+    *relres = std::sqrt(rr / bb);
+    return status;
+}
+
+int ensure_workspace(wcras_ctx* ctx) {
+    const size_t V = ctx->geom.V;
+    if (!ctx->w32[0]) {
+        for (int k = 0; k < 12; k++)
+            if (alloc_dev(ctx, (void**)&ctx->w32[k], sizeof(float4) * 6 * V)) return WCRAS_CUDA_ERROR;
+        for (int k = 0; k < 12; k++)
+            if (alloc_dev(ctx, (void**)&ctx->w64[k], sizeof(double2) * 12 * V)) return WCRAS_CUDA_ERROR;
+        for (int k = 0; k < 3; k++)
+            if (alloc_dev(ctx, (void**)&ctx->ras32[k], sizeof(float4) * 6 * V)) return WCRAS_CUDA_ERROR;
+        if (alloc_dev(ctx, (void**)&ctx->sc32, sizeof(Scalars))) return WCRAS_CUDA_ERROR;
+        if (alloc_dev(ctx, (void**)&ctx->sc64, sizeof(Scalars))) return WCRAS_CUDA_ERROR;
+        if (alloc_dev(ctx, (void**)&ctx->partials, sizeof(double) * RED_BLOCKS * 8)) return WCRAS_CUDA_ERROR;
+        if (alloc_dev(ctx, (void**)&ctx->ticket, sizeof(unsigned))) return WCRAS_CUDA_ERROR;
+        WC_CUDA(cudaMemsetAsync(ctx->ticket, 0, sizeof(unsigned), ctx->stream));
+        WC_CUDA(cudaMallocHost((void**)&ctx->sc_host, sizeof(Scalars)));
+    }
+    return WCRAS_OK;
+}
+
+static Work<float> work32(wcras_ctx* ctx) {
+    Work<float> w;
+    w.r = ctx->w32[0]; w.rt = ctx->w32[1]; w.p = ctx->w32[2]; w.v = ctx->w32[3]; w.s = ctx->w32[4];
+    w.t = ctx->w32[5]; w.ph = ctx->w32[6]; w.sh = ctx->w32[7];
+    w.sc = ctx->sc32; w.n = (size_t)6 * ctx->geom.V;
+    return w;
+}
+static Work<double> work64(wcras_ctx* ctx) {
+    Work<double> w;
+    w.r = ctx->w64[0]; w.rt = ctx->w64[1]; w.p = ctx->w64[2]; w.v = ctx->w64[3]; w.s = ctx->w64[4];
+    w.t = ctx->w64[5]; w.ph = ctx->w64[6]; w.sh = ctx->w64[7];
+    w.sc = ctx->sc64; w.n = (size_t)12 * ctx->geom.V;
+    return w;
+}
+
+// inner solve as the outer preconditioner: out64 ~= D^-1 in64
+static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int* inner_iters, int* inner_solves) {
+    const size_t V = ctx->geom.V;
+    float4* b32 = ctx->w32[8];
+    float4* x32 = ctx->w32[9];
+    {
+        TimedRegion tr(ctx, TC_BLAS);
+        LAUNCH(k_norm2_d, (size_t)12 * V, in64, ctx->sc64, ctx->partials, ctx->ticket);
+        LAUNCH(k_d2f_normalised, V, in64, b32, ctx->sc64);
+    }
+    Work<float> w = work32(ctx);
+    const bool use_ras = ctx->use_ras && ctx->ras.set;
+    int it = 0;
+    double rel = 0;
+    auto K = [ctx](const float4* in, float4* out) { return ras_apply(ctx, in, out); };
+    int rc = bicgstab<float>(ctx, w, b32, x32, ctx->inner_tol, ctx->inner_maxit, false, !use_ras, K, &it, &rel);
+    *inner_iters += it;
+    *inner_solves += 1;
+    if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
+    // an unconverged or broken-down inner solve is still a usable (flexible) preconditioner
+    {
+        TimedRegion tr(ctx, TC_BLAS);
+        LAUNCH(k_f2d_scaled, V, x32, out64, ctx->sc64);
+    }
+    return WCRAS_OK;
+}
+
+int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info) {
+    if (int rc = ensure_workspace(ctx)) return rc;
+    const size_t V = ctx->geom.V, n64 = 12 * V;
+    cudaEvent_t e0, e1;
+    WC_CUDA(cudaEventCreate(&e0));
+    WC_CUDA(cudaEventCreate(&e1));
+    WC_CUDA(cudaEventRecord(e0, ctx->stream));
+    ctx->dv32 = ctx->dv64 = ctx->block_dv = ctx->ras_applies = 0;
+    ctx->ev_used = 0;
+    for (int k = 0; k < TC_COUNT; k++) ctx->ms_class[k] = 0;
+
+    double2 *eta = ctx->w64[8], *phi = ctx->w64[9], *res = ctx->w64[10], *dx = ctx->w64[11];
+    if (int rc = to_internal(ctx, 64, eta_dev, eta)) return rc;
+    WC_CUDA(cudaMemsetAsync(phi, 0, sizeof(double2) * n64, ctx->stream));
+    WC_CUDA(cudaMemcpyAsync(res, eta, sizeof(double2) * n64, cudaMemcpyDeviceToDevice, ctx->stream));
+    LAUNCH(k_norm2_d, n64, eta, ctx->sc64, ctx->partials, ctx->ticket);
+    if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
+    const double en2 = ctx->sc_host->nrm;
+    double rn2 = en2, recur = 1.0;
+    int outer = 0, inner_iters = 0, inner_solves = 0, status = WCRAS_NOT_CONVERGED;
+    if (en2 == 0.0) status = WCRAS_OK;
+    Work<double> w = work64(ctx);
+    auto K = [&](const double2* in, double2* out) { return inner_solve(ctx, in, out, &inner_iters, &inner_solves); };
+    for (int pass = 0; pass < 10 && status != WCRAS_OK && outer < ctx->outer_maxit; pass++) {
+        int it = 0;
+        double rel = 0;
+        // solve D dx = res to relative accuracy tol*|eta|/|res| so that the total residual meets tol
+        const double tol_pass = 0.7 * tol * std::sqrt(en2 / rn2);
+        int rc = bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel);
+        if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
+        outer += it;
+        recur = rel * std::sqrt(rn2 / en2);
+        {
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH(k_add_d, n64, phi, dx);
+        }
+        if (int r2 = dslash<double>(ctx, phi, res, eta)) return r2;  // res = eta - D phi (true residual, fp64)
+        {
+            TimedRegion tr(ctx, TC_BLAS);
+            LAUNCH(k_norm2_d, n64, res, ctx->sc64, ctx->partials, ctx->ticket);
+        }
+        if (int r3 = read_scalars(ctx, ctx->sc64)) return r3;
+        rn2 = ctx->sc_host->nrm;
+        if (std::sqrt(rn2 / en2) <= tol) status = WCRAS_OK;
+        else if (rc == WCRAS_BREAKDOWN) { status = WCRAS_BREAKDOWN; break; }
+    }
+    if (int rc = from_internal(ctx, 64, phi, phi_dev)) return rc;
+    WC_CUDA(cudaEventRecord(e1, ctx->stream));
+    WC_CUDA(cudaStreamSynchronize(ctx->stream));
+    float ms = 0;
+    WC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (ctx->timing) {
+        for (size_t k = 0; k + 1 < ctx->ev_used; k += 2) {
+            float t = 0;
+            cudaEventElapsedTime(&t, ctx->ev_pool[k], ctx->ev_pool[k + 1]);
+            ctx->ms_class[ctx->ev_class[k]] += t;
+        }
+    }
+    if (info) {
+        info->outer_iters = outer; info->inner_iters = inner_iters; info->inner_solves = inner_solves;
+        info->dv_fp32 = ctx->dv32; info->dv_fp64 = ctx->dv64; info->block_dv = ctx->block_dv;
+        info->ras_applies = ctx->ras_applies; info->status = status;
+        info->rel_resid_recur = recur; info->rel_resid_true = en2 > 0 ? std::sqrt(rn2 / en2) : 0.0;
+        info->ms_total = ms;
+        info->ms_dslash = ctx->ms_class[TC_DSLASH]; info->ms_dslash64 = ctx->ms_class[TC_DSLASH64];
+        info->ms_blocksolve = ctx->ms_class[TC_BLOCK]; info->ms_blas = ctx->ms_class[TC_BLAS];
+    }
+    if (status == WCRAS_NOT_CONVERGED) snprintf(ctx->err, sizeof ctx->err, "solve: not converged after %d outer iterations", outer);
+    if (status == WCRAS_BREAKDOWN) snprintf(ctx->err, sizeof ctx->err, "solve: BiCGStab breakdown");
+    return status;
+}
+
+int time_blas(wcras_ctx* ctx, int reps, double* ms) {
+    if (int rc = ensure_workspace(ctx)) return rc;
+    Work<float> w = work32(ctx);
+    cudaEvent_t e0, e1;
+    WC_CUDA(cudaEventCreate(&e0));
+    WC_CUDA(cudaEventCreate(&e1));
+    WC_CUDA(cudaMemsetAsync(ctx->sc32, 0, sizeof(Scalars), ctx->stream));
+    for (int k = 0; k < 8; k++) WC_CUDA(cudaMemsetAsync(ctx->w32[k], 0, sizeof(float4) * w.n, ctx->stream));
+    WC_CUDA(cudaEventRecord(e0, ctx->stream));
+    for (int k = 0; k < reps; k++)
+        LAUNCH((k_update_xr<float, float4>), w.n, ctx->w32[9], w.ph, w.sh, w.s, w.t, w.rt, w.r, w.sc, ctx->partials, ctx->ticket);
+    WC_CUDA(cudaEventRecord(e1, ctx->stream));
+    WC_CUDA(cudaStreamSynchronize(ctx->stream));
+    float t = 0;
+    WC_CUDA(cudaEventElapsedTime(&t, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *ms = t / reps;
+    return WCRAS_OK;
+}
+
+}  // namespace wc
+
+TimedRegion::TimedRegion(wcras_ctx* c, int cls) : ctx(c), on(c->timing != 0) {
+    if (!on) return;
+    if (ctx->ev_used + 2 > ctx->ev_pool.size()) {
+        for (int k = 0; k < 2; k++) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            ctx->ev_pool.push_back(e);
+            ctx->ev_class.push_back(cls);
+        }
+    }
+    ctx->ev_class[ctx->ev_used] = cls;
+    cudaEventRecord(ctx->ev_pool[ctx->ev_used], ctx->stream);
+}
+TimedRegion::~TimedRegion() {
+    if (!on) return;
+    cudaEventRecord(ctx->ev_pool[ctx->ev_used + 1], ctx->stream);
+    ctx->ev_used += 2;
+}

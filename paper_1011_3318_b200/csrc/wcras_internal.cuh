@@ -1,0 +1,230 @@
+// wcras_internal.cuh -- context, internal SoA layouts and loaders shared by the kernels of libwcras.
+//
+// Internal layouts (north_star (a): "coalesced, vectorised SoA"); V = sites, site index x fastest:
+//   fp32 spinor  float4  [6][V]      chunk c holds reals 4c..4c+3 of the 24 (spin,colour,{re,im})
+//   fp64 spinor  double2 [12][V]     one complex per chunk
+//   fp32 links   float4  [4][4][V]   (mu, k<4: reals 4k..4k+3 of the 18) + float2 [4][V] (reals 16,17)
+//   fp64 links   double2 [4][9][V]
+//   fp32 clover  float4  [18][V]     72 packed reals (site_math.cuh)
+//   fp64 clover  double2 [36][V]
+// Consecutive threads handle consecutive sites, so every load is a full-width coalesced 16-byte access.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <vector>
+
+#include "../../include/wcras.h"
+#include "site_math.cuh"
+
+namespace wc {
+
+struct Geom {
+    int L[4];
+    int V;  // number of sites (<= 2^31 / 36)
+};
+
+template <typename T> struct VecOf;
+template <> struct VecOf<float> { typedef float4 type; static constexpr int CHUNKS = 6; };
+template <> struct VecOf<double> { typedef double2 type; static constexpr int CHUNKS = 12; };
+
+template <typename T> struct Fields;
+template <> struct Fields<float> {
+    const float4* ga;
+    const float2* gb;
+    const float4* cl;
+};
+template <> struct Fields<double> {
+    const double2* g;
+    const double2* cl;
+};
+
+// ---- loaders (device) ----
+__device__ __forceinline__ void load_spinor(const float4* __restrict__ p, size_t stride, size_t i, float* s) {
+#pragma unroll
+    for (int c = 0; c < 6; c++) {
+        const float4 v = p[c * stride + i];
+        s[4 * c] = v.x; s[4 * c + 1] = v.y; s[4 * c + 2] = v.z; s[4 * c + 3] = v.w;
+    }
+}
+__device__ __forceinline__ void load_spinor(const double2* __restrict__ p, size_t stride, size_t i, double* s) {
+#pragma unroll
+    for (int c = 0; c < 12; c++) {
+        const double2 v = p[c * stride + i];
+        s[2 * c] = v.x; s[2 * c + 1] = v.y;
+    }
+}
+__device__ __forceinline__ void store_spinor(float4* __restrict__ p, size_t stride, size_t i, const float* s) {
+#pragma unroll
+    for (int c = 0; c < 6; c++) p[c * stride + i] = make_float4(s[4 * c], s[4 * c + 1], s[4 * c + 2], s[4 * c + 3]);
+}
+__device__ __forceinline__ void store_spinor(double2* __restrict__ p, size_t stride, size_t i, const double* s) {
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c * stride + i] = make_double2(s[2 * c], s[2 * c + 1]);
+}
+__device__ __forceinline__ void load_link(const Fields<float>& f, size_t V, size_t site, int mu, float* u) {
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const float4 v = f.ga[(mu * 4 + k) * V + site];
+        u[4 * k] = v.x; u[4 * k + 1] = v.y; u[4 * k + 2] = v.z; u[4 * k + 3] = v.w;
+    }
+    const float2 w = f.gb[mu * V + site];
+    u[16] = w.x; u[17] = w.y;
+}
+__device__ __forceinline__ void load_link(const Fields<double>& f, size_t V, size_t site, int mu, double* u) {
+#pragma unroll
+    for (int k = 0; k < 9; k++) {
+        const double2 v = f.g[(mu * 9 + k) * V + site];
+        u[2 * k] = v.x; u[2 * k + 1] = v.y;
+    }
+}
+__device__ __forceinline__ void load_clover(const Fields<float>& f, size_t V, size_t site, float* c) {
+#pragma unroll
+    for (int k = 0; k < 18; k++) {
+        const float4 v = f.cl[k * V + site];
+        c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
+    }
+}
+__device__ __forceinline__ void load_clover(const Fields<double>& f, size_t V, size_t site, double* c) {
+#pragma unroll
+    for (int k = 0; k < 36; k++) {
+        const double2 v = f.cl[k * V + site];
+        c[2 * k] = v.x; c[2 * k + 1] = v.y;
+    }
+}
+
+__device__ __forceinline__ void site_coords(const Geom& g, int i, int x[4]) {
+    x[0] = i % g.L[0]; i /= g.L[0];
+    x[1] = i % g.L[1]; i /= g.L[1];
+    x[2] = i % g.L[2];
+    x[3] = i / g.L[2];
+}
+
+// ---- device-resident solver scalars (all fp64) ----
+struct Scalars {
+    double rho[2];      // <rt, r> of the current residual
+    double rho_old[2];  // value used in the previous iteration
+    double alpha[2], omega[2], beta[2];
+    double rtv[2];      // <rt, v>
+    double ts[2];       // <t, s>
+    double tt;          // <t, t>
+    double rr;          // |r|^2
+    double ss;          // |s|^2
+    double bb;          // |b|^2
+    double nrm;         // scratch norm^2 (conversion / true residual)
+    double scale;       // scratch
+};
+
+}  // namespace wc
+
+// ---- RAS configuration ----
+struct RasConfig {
+    bool set = false;
+    int b[4] = {0, 0, 0, 0};      // block shape
+    int ext[4] = {0, 0, 0, 0};    // extended-domain extents
+    int nblk[4] = {0, 0, 0, 0};   // blocks per direction
+    int s = 0, niter = 0, nras = 1;
+    int nd = 0;                   // number of domains
+    int nloc = 0;                 // sites per extended domain
+    int tier = 1;                 // 1 generic, 2 fused
+};
+
+enum TimeClass { TC_DSLASH = 0, TC_BLOCK = 1, TC_BLAS = 2, TC_DSLASH64 = 3, TC_COUNT = 4 };
+
+struct wcras_ctx {
+    wc::Geom geom;
+    double kappa, csw;
+    cudaStream_t stream;
+    // fields
+    double2* g64 = nullptr;
+    float4* g32a = nullptr;
+    float2* g32b = nullptr;
+    double2* c64 = nullptr;
+    float4* c32 = nullptr;
+    // RAS
+    RasConfig ras;
+    int tier_request = 0;
+    float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
+    double* mr_scal = nullptr;                                     // [niter][nd][4]
+    // solver parameters
+    double inner_tol = 1e-5;
+    int inner_maxit = 1000, outer_maxit = 50, use_ras = 1;
+    // workspace (allocated lazily)
+    std::vector<void*> owned;
+    float4* w32[12] = {nullptr};   // fp32 vectors, 6V float4 each
+    double2* w64[12] = {nullptr};  // fp64 vectors, 12V double2 each
+    float4* ras32[3] = {nullptr};  // r, v, phi scratch inside K_RAS
+    void* io_a = nullptr;          // canonical-layout staging for the ABI calls
+    void* io_b = nullptr;
+    wc::Scalars* sc32 = nullptr;   // device scalars of the inner solver
+    wc::Scalars* sc64 = nullptr;   // device scalars of the outer solver
+    wc::Scalars* sc_host = nullptr;  // pinned
+    double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
+    unsigned* ticket = nullptr;
+    // timing
+    int timing = 0;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_class;
+    size_t ev_used = 0;
+    double ms_class[TC_COUNT] = {0, 0, 0, 0};
+    long long launches = 0;
+    // counters of the running solve
+    int dv32 = 0, dv64 = 0, block_dv = 0, ras_applies = 0;
+    char err[512] = {0};
+
+    template <typename T> wc::Fields<T> fields() const;
+};
+template <> inline wc::Fields<float> wcras_ctx::fields<float>() const { return wc::Fields<float>{g32a, g32b, c32}; }
+template <> inline wc::Fields<double> wcras_ctx::fields<double>() const { return wc::Fields<double>{g64, c64}; }
+
+#define WC_CUDA(call)                                                                                   \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            snprintf(ctx->err, sizeof ctx->err, "%s:%d: %s: %s", __FILE__, __LINE__, #call,             \
+                     cudaGetErrorString(e_));                                                           \
+            return WCRAS_CUDA_ERROR;                                                                    \
+        }                                                                                               \
+    } while (0)
+
+#define WC_CHECK_LAUNCH() WC_CUDA(cudaGetLastError())
+
+// scoped per-class timing (events only when ctx->timing)
+struct TimedRegion {
+    wcras_ctx* ctx;
+    bool on;
+    TimedRegion(wcras_ctx* c, int cls);
+    ~TimedRegion();
+};
+
+// ---- host entry points implemented across the .cu files ----
+namespace wc {
+constexpr int RED_BLOCKS = 592;  // 148 SMs x 4
+constexpr int RED_THREADS = 256;
+
+int alloc_dev(wcras_ctx* ctx, void** p, size_t bytes);
+int ensure_workspace(wcras_ctx* ctx);
+
+// layout.cu
+int setup_fields(wcras_ctx* ctx, const double* gauge_dev);
+int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal);
+int from_internal(wcras_ctx* ctx, int prec, const void* internal, void* canonical);
+int export_clover(wcras_ctx* ctx, double* out_dev);
+
+// dslash.cu : out = D in   or   out = b - D in (b may alias out)
+template <typename T>
+int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>::type* out,
+           const typename VecOf<T>::type* b_minus = nullptr);
+template <typename T>
+int dslash_box(wcras_ctx* ctx, const int start[4], const int ext[4], bool all_blocks,
+               const typename VecOf<T>::type* in, typename VecOf<T>::type* out);
+
+// ras.cu
+int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras);
+int ras_apply(wcras_ctx* ctx, const float4* r, float4* v);  // v = K_RAS r, internal layout; r is preserved
+int ras_block_solve(wcras_ctx* ctx, const float4* r, float4* v);
+
+// solver.cu
+int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info);
+int time_blas(wcras_ctx* ctx, int reps, double* ms);
+}  // namespace wc
