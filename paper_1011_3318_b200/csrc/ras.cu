@@ -199,7 +199,7 @@ int add_f(wcras_ctx* ctx, float4* x, const float4* y) {
     return WCRAS_OK;
 }
 
-int ras_fused_supported(const wcras_ctx* ctx, const int b[4], const int ext[4], int s);
+int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], int s, int niter, FusedGeom* out);
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
@@ -215,7 +215,8 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         rc.nd *= rc.nblk[mu]; rc.nloc *= rc.ext[mu];
     }
     rc.s = s; rc.niter = niter; rc.nras = nras; rc.set = true;
-    const bool fused_ok = ras_fused_supported(ctx, rc.b, rc.ext, s) != 0;
+    FusedGeom fgeom;
+    const bool fused_ok = ctx->tier_request != 1 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
     if (ctx->tier_request == 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
     rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
     if (int e = ensure_workspace(ctx)) return e;
@@ -233,6 +234,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * niter));
     }
     ctx->ras = rc;
+    if (rc.tier == 2) ctx->fused = fgeom;
     return WCRAS_OK;
 }
 

@@ -1,9 +1,373 @@
-// ras_fused.cu -- tier 2 of the RAS block solver (north_star (c)): placeholder until the on-chip solver lands.
+// ras_fused.cu -- tier 2 of the RAS block solver (north_star (c)): the whole block solve of one domain runs on
+// chip in ONE launch.  Steps A2-A4 of SURVEY.md 8(a): projection P_Omega' r (Alg.1 line 4), N_dominv
+// MR iterations on D_Omega' v = P r with Dirichlet boundaries (readings Q7, Q9), restriction
+// R_Omega and the disjoint sum, optionally fused with phi += v (Alg.1 line 9).
+//
+// Mapping (north_star: "domains map onto CTAs or thread-block clusters"):
+//   * The extended domain Omega' (extents ext[mu]) is cut into c[0] x c[1] x c[2] x c[3] sub-blocks of shape
+//     sb[mu] = ext[mu]/c[mu] with at most 256 sites each; one CTA per sub-block, one thread per site, and the
+//     C = prod c[mu] <= 16 CTAs of a domain form one thread-block cluster (C = 1: a plain CTA).
+//   * Per thread, for the whole solve, IN REGISTERS: its 4 forward links U_mu(x) (72 reals), its clover
+//     blocks A(x) (72 reals), the MR residual rho(x) and the iterate v(x) (24 reals each).  Links and clover
+//     are read from HBM exactly once per block solve.
+//   * Only projected half spinors (12 reals) travel between sites, through shared memory: in every MR
+//     iteration site x scatters P^-_mu rho(x) to x-mu and U_mu(x)^dag P^+_mu rho(x) to x+mu (8 x 48 B), then
+//     gathers its own 8 slots, multiplies the forward ones by its own links and reconstructs.  A neighbour in
+//     another CTA of the cluster is reached with st.shared::cluster (DSMEM); a neighbour outside Omega' is
+//     never written and its slot stays zero = Dirichlet boundary.  Wrap-around inside Omega' (ext = L) is kept.
+//   * The domain-local dots <q,rho>, <q,q> go warp shuffle -> one float4 per warp pushed to every CTA of the
+//     cluster -> summed in a fixed order by every warp after the barrier (deterministic, no atomics).
+//   * Two barriers per MR iteration (barrier.cluster arrive/wait when C > 1, bar.sync when C = 1).
+// Shared memory per CTA: 8 x 3 float4 x 256 = 96 KB of half-spinor slots + 2 KB of dot partials.
+// Roofline: HBM floor = (96 + 576) B per extended site in + 96 B per bulk site out; the N_dominv sweeps are bound
+// by fp32 issue (~1.3 k instructions per site-sweep) and shared-memory traffic (768 B per site-sweep).
 #include "wcras_internal.cuh"
+
 namespace wc {
-int ras_fused_supported(const wcras_ctx*, const int*, const int*, int) { return 0; }
-int ras_fused_block_solve(wcras_ctx* ctx, const float4*, float4*, bool) {
-    snprintf(ctx->err, sizeof ctx->err, "fused tier not available");
-    return WCRAS_UNSUPPORTED;
+
+constexpr int FUSED_MAX_THREADS = 256;
+constexpr int FUSED_MAX_CLUSTER = 16;
+
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned cluster_rank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
 }
+__device__ __forceinline__ unsigned map_to_rank(unsigned addr, unsigned rank) {
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f4(unsigned addr, float a, float b, float c, float d) {
+    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void st_local_f4(unsigned addr, float a, float b, float c, float d) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+template <bool CL> __device__ __forceinline__ void barrier_arrive() {
+    if (CL) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+template <bool CL> __device__ __forceinline__ void barrier_wait() {
+    if (CL) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    else __syncthreads();
+}
+
+// 12 reals -> slot (3 float4 with a stride of nsp float4); NONE = no receiver (Dirichlet)
+constexpr unsigned NO_DST = 0xffffffffu;
+template <bool CL>
+__device__ __forceinline__ void st_half(unsigned dst, unsigned chunk_bytes, const float* h) {
+    if (dst == NO_DST) return;
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        if (CL) st_cluster_f4(dst + j * chunk_bytes, h[4 * j], h[4 * j + 1], h[4 * j + 2], h[4 * j + 3]);
+        else st_local_f4(dst + j * chunk_bytes, h[4 * j], h[4 * j + 1], h[4 * j + 2], h[4 * j + 3]);
+    }
+}
+__device__ __forceinline__ void ld_half(const float4* __restrict__ slot, int nsp, float* h) {
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const float4 v = slot[j * nsp];
+        h[4 * j] = v.x; h[4 * j + 1] = v.y; h[4 * j + 2] = v.z; h[4 * j + 3] = v.w;
+    }
+}
+
+template <bool CL>
+__global__ void __launch_bounds__(FUSED_MAX_THREADS, 1)
+ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum) {
+    extern __shared__ float4 smem[];
+    const int nsp = fg.nsp;                 // threads per CTA = slots per chunk
+    float4* hbuf = smem;                    // [8][3][nsp]
+    float4* red = smem + 24 * nsp;          // [C * nwarps]
+    const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
+    const unsigned rank = CL ? cluster_rank() : 0u;
+    const int dom = CL ? blockIdx.x / fg.C : blockIdx.x;
+    const bool active = k < fg.ns;
+
+    // ---- geometry of this thread's site ----
+    int lc[4], sc[4], ec[4];                // coords in the sub-block, of the sub-block, in Omega'
+    {
+        int kk = active ? k : 0, rr = (int)rank;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            lc[mu] = kk % fg.sb[mu]; kk /= fg.sb[mu];
+            sc[mu] = rr % fg.c[mu]; rr /= fg.c[mu];
+            ec[mu] = sc[mu] * fg.sb[mu] + lc[mu];
+        }
+    }
+    size_t gi;       // global site index
+    bool bulk = active;
+    {
+        int d = dom, x[4];
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int bc = d % fg.nblk[mu];
+            d /= fg.nblk[mu];
+            int st = bc * fg.b[mu] - (fg.split[mu] ? fg.s : 0) + ec[mu];
+            if (st < 0) st += fg.L[mu];
+            if (st >= fg.L[mu]) st -= fg.L[mu];
+            x[mu] = st;
+            if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
+        }
+        gi = x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3]));
+    }
+    // destination slot of the half spinor sent in direction (mu, -) [index 2mu: receiver x-mu uses it for its
+    // forward hop] and (mu, +) [index 2mu+1: receiver x+mu, backward hop]
+    const unsigned chunk_bytes = (unsigned)nsp * 16u;
+    unsigned dst[8];
+    {
+        const unsigned base = smem_u32(hbuf);
+        int lstride = 1, cstride = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+#pragma unroll
+            for (int sg = 0; sg < 2; sg++) {  // sg 0: receiver x-mu, sg 1: receiver x+mu
+                int kd = k, rk = (int)rank;
+                bool ok = active;
+                if (sg == 0) {
+                    if (lc[mu] > 0) kd -= lstride;
+                    else {
+                        kd += (fg.sb[mu] - 1) * lstride;
+                        if (sc[mu] > 0) rk -= cstride;
+                        else if (fg.wrap[mu]) rk += (fg.c[mu] - 1) * cstride;
+                        else ok = false;
+                    }
+                } else {
+                    if (lc[mu] + 1 < fg.sb[mu]) kd += lstride;
+                    else {
+                        kd -= (fg.sb[mu] - 1) * lstride;
+                        if (sc[mu] + 1 < fg.c[mu]) rk += cstride;
+                        else if (fg.wrap[mu]) rk -= (fg.c[mu] - 1) * cstride;
+                        else ok = false;
+                    }
+                }
+                unsigned a = base + (unsigned)((2 * mu + sg) * 3 * nsp + kd) * 16u;
+                if (CL) a = map_to_rank(a, (unsigned)rk);
+                dst[2 * mu + sg] = ok ? a : NO_DST;
+            }
+            lstride *= fg.sb[mu];
+            cstride *= fg.c[mu];
+        }
+    }
+
+    // ---- zero the slots (Dirichlet faces are never written), load the site data ----
+#pragma unroll
+    for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float U[72], A[72], rho[24], v[24];
+    if (active) {
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) load_link(f, (size_t)fg.V, gi, mu, U + 18 * mu);
+        load_clover(f, (size_t)fg.V, gi, A);
+        load_spinor(r, (size_t)fg.V, gi, rho);  // projection P_Omega' r
+    } else {
+#pragma unroll
+        for (int n = 0; n < 72; n++) { U[n] = 0.f; A[n] = 0.f; }
+#pragma unroll
+        for (int n = 0; n < 24; n++) rho[n] = 0.f;
+    }
+#pragma unroll
+    for (int n = 0; n < 24; n++) v[n] = 0.f;
+    barrier_arrive<CL>();
+    barrier_wait<CL>();
+
+    for (int it = 0; it < fg.niter; it++) {
+        // ---- scatter: projected half spinors to the 8 neighbours ----
+        {
+            float h[12], g[12];
+#define WC_SCATTER(MU)                                            \
+    project<float, MU, -1>(rho, h);                               \
+    st_half<CL>(dst[2 * MU], chunk_bytes, h);                     \
+    project<float, MU, +1>(rho, h);                               \
+    su3_adj_mul<float>(U + 18 * MU, h, g);                        \
+    st_half<CL>(dst[2 * MU + 1], chunk_bytes, g);
+            WC_SCATTER(0) WC_SCATTER(1) WC_SCATTER(2) WC_SCATTER(3)
+#undef WC_SCATTER
+        }
+        barrier_arrive<CL>();
+        float q[24];
+        clover_apply<float>(A, rho, q);  // independent of the exchange: overlaps the barrier
+        barrier_wait<CL>();
+        // ---- gather: q = A rho - kappa * hop ----
+        {
+            float hop[24];
+#pragma unroll
+            for (int n = 0; n < 24; n++) hop[n] = 0.f;
+            float h[12], g[12];
+#define WC_GATHER(MU)                                             \
+    ld_half(hbuf + (2 * MU) * 3 * nsp + k, nsp, h);               \
+    su3_mul<float>(U + 18 * MU, h, g);                            \
+    reconstruct_add<float, MU, -1>(g, hop);                       \
+    ld_half(hbuf + (2 * MU + 1) * 3 * nsp + k, nsp, g);           \
+    reconstruct_add<float, MU, +1>(g, hop);
+            WC_GATHER(0) WC_GATHER(1) WC_GATHER(2) WC_GATHER(3)
+#undef WC_GATHER
+#pragma unroll
+            for (int n = 0; n < 24; n++) q[n] -= kappa * hop[n];
+        }
+        // ---- domain-local dots <q,rho>, <q,q> ----
+        float d0 = 0.f, d1 = 0.f, d2 = 0.f;
+#pragma unroll
+        for (int n = 0; n < 12; n++) {
+            const float qr = q[2 * n], qi = q[2 * n + 1], rr = rho[2 * n], ri = rho[2 * n + 1];
+            d0 += qr * rr + qi * ri;
+            d1 += qr * ri - qi * rr;
+            d2 += qr * qr + qi * qi;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            d0 += __shfl_xor_sync(0xffffffffu, d0, o);
+            d1 += __shfl_xor_sync(0xffffffffu, d1, o);
+            d2 += __shfl_xor_sync(0xffffffffu, d2, o);
+        }
+        {
+            const unsigned slot = smem_u32(red + rank * nwarps + warp);
+            if (CL) {
+                if (lane < fg.C) st_cluster_f4(map_to_rank(slot, (unsigned)lane), d0, d1, d2, 0.f);
+            } else if (lane == 0) {
+                st_local_f4(slot, d0, d1, d2, 0.f);
+            }
+        }
+        barrier_arrive<CL>();
+        barrier_wait<CL>();
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f;
+        for (int n = lane; n < fg.C * nwarps; n += 32) {
+            const float4 p = red[n];
+            s0 += p.x; s1 += p.y; s2 += p.z;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9); v += alpha rho; rho -= alpha q
+        const float ar = s2 > 0.f ? s0 / s2 : 0.f, ai = s2 > 0.f ? s1 / s2 : 0.f;
+        const bool last = it + 1 == fg.niter;
+#pragma unroll
+        for (int n = 0; n < 12; n++) {
+            const float rr = rho[2 * n], ri = rho[2 * n + 1];
+            v[2 * n] += ar * rr - ai * ri;
+            v[2 * n + 1] += ar * ri + ai * rr;
+            if (!last) {
+                rho[2 * n] = rr - (ar * q[2 * n] - ai * q[2 * n + 1]);
+                rho[2 * n + 1] = ri - (ar * q[2 * n + 1] + ai * q[2 * n]);
+            }
+        }
+    }
+    // ---- restriction R_Omega: bulk sites only; disjoint over domains, so a plain store (or phi += v) ----
+    if (bulk) {
+        if (accum) {
+            float o[24];
+            load_spinor(vout, (size_t)fg.V, gi, o);
+#pragma unroll
+            for (int n = 0; n < 24; n++) v[n] += o[n];
+        }
+        store_spinor(vout, (size_t)fg.V, gi, v);
+    }
+}
+
+// ---- host side ----
+// Choose the cut of Omega' into sub-blocks: minimal cluster size, then the most cubic sub-block.
+static bool choose_cut(const int ext[4], int c[4], int sb[4]) {
+    int best_C = 1 << 30, best_spread = 1 << 30;
+    bool found = false;
+    for (int c0 = 1; c0 <= ext[0]; c0++) if (ext[0] % c0 == 0)
+    for (int c1 = 1; c1 <= ext[1]; c1++) if (ext[1] % c1 == 0)
+    for (int c2 = 1; c2 <= ext[2]; c2++) if (ext[2] % c2 == 0)
+    for (int c3 = 1; c3 <= ext[3]; c3++) if (ext[3] % c3 == 0) {
+        const int cc[4] = {c0, c1, c2, c3};
+        long C = (long)c0 * c1 * c2 * c3, ns = 1;
+        int mx = 0, mn = 1 << 30;
+        for (int mu = 0; mu < 4; mu++) {
+            const int e = ext[mu] / cc[mu];
+            ns *= e; mx = e > mx ? e : mx; mn = e < mn ? e : mn;
+        }
+        if (C > FUSED_MAX_CLUSTER || ns > FUSED_MAX_THREADS) continue;
+        const int spread = mx - mn;
+        if (C < best_C || (C == best_C && spread < best_spread)) {
+            best_C = (int)C; best_spread = spread; found = true;
+            for (int mu = 0; mu < 4; mu++) { c[mu] = cc[mu]; sb[mu] = ext[mu] / cc[mu]; }
+        }
+    }
+    return found;
+}
+
+static FusedGeom make_fused_geom(const wcras_ctx* ctx, const int b[4], const int ext[4], int s, int niter, bool* ok) {
+    FusedGeom fg;
+    *ok = choose_cut(ext, fg.c, fg.sb);
+    fg.ns = 1; fg.C = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        fg.L[mu] = ctx->geom.L[mu]; fg.b[mu] = b[mu]; fg.nblk[mu] = ctx->geom.L[mu] / b[mu]; fg.ext[mu] = ext[mu];
+        fg.split[mu] = b[mu] < ctx->geom.L[mu];
+        fg.wrap[mu] = ext[mu] == ctx->geom.L[mu];
+        if (*ok) { fg.ns *= fg.sb[mu]; fg.C *= fg.c[mu]; }
+    }
+    fg.V = ctx->geom.V; fg.s = s; fg.niter = niter;
+    fg.nsp = (fg.ns + 31) / 32 * 32;
+    return fg;
+}
+
+static size_t fused_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)24 * fg.nsp + (size_t)fg.C * (fg.nsp / 32)); }
+
+template <bool CL>
+static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
+    auto kern = ras_fused_kernel<CL>;
+    const size_t smem = fused_smem_bytes(fg);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (!CL) { *max_clusters = 1; return cudaSuccess; }
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, fg.C > 8 ? 1 : 0);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)fg.C);
+    cfg.blockDim = dim3((unsigned)fg.nsp);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)fg.C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaOccupancyMaxActiveClusters(max_clusters, kern, &cfg);
+}
+
+template <bool CL>
+static cudaError_t launch_fused(const FusedGeom& fg, int nd, cudaStream_t stream, const Fields<float>& f, float kappa,
+                                const float4* r, float4* vout, int accum) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)nd * fg.C);
+    cfg.blockDim = dim3((unsigned)fg.nsp);
+    cfg.dynamicSmemBytes = fused_smem_bytes(fg);
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)fg.C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = CL ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, f, kappa, r, vout, accum);
+}
+
+// Fill *out and return 1 if the extended domain fits the fused tier on this device: a cut into <= 16 sub-blocks of
+// <= 256 sites exists and the cluster can be scheduled (cudaOccupancyMaxActiveClusters > 0).
+int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], int s, int niter, FusedGeom* out) {
+    bool ok;
+    const FusedGeom fg = make_fused_geom(ctx, b, ext, s, niter, &ok);
+    if (!ok) return 0;
+    int nclusters = 0;
+    const cudaError_t e = fg.C > 1 ? prepare_fused<true>(fg, &nclusters) : prepare_fused<false>(fg, &nclusters);
+    if (e != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (nclusters < 1) return 0;
+    *out = fg;
+    return 1;
+}
+
+int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
+    const FusedGeom& fg = ctx->fused;
+    const Fields<float> f = ctx->fields<float>();
+    if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
+    else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
+    ctx->launches++;
+    return WCRAS_OK;
+}
+
 }  // namespace wc

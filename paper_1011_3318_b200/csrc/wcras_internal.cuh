@@ -118,6 +118,14 @@ struct Scalars {
 }  // namespace wc
 
 // ---- RAS configuration ----
+// geometry of the fused on-chip block solver (ras_fused.cu)
+struct FusedGeom {
+    int L[4], b[4], nblk[4], ext[4], sb[4], c[4];
+    int split[4];  // b < L: direction is cut, Omega' extended by s per side, Dirichlet unless ext == L
+    int wrap[4];   // ext == L: hops across the domain edge stay inside Omega' (Q7)
+    int V, s, ns, nsp, C, niter;
+};
+
 struct RasConfig {
     bool set = false;
     int b[4] = {0, 0, 0, 0};      // block shape
@@ -144,6 +152,7 @@ struct wcras_ctx {
     // RAS
     RasConfig ras;
     int tier_request = 0;
+    FusedGeom fused;               // valid when ras.tier == 2
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
     double* mr_scal = nullptr;                                     // [niter][nd][4]
     // solver parameters
