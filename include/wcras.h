@@ -80,7 +80,9 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 
 /* Block-solver tier: 0 = automatic (fused on-chip solver when the extended domain fits, else generic),
  * 1 = generic global-memory tier, 2 = fused tier (WCRAS_UNSUPPORTED at the next wcras_ras_precondition if
- * the shape does not fit).  Call before wcras_ras_precondition. */
+ * the shape does not fit; extended domains of <= 256 sites use the persistent one-CTA-per-domain kernel,
+ * larger ones a thread-block cluster per domain), 3 = fused tier, cluster kernel forced (for checking).
+ * Call before wcras_ras_precondition. */
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
 
 /* out = P'^T D_Omega' P' in : the principal sub-matrix of D on the extended domain Omega'_index of the

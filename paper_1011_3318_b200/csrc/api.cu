@@ -51,6 +51,7 @@ int wcras_destroy(wcras_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
+    if (ctx->dm) cudaFree(ctx->dm);
     if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
@@ -77,7 +78,7 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     NEED(ctx, "null ctx");
-    NEED(tier >= 0 && tier <= 2, "set_ras_tier: tier must be 0, 1 or 2");
+    NEED(tier >= 0 && tier <= 3, "set_ras_tier: tier must be 0..3");
     ctx->tier_request = tier;
     return WCRAS_OK;
 }

@@ -201,6 +201,8 @@ int add_f(wcras_ctx* ctx, float4* x, const float4* y) {
 
 int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], int s, int niter, FusedGeom* out);
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd);
+int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
     RasConfig rc;
@@ -217,7 +219,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     rc.s = s; rc.niter = niter; rc.nras = nras; rc.set = true;
     FusedGeom fgeom;
     const bool fused_ok = ctx->tier_request != 1 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
-    if (ctx->tier_request == 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
+    if (ctx->tier_request >= 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
     rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
     if (int e = ensure_workspace(ctx)) return e;
     // per-domain workspace of the generic tier (kept even when the fused tier is active: cheap to hold)
@@ -233,8 +235,16 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         WC_CUDA(cudaMalloc((void**)&ctx->mr_v, nb));
         WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * niter));
     }
+    if (ctx->dm) {
+        WC_CUDA(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->dm);
+        ctx->dm = nullptr;
+    }
+    if (rc.tier == 2) {
+        ctx->fused = fgeom;
+        rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
+    }
     ctx->ras = rc;
-    if (rc.tier == 2) ctx->fused = fgeom;
     return WCRAS_OK;
 }
 
@@ -267,6 +277,7 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
 static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     TimedRegion tr(ctx, TC_BLOCK);
     ctx->block_dv += ctx->ras.niter;
+    if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);
     if (ctx->ras.tier == 2) return ras_fused_block_solve(ctx, r, vout, accum);
     return generic_block_solve(ctx, r, vout, accum);
 }

@@ -1,0 +1,292 @@
+// ras_cta.cu -- tier 2a of the RAS block solver (north_star (c)): extended domains of at most 256 sites, one CTA
+// per domain, PERSISTENT: each CTA walks over domains dom = blockIdx.x, blockIdx.x + gridDim.x, ... and, while it
+// runs the MR sweeps of one domain on chip, the data of its next domain is pulled from HBM into L2
+// (cp.async.bulk.prefetch.L2 on the contiguous domain-major block + prefetch.global.L2 on the residual rows), so
+// HBM streams continuously behind the arithmetic.  Steps A2-A4 of SURVEY.md 8(a): projection P_Omega' r
+// (Alg.1 line 4), N_dominv MR iterations on D_Omega' v = P r with Dirichlet boundaries (PAPER.md:68,
+// :83; readings Q7, Q9), restriction R_Omega and the disjoint sum, optionally phi += v (line 9).
+//
+//   * Domain-major operand copy (built once in wcras_ras_precondition): dm = float4 [nd][36][nsp]; chunks 0..17 are
+//     the 72 reals of the four forward links of the site PRE-SCALED by -kappa, chunks 18..35 the packed clover
+//     blocks.  Thread k reads dm[(dom*36 + c)*nsp + k]: 4 KB contiguous per chunk, 147 KB contiguous per domain.
+//     This is the paper's "overlapped region data is replicated per domain" applied to the operands.
+//   * Per thread, in registers for the whole block solve: -kappa U_mu(x) (72), A(x) (72), rho(x), v(x) (24 + 24).
+//   * Per MR iteration: scatter 8 projected half spinors (backward ones pre-multiplied by -kappa U^dag) into the
+//     neighbour's slot in shared memory, q = A rho, barrier, gather the own 8 slots (forward ones multiplied by
+//     -kappa U) straight onto q.  Slots of neighbours outside Omega' are never written and stay zero = Dirichlet.
+//   * <q,rho>, <q,q>: warp shuffle -> one float4 per warp in shared memory -> fixed-order sum by every thread.
+// Shared memory: 8 x 3 float4 x nsp half-spinor slots (96 KB at nsp = 256) + nwarps float4.
+// Roofline: HBM, (96 + 576) B per extended site in + 96 B per bulk site out (768 B/site at s = 0); the sweeps
+// cost ~1.4 k fp32 instructions per site each and must hide behind that stream.
+#include "wcras_internal.cuh"
+
+namespace wc {
+
+__device__ __forceinline__ unsigned cta_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+// predicated 16-byte shared store (no branch): dst == 0xffffffff means "no receiver" (Dirichlet)
+__device__ __forceinline__ void st_pred_f4(unsigned addr, float a, float b, float c, float d) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0xffffffff;\n\t@p st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n\t}" ::"r"(addr),
+        "f"(a), "f"(b), "f"(c), "f"(d)
+        : "memory");
+}
+__device__ __forceinline__ void st_half_pred(unsigned dst, unsigned chunk_bytes, const float* h) {
+    const unsigned d1 = dst == 0xffffffffu ? dst : dst + chunk_bytes;
+    const unsigned d2 = dst == 0xffffffffu ? dst : dst + 2 * chunk_bytes;
+    st_pred_f4(dst, h[0], h[1], h[2], h[3]);
+    st_pred_f4(d1, h[4], h[5], h[6], h[7]);
+    st_pred_f4(d2, h[8], h[9], h[10], h[11]);
+}
+__device__ __forceinline__ void ld_half_cta(const float4* __restrict__ slot, int nsp, float* h) {
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        const float4 v = slot[j * nsp];
+        h[4 * j] = v.x; h[4 * j + 1] = v.y; h[4 * j + 2] = v.z; h[4 * j + 3] = v.w;
+    }
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// global site index of local site (lc) of domain dom; bulk = belongs to the non-overlapping block
+__device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const int lc[4]) {
+    int x[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        const int bc = dom % fg.nblk[mu];
+        dom /= fg.nblk[mu];
+        int st = bc * fg.b[mu] - (fg.split[mu] ? fg.s : 0) + lc[mu];
+        if (st < 0) st += fg.L[mu];
+        if (st >= fg.L[mu]) st -= fg.L[mu];
+        x[mu] = st;
+    }
+    return x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3]));
+}
+
+// pack the domain-major operand copy: one thread per (domain, local site)
+__global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, float mkappa, float4* __restrict__ dm) {
+    const int dom = blockIdx.x, k = threadIdx.x;
+    if (dom >= nd) return;
+    float4* out = dm + (size_t)dom * 36 * fg.nsp + k;
+    if (k >= fg.ns) {
+        for (int c = 0; c < 36; c++) out[(size_t)c * fg.nsp] = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    int lc[4], kk = k;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) { lc[mu] = kk % fg.ext[mu]; kk /= fg.ext[mu]; }
+    const size_t gi = cta_site(fg, dom, lc), V = fg.V;
+    float u[72];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) load_link(f, V, gi, mu, u + 18 * mu);
+#pragma unroll
+    for (int c = 0; c < 18; c++)
+        out[(size_t)c * fg.nsp] = make_float4(mkappa * u[4 * c], mkappa * u[4 * c + 1], mkappa * u[4 * c + 2], mkappa * u[4 * c + 3]);
+#pragma unroll
+    for (int c = 0; c < 18; c++) out[(size_t)(18 + c) * fg.nsp] = f.cl[(size_t)c * V + gi];
+}
+
+__global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
+ras_cta_kernel(FusedGeom fg, int nd, const float4* __restrict__ dm, const float4* __restrict__ r, float4* __restrict__ vout,
+               int accum) {
+    extern __shared__ float4 smem[];
+    const int nsp = fg.nsp;
+    float4* hbuf = smem;            // [8][3][nsp]
+    float4* red = smem + 24 * nsp;  // [nwarps]
+    const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
+    const bool active = k < fg.ns;
+
+    // ---- domain-independent geometry: local coordinates, bulk flag, destination slots ----
+    int lc[4];
+    bool bulk = active;
+    {
+        int kk = active ? k : 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            lc[mu] = kk % fg.ext[mu]; kk /= fg.ext[mu];
+            if (fg.split[mu]) bulk = bulk && lc[mu] >= fg.s && lc[mu] < fg.s + fg.b[mu];
+        }
+    }
+    const unsigned chunk_bytes = (unsigned)nsp * 16u;
+    unsigned dst[8];  // slot 2mu: receiver x-mu (its forward hop); slot 2mu+1: receiver x+mu (its backward hop)
+    {
+        const unsigned base = cta_smem_u32(hbuf);
+        int lstride = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int e = fg.ext[mu];
+            int kd = k - lstride;
+            bool ok = active;
+            if (lc[mu] == 0) { kd = k + (e - 1) * lstride; ok = ok && fg.wrap[mu]; }
+            dst[2 * mu] = ok ? base + (unsigned)((2 * mu) * 3 * nsp + kd) * 16u : 0xffffffffu;
+            kd = k + lstride;
+            ok = active;
+            if (lc[mu] + 1 == e) { kd = k - (e - 1) * lstride; ok = ok && fg.wrap[mu]; }
+            dst[2 * mu + 1] = ok ? base + (unsigned)((2 * mu + 1) * 3 * nsp + kd) * 16u : 0xffffffffu;
+            lstride *= e;
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+
+    const size_t V = fg.V;
+    const unsigned dm_bytes = 36u * (unsigned)nsp * 16u;
+    for (int dom = blockIdx.x; dom < nd; dom += gridDim.x) {
+        const size_t gi = cta_site(fg, dom, lc);
+        float U[72], A[72], rho[24], v[24];
+        {
+            const float4* p = dm + (size_t)dom * 36 * nsp + k;
+#pragma unroll
+            for (int c = 0; c < 18; c++) {
+                const float4 t = __ldcs(p + (size_t)c * nsp);
+                U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;
+            }
+            if (active) {
+#pragma unroll
+                for (int c = 0; c < 6; c++) {
+                    const float4 t = r[(size_t)c * V + gi];
+                    rho[4 * c] = t.x; rho[4 * c + 1] = t.y; rho[4 * c + 2] = t.z; rho[4 * c + 3] = t.w;
+                }
+            } else {
+#pragma unroll
+                for (int n = 0; n < 24; n++) rho[n] = 0.f;
+            }
+#pragma unroll
+            for (int c = 0; c < 18; c++) {
+                const float4 t = __ldcs(p + (size_t)(18 + c) * nsp);
+                A[4 * c] = t.x; A[4 * c + 1] = t.y; A[4 * c + 2] = t.z; A[4 * c + 3] = t.w;
+            }
+        }
+        // ---- pull the next domain of this CTA towards L2 while this one is solved ----
+        {
+            const int nxt = dom + gridDim.x;
+            if (nxt < nd) {
+                if (k == 0) prefetch_l2_bulk(dm + (size_t)nxt * 36 * nsp, dm_bytes);
+                if (active) {
+                    const size_t gn = cta_site(fg, nxt, lc);
+#pragma unroll
+                    for (int c = 0; c < 6; c++) prefetch_l2(r + (size_t)c * V + gn);
+                }
+            }
+        }
+#pragma unroll
+        for (int n = 0; n < 24; n++) v[n] = 0.f;
+
+        for (int it = 0; it < fg.niter; it++) {
+            {
+                float h[12], g[12];
+#define WC_SCATTER(MU)                                       \
+    project<float, MU, -1>(rho, h);                          \
+    st_half_pred(dst[2 * MU], chunk_bytes, h);               \
+    project<float, MU, +1>(rho, h);                          \
+    su3_adj_mul<float>(U + 18 * MU, h, g);                   \
+    st_half_pred(dst[2 * MU + 1], chunk_bytes, g);
+                WC_SCATTER(0) WC_SCATTER(1) WC_SCATTER(2) WC_SCATTER(3)
+#undef WC_SCATTER
+            }
+            float q[24];
+            clover_apply<float>(A, rho, q);
+            __syncthreads();
+            {
+                float h[12], g[12];
+#define WC_GATHER(MU)                                        \
+    ld_half_cta(hbuf + (2 * MU) * 3 * nsp + k, nsp, h);      \
+    su3_mul<float>(U + 18 * MU, h, g);                       \
+    reconstruct_add<float, MU, -1>(g, q);                    \
+    ld_half_cta(hbuf + (2 * MU + 1) * 3 * nsp + k, nsp, g);  \
+    reconstruct_add<float, MU, +1>(g, q);
+                WC_GATHER(0) WC_GATHER(1) WC_GATHER(2) WC_GATHER(3)
+#undef WC_GATHER
+            }
+            float d0 = 0.f, d1 = 0.f, d2 = 0.f;
+#pragma unroll
+            for (int n = 0; n < 12; n++) {
+                const float qr = q[2 * n], qi = q[2 * n + 1], rr = rho[2 * n], ri = rho[2 * n + 1];
+                d0 = fmaf(qr, rr, d0); d0 = fmaf(qi, ri, d0);
+                d1 = fmaf(qr, ri, d1); d1 = fmaf(-qi, rr, d1);
+                d2 = fmaf(qr, qr, d2); d2 = fmaf(qi, qi, d2);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                d0 += __shfl_xor_sync(0xffffffffu, d0, o);
+                d1 += __shfl_xor_sync(0xffffffffu, d1, o);
+                d2 += __shfl_xor_sync(0xffffffffu, d2, o);
+            }
+            if (lane == 0) red[warp] = make_float4(d0, d1, d2, 0.f);
+            __syncthreads();
+            float s0 = 0.f, s1 = 0.f, s2 = 0.f;
+            for (int n = 0; n < nwarps; n++) {
+                const float4 p = red[n];
+                s0 += p.x; s1 += p.y; s2 += p.z;
+            }
+            // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9); v += alpha rho; rho -= alpha q
+            const float inv = s2 > 0.f ? 1.f / s2 : 0.f;
+            const float ar = s0 * inv, ai = s1 * inv;
+            const bool last = it + 1 == fg.niter;
+#pragma unroll
+            for (int n = 0; n < 12; n++) {
+                const float rr = rho[2 * n], ri = rho[2 * n + 1];
+                v[2 * n] = fmaf(ar, rr, v[2 * n]); v[2 * n] = fmaf(-ai, ri, v[2 * n]);
+                v[2 * n + 1] = fmaf(ar, ri, v[2 * n + 1]); v[2 * n + 1] = fmaf(ai, rr, v[2 * n + 1]);
+                if (!last) {
+                    rho[2 * n] = fmaf(-ar, q[2 * n], rr); rho[2 * n] = fmaf(ai, q[2 * n + 1], rho[2 * n]);
+                    rho[2 * n + 1] = fmaf(-ar, q[2 * n + 1], ri); rho[2 * n + 1] = fmaf(-ai, q[2 * n], rho[2 * n + 1]);
+                }
+            }
+        }
+        // ---- restriction R_Omega: bulk sites only; disjoint over domains, so a plain store (or phi += v) ----
+        if (bulk) {
+            if (accum) {
+#pragma unroll
+                for (int c = 0; c < 6; c++) {
+                    const float4 o = vout[(size_t)c * V + gi];
+                    v[4 * c] += o.x; v[4 * c + 1] += o.y; v[4 * c + 2] += o.z; v[4 * c + 3] += o.w;
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 6; c++)
+                __stcs(vout + (size_t)c * V + gi, make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]));
+        }
+    }
+}
+
+// ---- host side ----
+static size_t cta_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)24 * fg.nsp + fg.nsp / 32); }
+
+// allocate and fill the domain-major operand copy; sets ctx->dm and the persistent grid size
+int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
+    if (fg.C != 1 || fg.nsp > FUSED_CTA_MAX_THREADS) return 0;
+    const size_t smem = cta_smem_bytes(fg);
+    if (cudaFuncSetAttribute(ras_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    int per_sm = 0, dev = 0, sms = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta_kernel, fg.nsp, smem) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return 0;
+    }
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (ctx->dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm); ctx->dm = nullptr; }
+    const size_t bytes = sizeof(float4) * 36 * (size_t)fg.nsp * nd;
+    if (cudaMalloc((void**)&ctx->dm, bytes) != cudaSuccess) { cudaGetLastError(); ctx->dm = nullptr; return 0; }
+    pack_domain_major_kernel<<<nd, fg.nsp, 0, ctx->stream>>>(fg, nd, ctx->fields<float>(), -(float)ctx->kappa, ctx->dm);
+    ctx->launches++;
+    if (cudaGetLastError() != cudaSuccess) return 0;
+    const long want = (long)per_sm * sms;
+    ctx->cta_grid = (int)(nd < want ? nd : want);
+    return 1;
+}
+
+int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
+    const FusedGeom& fg = ctx->fused;
+    ras_cta_kernel<<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(fg, ctx->ras.nd, ctx->dm, r, vout, accum ? 1 : 0);
+    ctx->launches++;
+    WC_CHECK_LAUNCH();
+    return WCRAS_OK;
+}
+
+}  // namespace wc

@@ -79,6 +79,11 @@ WC_HD void reconstruct_add(const T* __restrict__ g, T* __restrict__ acc) {
     }
 }
 
+// Explicit fused multiply-add chains: written out because the compiler may not re-associate
+// "re += ur*hr - ui*hi" into two FMAs on the accumulator (it emits FMUL + FFMA + FADD instead).
+WC_HD float wc_fma(float a, float b, float c) { return fmaf(a, b, c); }
+WC_HD double wc_fma(double a, double b, double c) { return fma(a, b, c); }
+
 // g = U h  (both half-spin components)
 template <typename T>
 WC_HD void su3_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restrict__ g) {
@@ -86,13 +91,18 @@ WC_HD void su3_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restri
     for (int hs = 0; hs < 2; hs++)
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            T re = 0, im = 0;
+            const T* ua = u + a * 6;
+            const T* hh = h + hs * 6;
+            T re = ua[0] * hh[0];
+            T im = ua[0] * hh[1];
+            re = wc_fma(-ua[1], hh[1], re);
+            im = wc_fma(ua[1], hh[0], im);
 #pragma unroll
-            for (int b = 0; b < 3; b++) {
-                const T ur = u[(a * 3 + b) * 2], ui = u[(a * 3 + b) * 2 + 1];
-                const T hr = h[(hs * 3 + b) * 2], hi = h[(hs * 3 + b) * 2 + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+            for (int b = 1; b < 3; b++) {
+                re = wc_fma(ua[2 * b], hh[2 * b], re);
+                im = wc_fma(ua[2 * b], hh[2 * b + 1], im);
+                re = wc_fma(-ua[2 * b + 1], hh[2 * b + 1], re);
+                im = wc_fma(ua[2 * b + 1], hh[2 * b], im);
             }
             g[(hs * 3 + a) * 2] = re;
             g[(hs * 3 + a) * 2 + 1] = im;
@@ -106,13 +116,19 @@ WC_HD void su3_adj_mul(const T* __restrict__ u, const T* __restrict__ h, T* __re
     for (int hs = 0; hs < 2; hs++)
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            T re = 0, im = 0;
+            const T* hh = h + hs * 6;
+            // (U^dag)_ab = conj(U_ba): real part u[(b*3+a)*2], imaginary part -u[(b*3+a)*2+1]
+            T re = u[a * 2] * hh[0];
+            T im = u[a * 2] * hh[1];
+            re = wc_fma(u[a * 2 + 1], hh[1], re);
+            im = wc_fma(-u[a * 2 + 1], hh[0], im);
 #pragma unroll
-            for (int b = 0; b < 3; b++) {
-                const T ur = u[(b * 3 + a) * 2], ui = -u[(b * 3 + a) * 2 + 1];
-                const T hr = h[(hs * 3 + b) * 2], hi = h[(hs * 3 + b) * 2 + 1];
-                re += ur * hr - ui * hi;
-                im += ur * hi + ui * hr;
+            for (int b = 1; b < 3; b++) {
+                const T ur = u[(b * 3 + a) * 2], ui = u[(b * 3 + a) * 2 + 1];
+                re = wc_fma(ur, hh[2 * b], re);
+                im = wc_fma(ur, hh[2 * b + 1], im);
+                re = wc_fma(ui, hh[2 * b + 1], re);
+                im = wc_fma(-ui, hh[2 * b], im);
             }
             g[(hs * 3 + a) * 2] = re;
             g[(hs * 3 + a) * 2 + 1] = im;
@@ -147,12 +163,16 @@ WC_HD void herm6_mul(const T* __restrict__ b, const T* __restrict__ x, T* __rest
         for (int j = 0; j < 6; j++) {
             if (j < i) {  // A_ij, stored
                 const int k = 6 + 2 * (i * (i - 1) / 2 + j);
-                re += b[k] * x[2 * j] - b[k + 1] * x[2 * j + 1];
-                im += b[k] * x[2 * j + 1] + b[k + 1] * x[2 * j];
+                re = wc_fma(b[k], x[2 * j], re);
+                im = wc_fma(b[k], x[2 * j + 1], im);
+                re = wc_fma(-b[k + 1], x[2 * j + 1], re);
+                im = wc_fma(b[k + 1], x[2 * j], im);
             } else if (j > i) {  // A_ij = conj(A_ji)
                 const int k = 6 + 2 * (j * (j - 1) / 2 + i);
-                re += b[k] * x[2 * j] + b[k + 1] * x[2 * j + 1];
-                im += b[k] * x[2 * j + 1] - b[k + 1] * x[2 * j];
+                re = wc_fma(b[k], x[2 * j], re);
+                im = wc_fma(b[k], x[2 * j + 1], im);
+                re = wc_fma(b[k + 1], x[2 * j + 1], re);
+                im = wc_fma(-b[k + 1], x[2 * j], im);
             }
         }
         out[2 * i] = re;

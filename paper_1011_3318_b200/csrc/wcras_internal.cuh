@@ -135,7 +135,9 @@ struct RasConfig {
     int nd = 0;                   // number of domains
     int nloc = 0;                 // sites per extended domain
     int tier = 1;                 // 1 generic, 2 fused
+    bool cta = false;             // fused tier, single persistent CTA per domain (ras_cta.cu)
 };
+constexpr int FUSED_CTA_MAX_THREADS = 256;
 
 enum TimeClass { TC_DSLASH = 0, TC_BLOCK = 1, TC_BLAS = 2, TC_DSLASH64 = 3, TC_COUNT = 4 };
 
@@ -153,6 +155,8 @@ struct wcras_ctx {
     RasConfig ras;
     int tier_request = 0;
     FusedGeom fused;               // valid when ras.tier == 2
+    float4* dm = nullptr;          // domain-major operand copy of the persistent-CTA tier: [nd][36][nsp]
+    int cta_grid = 0;              // its persistent grid size
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
     double* mr_scal = nullptr;                                     // [niter][nd][4]
     // solver parameters
