@@ -81,7 +81,10 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 /* Block-solver tier: 0 = automatic (fused on-chip solver when the extended domain fits, else generic),
  * 1 = generic global-memory tier, 2 = fused tier (WCRAS_UNSUPPORTED at the next wcras_ras_precondition if
  * the shape does not fit; extended domains of <= 256 sites use the persistent one-CTA-per-domain kernel,
- * larger ones a thread-block cluster per domain), 3 = fused tier, cluster kernel forced (for checking).
+ * larger ones a thread-block cluster per domain), 3 = fused tier, cluster kernel forced (for checking),
+ * 4 = fused tier with the NRAS cycles NOT chained (for checking).  On the persistent-CTA kernel with overlap 0
+ * the cycles of Alg.1 are chained: the MR recurrence leaves rho = r - D_Omega v on every domain, so line 9,
+ * r -= D v, only adds the hops of v that cross a domain boundary and no full-lattice D runs between cycles.
  * Call before wcras_ras_precondition. */
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
 
@@ -95,8 +98,10 @@ int wcras_apply_D_restricted(wcras_ctx* ctx, int prec, int domain_index, const v
  * block solve.  fp32, canonical layout, device. */
 int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev);
 
-/* Solver parameters (reading Q13): inner relative tolerance (default 1e-5), iteration caps (1000 / 50),
- * use_ras = 0 runs the inner solver without preconditioner ("No prec." column of Table 1). */
+/* Solver parameters (readings Q13, A2): inner_tol = the deepest relative accuracy one fp32 inner solve is asked
+ * for (default 5e-7); each inner solve gets the tolerance max(inner_tol, R^(1/n)), R = 0.5 target/|rhs|,
+ * n = ceil(log R / log inner_tol), so that the outer target is met without overshooting it.  Iteration caps
+ * (default 1000 / 50).  use_ras = 0 runs the inner solver without preconditioner ("No prec." column of Table 1). */
 int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int outer_maxit, int use_ras);
 
 /* Per-kernel-class CUDA-event timing inside wcras_solve (fills ms_dslash / ms_blocksolve / ms_blas). */

@@ -52,6 +52,7 @@ int wcras_destroy(wcras_ctx* ctx) {
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
     if (ctx->dm) cudaFree(ctx->dm);
+    if (ctx->hb) cudaFree(ctx->hb);
     if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
@@ -78,8 +79,9 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     NEED(ctx, "null ctx");
-    NEED(tier >= 0 && tier <= 3, "set_ras_tier: tier must be 0..3");
-    ctx->tier_request = tier;
+    NEED(tier >= 0 && tier <= 4, "set_ras_tier: tier must be 0..4");
+    ctx->tier_request = tier == 4 ? 2 : tier;
+    ctx->chain_cycles = tier != 4;
     return WCRAS_OK;
 }
 

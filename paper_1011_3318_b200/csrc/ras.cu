@@ -203,6 +203,7 @@ int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], in
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
     RasConfig rc;
@@ -291,6 +292,8 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     if (!rc.set) { snprintf(ctx->err, sizeof ctx->err, "ras_apply: call wcras_ras_precondition first"); return WCRAS_INVALID_ARG; }
     ctx->ras_applies++;
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
+    // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
+    if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];
     const float4* rcur = r;

@@ -50,8 +50,7 @@ __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) 
 }
 
 // global site index of local site (lc) of domain dom; bulk = belongs to the non-overlapping block
-__device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const int lc[4]) {
-    int x[4];
+__device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const int lc[4], int x[4]) {
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         const int bc = dom % fg.nblk[mu];
@@ -62,6 +61,11 @@ __device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const i
         x[mu] = st;
     }
     return x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3]));
+}
+
+__device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const int lc[4]) {
+    int x[4];
+    return cta_site(fg, dom, lc, x);
 }
 
 // pack the domain-major operand copy: one thread per (domain, local site)
@@ -87,9 +91,25 @@ __global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, 
     for (int c = 0; c < 18; c++) out[(size_t)(18 + c) * fg.nsp] = f.cl[(size_t)c * V + gi];
 }
 
+// One K_RAS cycle (Alg.1 lines 3-9) for all domains.  Cycle 0: rho = P r.  Cycles j >= 1 (CHAIN, overlap 0 only):
+// the MR recurrence of cycle j-1 left rho_fin = r_{j-1} - D_Omega v_{j-1} on every domain, so the residual update of
+// Alg.1 line 9, r_j = r_{j-1} - D v_{j-1}, is rho_fin minus the hops of v_{j-1} that CROSS a domain boundary:
+// no full-lattice D is applied between two cycles, only the boundary coupling, which is the data the paper
+// exchanges between GPUs in T_Dv^comm.  The coupling travels as projected half spinors through a
+// global halo buffer hb = float4 [nd][8 slots][3][nface], the continuation of the shared-memory slots across the
+// domain boundary: a site on the lower mu-face sends P^-_mu v to slot 2mu of the domain at -mu, a site on the
+// upper face sends (-kappa U_mu)^dag P^+_mu v to slot 2mu+1 of the domain at +mu (48 B per crossing hop).
+//   r_src   residual source read at the own site: r (cycle 0) or rho_fin of the previous cycle
+//   hb_in   CHAIN: halo slots of this domain, filled by its neighbours in the previous cycle
+//   hb_out  halo buffer the final v of this cycle is scattered into (other parity), or nullptr
+//   phi_in  own-site value added to v before the store (phi += v, Alg.1 line 9), or nullptr
+//   phi_out where R_Omega (v [+ phi_in]) is stored
+//   rho_out rho_fin of this cycle, or nullptr (then the last MR residual update is skipped, Q12)
+template <bool CHAIN>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
-ras_cta_kernel(FusedGeom fg, int nd, const float4* __restrict__ dm, const float4* __restrict__ r, float4* __restrict__ vout,
-               int accum) {
+ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, const float4* __restrict__ r_src,
+               const float4* __restrict__ hb_in, float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out,
+               float4* rho_out) {
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     float4* hbuf = smem;            // [8][3][nsp]
@@ -110,12 +130,14 @@ ras_cta_kernel(FusedGeom fg, int nd, const float4* __restrict__ dm, const float4
     }
     const unsigned chunk_bytes = (unsigned)nsp * 16u;
     unsigned dst[8];  // slot 2mu: receiver x-mu (its forward hop); slot 2mu+1: receiver x+mu (its backward hop)
+    int fidx[4];      // index of the site within the mu-face (local index with coordinate mu removed)
     {
         const unsigned base = cta_smem_u32(hbuf);
         int lstride = 1;
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
             const int e = fg.ext[mu];
+            fidx[mu] = (k % lstride) + (k / (lstride * e)) * lstride;
             int kd = k - lstride;
             bool ok = active;
             if (lc[mu] == 0) { kd = k + (e - 1) * lstride; ok = ok && fg.wrap[mu]; }
@@ -136,38 +158,64 @@ ras_cta_kernel(FusedGeom fg, int nd, const float4* __restrict__ dm, const float4
     for (int dom = blockIdx.x; dom < nd; dom += gridDim.x) {
         const size_t gi = cta_site(fg, dom, lc);
         float U[72], A[72], rho[24], v[24];
-        {
-            const float4* p = dm + (size_t)dom * 36 * nsp + k;
+        const float4* p = dm + (size_t)dom * 36 * nsp + k;
 #pragma unroll
-            for (int c = 0; c < 18; c++) {
-                const float4 t = __ldcs(p + (size_t)c * nsp);
-                U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;
+        for (int c = 0; c < 18; c++) {
+            const float4 t = __ldcs(p + (size_t)c * nsp);
+            U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;
+        }
+        if (active) {
+#pragma unroll
+            for (int c = 0; c < 6; c++) {
+                const float4 t = r_src[(size_t)c * V + gi];
+                rho[4 * c] = t.x; rho[4 * c + 1] = t.y; rho[4 * c + 2] = t.z; rho[4 * c + 3] = t.w;
             }
-            if (active) {
+        } else {
 #pragma unroll
-                for (int c = 0; c < 6; c++) {
-                    const float4 t = r[(size_t)c * V + gi];
-                    rho[4 * c] = t.x; rho[4 * c + 1] = t.y; rho[4 * c + 2] = t.z; rho[4 * c + 3] = t.w;
+            for (int n = 0; n < 24; n++) rho[n] = 0.f;
+        }
+        if (CHAIN) {
+            // ---- boundary coupling: rho -= D-terms of v_{j-1} that cross the domain boundary.  A lane whose
+            // in-domain slot 2mu+1 (2mu) has no receiver sits on the upper (lower) face and receives the
+            // outside forward (backward) hop from halo slot 2mu (2mu+1).  All loads are issued first. ----
+            const float4* hin = hb_in + (size_t)dom * 24 * nface;
+            float hh[8][12];
+#pragma unroll
+            for (int sl = 0; sl < 8; sl++) {
+                const bool rcv = active && dst[sl ^ 1] == 0xffffffffu;
+                const float4* q4 = hin + (size_t)sl * 3 * nface + fidx[sl >> 1];
+#pragma unroll
+                for (int j = 0; j < 3; j++) {
+                    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (rcv) t = __ldcs(q4 + (size_t)j * nface);
+                    hh[sl][4 * j] = t.x; hh[sl][4 * j + 1] = t.y; hh[sl][4 * j + 2] = t.z; hh[sl][4 * j + 3] = t.w;
                 }
-            } else {
-#pragma unroll
-                for (int n = 0; n < 24; n++) rho[n] = 0.f;
             }
+            float g[12];
+#define WC_CROSS(MU)                                                   \
+    su3_mul<float>(U + 18 * MU, hh[2 * MU], g);                        \
+    for (int n = 0; n < 12; n++) g[n] = -g[n];                         \
+    reconstruct_add<float, MU, -1>(g, rho);                            \
+    for (int n = 0; n < 12; n++) g[n] = -hh[2 * MU + 1][n];            \
+    reconstruct_add<float, MU, +1>(g, rho);
+            WC_CROSS(0) WC_CROSS(1) WC_CROSS(2) WC_CROSS(3)
+#undef WC_CROSS
+        }
 #pragma unroll
-            for (int c = 0; c < 18; c++) {
-                const float4 t = __ldcs(p + (size_t)(18 + c) * nsp);
-                A[4 * c] = t.x; A[4 * c + 1] = t.y; A[4 * c + 2] = t.z; A[4 * c + 3] = t.w;
-            }
+        for (int c = 0; c < 18; c++) {
+            const float4 t = __ldcs(p + (size_t)(18 + c) * nsp);
+            A[4 * c] = t.x; A[4 * c + 1] = t.y; A[4 * c + 2] = t.z; A[4 * c + 3] = t.w;
         }
         // ---- pull the next domain of this CTA towards L2 while this one is solved ----
         {
             const int nxt = dom + gridDim.x;
             if (nxt < nd) {
                 if (k == 0) prefetch_l2_bulk(dm + (size_t)nxt * 36 * nsp, dm_bytes);
+                if (CHAIN && k == 32) prefetch_l2_bulk(hb_in + (size_t)nxt * 24 * nface, 24u * (unsigned)nface * 16u);
                 if (active) {
                     const size_t gn = cta_site(fg, nxt, lc);
 #pragma unroll
-                    for (int c = 0; c < 6; c++) prefetch_l2(r + (size_t)c * V + gn);
+                    for (int c = 0; c < 6; c++) prefetch_l2(r_src + (size_t)c * V + gn);
                 }
             }
         }
@@ -224,30 +272,61 @@ ras_cta_kernel(FusedGeom fg, int nd, const float4* __restrict__ dm, const float4
             // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9); v += alpha rho; rho -= alpha q
             const float inv = s2 > 0.f ? 1.f / s2 : 0.f;
             const float ar = s0 * inv, ai = s1 * inv;
-            const bool last = it + 1 == fg.niter;
+            const bool upd_rho = it + 1 < fg.niter || rho_out != nullptr;
 #pragma unroll
             for (int n = 0; n < 12; n++) {
                 const float rr = rho[2 * n], ri = rho[2 * n + 1];
                 v[2 * n] = fmaf(ar, rr, v[2 * n]); v[2 * n] = fmaf(-ai, ri, v[2 * n]);
                 v[2 * n + 1] = fmaf(ar, ri, v[2 * n + 1]); v[2 * n + 1] = fmaf(ai, rr, v[2 * n + 1]);
-                if (!last) {
+                if (upd_rho) {
                     rho[2 * n] = fmaf(-ar, q[2 * n], rr); rho[2 * n] = fmaf(ai, q[2 * n + 1], rho[2 * n]);
                     rho[2 * n + 1] = fmaf(-ar, q[2 * n + 1], ri); rho[2 * n + 1] = fmaf(-ai, q[2 * n], rho[2 * n + 1]);
                 }
             }
         }
+        // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
+        if (hb_out) {
+            int dd = dom, dstride = 1;
+            float h[12], g[12];
+#define WC_HALO(MU)                                                                                              \
+    {                                                                                                            \
+        const int nb = fg.nblk[MU], bc = dd % nb;                                                                \
+        dd /= nb;                                                                                                \
+        if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the domain at -mu */            \
+            const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                              \
+            project<float, MU, -1>(v, h);                                                                        \
+            for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(h[4 * j], h[4 * j + 1], h[4 * j + 2], h[4 * j + 3]); \
+        }                                                                                                        \
+        if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the domain at +mu */      \
+            const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                          \
+            project<float, MU, +1>(v, h);                                                                        \
+            su3_adj_mul<float>(U + 18 * MU, h, g);                                                               \
+            for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(g[4 * j], g[4 * j + 1], g[4 * j + 2], g[4 * j + 3]); \
+        }                                                                                                        \
+        dstride *= nb;                                                                                           \
+    }
+            WC_HALO(0) WC_HALO(1) WC_HALO(2) WC_HALO(3)
+#undef WC_HALO
+        }
         // ---- restriction R_Omega: bulk sites only; disjoint over domains, so a plain store (or phi += v) ----
         if (bulk) {
-            if (accum) {
+            if (rho_out) {
+#pragma unroll
+                for (int c = 0; c < 6; c++)
+                    __stcs(rho_out + (size_t)c * V + gi, make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]));
+            }
+            if (phi_in) {
 #pragma unroll
                 for (int c = 0; c < 6; c++) {
-                    const float4 o = vout[(size_t)c * V + gi];
+                    const float4 o = phi_in[(size_t)c * V + gi];
                     v[4 * c] += o.x; v[4 * c + 1] += o.y; v[4 * c + 2] += o.z; v[4 * c + 3] += o.w;
                 }
             }
 #pragma unroll
             for (int c = 0; c < 6; c++)
-                __stcs(vout + (size_t)c * V + gi, make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]));
+                phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
         }
     }
 }
@@ -259,20 +338,33 @@ static size_t cta_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((si
 int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
     if (fg.C != 1 || fg.nsp > FUSED_CTA_MAX_THREADS) return 0;
     const size_t smem = cta_smem_bytes(fg);
-    if (cudaFuncSetAttribute(ras_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(ras_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        cudaFuncSetAttribute(ras_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
-    int per_sm = 0, dev = 0, sms = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta_kernel, fg.nsp, smem) != cudaSuccess || per_sm < 1) {
+    int per_sm = 0, per_sm_chain = 0, dev = 0, sms = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta_kernel<false>, fg.nsp, smem) != cudaSuccess || per_sm < 1 ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_chain, ras_cta_kernel<true>, fg.nsp, smem) != cudaSuccess ||
+        per_sm_chain < 1) {
         cudaGetLastError();
         return 0;
     }
+    if (per_sm_chain < per_sm) per_sm = per_sm_chain;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (ctx->dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm); ctx->dm = nullptr; }
     const size_t bytes = sizeof(float4) * 36 * (size_t)fg.nsp * nd;
     if (cudaMalloc((void**)&ctx->dm, bytes) != cudaSuccess) { cudaGetLastError(); ctx->dm = nullptr; return 0; }
+    // halo buffers of the chained cycles (two parities): float4 [2][nd][8][3][nface]
+    int nface = 1;
+    for (int mu = 0; mu < 4; mu++) nface = fg.ns / fg.ext[mu] > nface ? fg.ns / fg.ext[mu] : nface;
+    nface = (nface + 7) / 8 * 8;
+    if (ctx->hb) { cudaFree(ctx->hb); ctx->hb = nullptr; }
+    if (cudaMalloc((void**)&ctx->hb, sizeof(float4) * 2 * 24 * (size_t)nface * nd) != cudaSuccess) {
+        cudaGetLastError(); ctx->hb = nullptr; cudaFree(ctx->dm); ctx->dm = nullptr; return 0;
+    }
+    ctx->nface = nface;
     pack_domain_major_kernel<<<nd, fg.nsp, 0, ctx->stream>>>(fg, nd, ctx->fields<float>(), -(float)ctx->kappa, ctx->dm);
     ctx->launches++;
     if (cudaGetLastError() != cudaSuccess) return 0;
@@ -283,8 +375,33 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
 
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
-    ras_cta_kernel<<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(fg, ctx->ras.nd, ctx->dm, r, vout, accum ? 1 : 0);
+    ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(
+        fg, ctx->ras.nd, ctx->nface, ctx->dm, r, nullptr, nullptr, accum ? vout : nullptr, vout, nullptr);
     ctx->launches++;
+    WC_CHECK_LAUNCH();
+    return WCRAS_OK;
+}
+
+// v = K_RAS r with NRAS chained cycles (overlap 0): one launch per cycle, no full-lattice D in between.
+// rf = rho_fin (updated in place, own sites only); the halo buffer alternates between its two parities.
+int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
+    const FusedGeom& fg = ctx->fused;
+    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;
+    float4* rf = ctx->ras32[0];
+    float4* hb[2] = {ctx->hb, ctx->hb + (size_t)24 * nface * nd};
+    const size_t smem = cta_smem_bytes(fg);
+    for (int j = 0; j < nras; j++) {
+        const bool last = j == nras - 1;
+        TimedRegion tr(ctx, TC_BLOCK);
+        ctx->block_dv += ctx->ras.niter;
+        if (j == 0)
+            ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, nface, ctx->dm, r, nullptr, last ? nullptr : hb[0],
+                                                                                nullptr, v, last ? nullptr : rf);
+        else
+            ras_cta_kernel<true><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, nface, ctx->dm, rf, hb[(j - 1) & 1],
+                                                                               last ? nullptr : hb[j & 1], v, v, last ? nullptr : rf);
+        ctx->launches++;
+    }
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
 }

@@ -295,7 +295,8 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
     Vec* sh = k_identity ? w.s : w.sh;
     const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
     int it = 0, restarts = 0, status = WCRAS_NOT_CONVERGED;
-    double rr = bb;
+    double rr = bb, best = bb;
+    int it_best = 0;
     while (it < maxit) {
         const Scalars& h = *ctx->sc_host;
         if (hypot(h.rho[0], h.rho[1]) < tiny * bb || (it > 0 && hypot(h.omega[0], h.omega[1]) < tiny)) {
@@ -337,6 +338,9 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
         rr = ctx->sc_host->rr;
         if (!(rr == rr)) { status = WCRAS_BREAKDOWN; break; }  // NaN
         if (std::sqrt(rr / bb) < tol) { status = WCRAS_OK; break; }
+        // stagnation guard (fp32 inner solver at the end of its accuracy): no new minimum of |r| for 10 iterations
+        if (rr < best) { best = rr; it_best = it; }
+        else if (it - it_best >= 10) break;
     }
     WC_CHECK_LAUNCH();
     *iters = it;
@@ -388,12 +392,30 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
         LAUNCH(k_norm2_d, (size_t)12 * V, in64, ctx->sc64, ctx->partials, ctx->ticket);
         LAUNCH(k_d2f_normalised, V, in64, b32, ctx->sc64);
     }
+    // Tolerance of this inner solve (reading A2): the outer residual after this preconditioner call is
+    // about (inner accuracy) x |in|, so the reduction still missing is R = target/|in|.  It is spread evenly over
+    // the n = ceil(log R / log inner_tol) calls that are needed when no call may go deeper than inner_tol (the
+    // accuracy fp32 can deliver), instead of solving every call to inner_tol and overshooting the target.
+    if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
+    double itol = ctx->inner_tol;
+    const double in_norm = std::sqrt(ctx->sc_host->nrm);
+    if (ctx->outer_target > 0 && in_norm > 0) {
+        const double R = 0.5 * ctx->outer_target / in_norm;
+        if (R < 1.0) {
+            const double n = std::ceil(std::log(R) / std::log(ctx->inner_tol) - 1e-9);
+            itol = std::pow(R, 1.0 / (n < 1 ? 1 : n));
+        } else {
+            itol = 0.1;
+        }
+        if (itol < ctx->inner_tol) itol = ctx->inner_tol;
+        if (itol > 0.1) itol = 0.1;
+    }
     Work<float> w = work32(ctx);
     const bool use_ras = ctx->use_ras && ctx->ras.set;
     int it = 0;
     double rel = 0;
     auto K = [ctx](const float4* in, float4* out) { return ras_apply(ctx, in, out); };
-    int rc = bicgstab<float>(ctx, w, b32, x32, ctx->inner_tol, ctx->inner_maxit, false, !use_ras, K, &it, &rel);
+    int rc = bicgstab<float>(ctx, w, b32, x32, itol, ctx->inner_maxit, true, !use_ras, K, &it, &rel);
     *inner_iters += it;
     *inner_solves += 1;
     if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
@@ -433,6 +455,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         double rel = 0;
         // solve D dx = res to relative accuracy tol*|eta|/|res| so that the total residual meets tol
         const double tol_pass = 0.7 * tol * std::sqrt(en2 / rn2);
+        ctx->outer_target = tol_pass * std::sqrt(rn2);  // absolute |r| this pass has to reach
         int rc = bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel);
         if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
         outer += it;

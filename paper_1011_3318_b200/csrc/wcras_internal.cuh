@@ -154,13 +154,17 @@ struct wcras_ctx {
     // RAS
     RasConfig ras;
     int tier_request = 0;
+    int chain_cycles = 1;          // overlap 0, persistent-CTA tier: NRAS cycles chained through rho_fin (ras_cta.cu)
     FusedGeom fused;               // valid when ras.tier == 2
     float4* dm = nullptr;          // domain-major operand copy of the persistent-CTA tier: [nd][36][nsp]
     int cta_grid = 0;              // its persistent grid size
+    float4* hb = nullptr;          // halo buffers of the chained K_RAS cycles: [2][nd][8][3][nface]
+    int nface = 0;
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
     double* mr_scal = nullptr;                                     // [niter][nd][4]
     // solver parameters
-    double inner_tol = 1e-5;
+    double inner_tol = 5e-7;       // deepest relative accuracy asked of one fp32 inner solve (reading A2)
+    double outer_target = 0;       // absolute residual norm the running outer pass has to reach
     int inner_maxit = 1000, outer_maxit = 50, use_ras = 1;
     // workspace (allocated lazily)
     std::vector<void*> owned;

@@ -161,21 +161,24 @@ RAS_CASES = [
     (0, (2, 2, 2, 2), 0, 4, 1), (0, (2, 2, 2, 2), 0, 4, 3), (0, (2, 2, 2, 2), 1, 3, 2), (0, (4, 4, 4, 4), 0, 6, 1),
     (1, (4, 4, 4, 4), 0, 4, 1), (1, (4, 4, 4, 4), 1, 4, 1), (1, (4, 4, 4, 4), 0, 5, 3), (1, (8, 4, 4, 4), 1, 2, 2),
     ("ragged", (2, 2, 5, 4), 1, 3, 2), ("ragged", (3, 4, 5, 2), 0, 1, 1),
+    # chained cycles (overlap 0, NRAS > 1): plain, with a wrap-around direction (block = L in x), ragged
+    (1, (4, 4, 4, 4), 0, 2, 2), (1, (8, 4, 4, 2), 0, 3, 3), ("ragged", (3, 4, 5, 2), 0, 2, 3),
 ]
 
 
-@pytest.mark.parametrize("tier", [1, 0, 3])
+@pytest.mark.parametrize("tier", [1, 0, 3, 4])
 @pytest.mark.parametrize("which,block,s,nit,nras", RAS_CASES)
 def test_ras_apply(which, block, s, nit, nras, tier):
     """tier 1 = generic, 0 = automatic (persistent CTA kernel for |Omega'| <= 256, cluster kernel above, generic
-    if neither fits), 3 = cluster kernel forced (skipped where the shape does not fit it)."""
+    if neither fits), 3 = cluster kernel forced (skipped where the shape does not fit it), 4 = fused tier with the
+    NRAS cycles not chained (tier 0 chains them when the overlap is 0)."""
     cs = ragged_case() if which == "ragged" else case(which)
     cs.ctx.set_ras_tier(tier)
     try:
         cs.ctx.ras_precondition(block, s, nit, nras)
     except binding.WcrasError as e:
         cs.ctx.set_ras_tier(0)
-        if tier == 3 and e.code == binding.UNSUPPORTED:
+        if tier in (3, 4) and e.code == binding.UNSUPPORTED:
             pytest.skip("shape does not fit the cluster kernel")
         raise
     r = I.spinor(cs.dims, 55)
@@ -233,7 +236,9 @@ def test_solve_true_residual(which, ras):
     # nested scheme with inner_tol 1e-5: each outer half-step gains ~5 digits (catches a broken preconditioner path)
     assert info["outer_iters"] <= 3 and info["inner_solves"] <= 5
     if ras is not None:
-        assert info["ras_applies"] == 2 * info["inner_iters"] and info["block_dv"] > 0
+        # two K_RAS per inner iteration, one when an inner solve leaves at the half step
+        assert 2 * info["inner_iters"] - info["inner_solves"] <= info["ras_applies"] <= 2 * info["inner_iters"]
+        assert info["block_dv"] > 0
     if which <= 1:  # compare with the oracle's own solution (reported, loose: cond(D) * tol)
         x, _ = cs.op.bicgstab(eta, tol=1e-13)
         assert rel(phi, x) < 1e-9
