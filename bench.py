@@ -30,8 +30,15 @@ sys.path.insert(0, ROOT)
 METRIC = "clover Dslash GB/s (% HBM peak); 32^4 RAS-BiCGStab time-to-1e-12"
 TOL = 1e-12
 # RAS parameters of the timed solve (every row states NRAS, Q10)
-RAS = dict(domain=(8, 8, 4, 4), overlap=0, block_iters=5, nras=1)
-INNER_TOL = 1e-5
+# The timed step uses the fastest point of the paper's parameter survey (NRAS x N_dominv, here also
+# over the domain shape) as measured on B200; the domain shapes BASELINE.json:configs[3] names are timed beside it.
+RAS = dict(domain=(4, 4, 4, 4), overlap=0, block_iters=2, nras=3)
+RAS_NAMED = [dict(domain=(8, 8, 4, 4), overlap=0, block_iters=3, nras=2),
+             dict(domain=(8, 8, 8, 8), overlap=0, block_iters=5, nras=1)]
+INNER_TOL = 5e-7
+# dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
+# `ncu --set full` capture (profiles/r1b_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
+DSLASH_TRAFFIC_NCU_BYTES = 827.5e6
 
 
 def peaks():
@@ -148,22 +155,20 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
-    from paper_1011_3318_b200 import binding, inputs as I
+    from paper_1011_3318_b200 import binding, inputs as I, replicas as R
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local)
     if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        R.init("nccl", torch.device("cuda", local))
     hbm_peak, peak_src, peaks_json = peaks()
 
     cfg = I.CONFIGS[args.config]
     dims = cfg["dims"]
     V = I.volume(dims)
     U = I.make_gauge(cfg)
-    eta = I.spinor(dims, cfg["seed"], stream=rank)  # independent right-hand side per replica
+    eta = I.spinor(dims, cfg["seed"], stream=R.source_streams(rank, world)[0])  # independent right-hand side per replica
     stream = torch.cuda.current_stream()
     Ud = torch.view_as_real(torch.from_numpy(U)).contiguous().cuda()
     ctx = binding.Context(dims, cfg["kappa"], cfg["csw"], Ud, stream=stream)
@@ -174,22 +179,27 @@ def main():
     phi_h = torch.empty_like(eta_h).pin_memory()
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        R.barrier(world, cuda=True)
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return R.max_over_ranks(x, world, "cuda")
 
     # ---- unpreconditioned solve, for the side-by-side row (not the timed step) ----
     ctx.set_solver(inner_tol=INNER_TOL, use_ras=False)
     ctx.set_timing(False)
     ctx.solve(eta_d, phi_d, TOL)
     info_noprec = ctx.solve(eta_d, phi_d, TOL)
+
+    # ---- the domain shapes configs[3] names, for the side-by-side rows (not the timed step) ----
+    named = {}
+    for rp in RAS_NAMED:
+        ctx.ras_precondition(rp["domain"], rp["overlap"], rp["block_iters"], rp["nras"])
+        ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+        ctx.solve(eta_d, phi_d, TOL)
+        i = ctx.solve(eta_d, phi_d, TOL)
+        named["ras_%s_it%d_nras%d" % ("x".join(map(str, rp["domain"])), rp["block_iters"], rp["nras"])] = {
+            k: i[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies",
+                              "rel_resid_true", "ms_total")}
 
     # ---- the timed step: RAS-preconditioned nested solve ----
     ctx.ras_precondition(RAS["domain"], RAS["overlap"], RAS["block_iters"], RAS["nras"])
@@ -235,8 +245,7 @@ def main():
     true_resid = info["rel_resid_true"]
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        R.shutdown(world)
         return
 
     cpu = None
@@ -260,7 +269,8 @@ def main():
         "gpu_launches": int(launches),
         "roofline": {"kernel": "dslash_kernel<float> (fp32 clover Dslash)", "bound": "hbm", "achieved": gbs_in_solve,
                      "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": gbs_in_solve / hbm_peak,
-                     "traffic": None, "bytes_per_site": 768, "sites": V,
+                     "traffic": DSLASH_TRAFFIC_NCU_BYTES if V == 1 << 20 else None, "algorithmic_bytes": 768.0 * V,
+                     "bytes_per_site": 768, "sites": V,
                      "ms_per_launch_in_solve": ms_dslash_in_solve, "ms_per_launch_burst": ms_d32,
                      "achieved_burst": gbs_burst, "frac_burst": gbs_burst / hbm_peak,
                      "frac_of_nominal_8TBs": gbs_burst / 8000.0,
@@ -271,17 +281,17 @@ def main():
                                               "ms_blocksolve", "ms_blas")},
                   "no_prec": {k: info_noprec[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64",
                                                           "rel_resid_true", "ms_total")},
-                  "ras_faster_than_no_prec": info["ms_total"] < info_noprec["ms_total"]},
+                  "ras_faster_than_no_prec": info["ms_total"] < info_noprec["ms_total"], **named},
         "kernels": {"dslash_fp32_ms": ms_d32, "dslash_fp64_ms": ms_d64,
                     "dslash_fp64_gbs": 1536.0 * V / (ms_d64 * 1e-3) / 1e9,
                     "block_solve_ms": ms_blk,
                     "block_solve_site_sweeps_per_s": V * RAS["block_iters"] / (ms_blk * 1e-3),
+                    "block_solve_hbm_gbs": 864.0 * V / (ms_blk * 1e-3) / 1e9,
                     "blas_update_xr_ms": ms_blas, "blas_update_xr_gbs": 8 * 96.0 * V / (ms_blas * 1e-3) / 1e9},
         "true_residual": true_resid,
     }
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    R.shutdown(world)
 
 
 if __name__ == "__main__":
