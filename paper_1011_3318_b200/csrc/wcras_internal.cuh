@@ -216,8 +216,17 @@ struct TimedRegion {
 
 // ---- host entry points implemented across the .cu files ----
 namespace wc {
-constexpr int RED_BLOCKS = 592;  // 148 SMs x 4
-constexpr int RED_THREADS = 256;
+// BLAS-1 grid: ONE 1024-thread CTA per SM.  Measured on B200 at 32^4 (k_update_xr, 8 vector passes): 148 x 1024
+// 125 us = 6.4 TB/s, 296 x 1024 127 us, 592 x 256 150 us, 1184 x 256 155 us, 296 x 256 221 us -- with several
+// smaller CTAs per SM the block scheduler leaves the SMs unevenly loaded and the slowest SM sets the time.
+#ifndef WC_RED_BLOCKS
+#define WC_RED_BLOCKS 148
+#endif
+#ifndef WC_RED_THREADS
+#define WC_RED_THREADS 1024
+#endif
+constexpr int RED_BLOCKS = WC_RED_BLOCKS;
+constexpr int RED_THREADS = WC_RED_THREADS;
 
 int alloc_dev(wcras_ctx* ctx, void** p, size_t bytes);
 int ensure_workspace(wcras_ctx* ctx);
