@@ -4,7 +4,7 @@
 // One thread per site, consecutive threads = consecutive x (coalesced 16-byte loads from the SoA fields).
 // HBM-bound: algorithmic traffic per site (fp32) = 4 links 288 B + clover 288 B + spinor in 96 B + out 96 B
 // = 768 B (fp64: 1536 B); neighbour spinors and backward links are re-reads that L1/L2 must serve.
-#include "wcras_internal.cuh"
+#include "blas.cuh"
 
 namespace wc {
 
@@ -27,38 +27,136 @@ __device__ __forceinline__ void hop_pair(const Fields<T>& f, size_t V, const Geo
     }
 }
 
-template <typename T, bool XPAY, int TH, int MINB>
+// Two-level deterministic grid reduction for the dots fused into the Dslash (north_star (d)): a CTA writes its
+// partial, the last CTA of each group of DOT_GROUP CTAs (atomic ticket) sums the group in a fixed order, the last
+// group to finish sums the group partials in a fixed order.  Returns true in thread 0 of that last CTA.
+constexpr int DOT_GROUP = 128;
+template <int TH>
+__device__ __forceinline__ bool dslash_grid_reduce(double (&v)[3], double* __restrict__ part, double* __restrict__ gpart,
+                                                   unsigned* __restrict__ tickets, double (&tot)[3]) {
+    constexpr int NW = TH / 32;
+    __shared__ double sm[3][NW];
+    __shared__ int stage;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned nblk = gridDim.x, grp = blockIdx.x / DOT_GROUP, ngrp = (nblk + DOT_GROUP - 1) / DOT_GROUP;
+    const unsigned gsize = min((unsigned)DOT_GROUP, nblk - grp * DOT_GROUP);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const double t = warp_sum(v[k]);
+        if (lane == 0) sm[k][w] = t;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            double t = 0;
+            for (int j = 0; j < NW; j++) t += sm[k][j];
+            part[(size_t)blockIdx.x * 3 + k] = t;
+        }
+        __threadfence();
+        stage = atomicInc(&tickets[1 + grp], gsize - 1) == gsize - 1 ? 1 : 0;
+    }
+    __syncthreads();
+    if (!stage) return false;
+    __threadfence();
+    // last CTA of the group: fixed-order sum of the group's partials (warp 0 only)
+    if (w == 0) {
+        double t[3] = {0, 0, 0};
+        for (unsigned j = lane; j < gsize; j += 32)
+#pragma unroll
+            for (int k = 0; k < 3; k++) t[k] += __ldcg(&part[((size_t)grp * DOT_GROUP + j) * 3 + k]);
+#pragma unroll
+        for (int k = 0; k < 3; k++) t[k] = warp_sum(t[k]);
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; k++) gpart[(size_t)grp * 3 + k] = t[k];
+            __threadfence();
+            stage = atomicInc(&tickets[0], ngrp - 1) == ngrp - 1 ? 2 : 1;
+        }
+    }
+    __syncthreads();
+    if (stage != 2) return false;
+    __threadfence();
+    if (w == 0) {
+        double t[3] = {0, 0, 0};
+        for (unsigned j = lane; j < ngrp; j += 32)
+#pragma unroll
+            for (int k = 0; k < 3; k++) t[k] += __ldcg(&gpart[(size_t)j * 3 + k]);
+#pragma unroll
+        for (int k = 0; k < 3; k++) tot[k] = warp_sum(t[k]);
+        return lane == 0;
+    }
+    return false;
+}
+
+// DOT = 0: out = D in (XPAY: out = bsrc - D in).
+// DOT = 1: also rtv = <dotv, out> and alpha = rho / rtv          (BiCGStab: v = D ph, dotv = rt)
+// DOT = 2: also ts = <out, dotv>, tt = <out, out>, omega = ts/tt (BiCGStab: t = D sh, dotv = s)
+template <typename T, bool XPAY, int TH, int MINB, int DOT>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
                                                      typename VecOf<T>::type* __restrict__ out,
-                                                     const typename VecOf<T>::type* bsrc) {
+                                                     const typename VecOf<T>::type* bsrc,
+                                                     const typename VecOf<T>::type* __restrict__ dotv, Scalars* sc,
+                                                     double* part, double* gpart, unsigned* tickets) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.V) return;
-    const size_t V = g.V;
-    int x[4];
-    site_coords(g, i, x);
-    T hop[24];
+    const bool valid = i < g.V;
+    if (!DOT && !valid) return;
+    double dsum[3] = {0, 0, 0};
+    if (valid) {
+        const size_t V = g.V;
+        int x[4];
+        site_coords(g, i, x);
+        T hop[24];
 #pragma unroll
-    for (int k = 0; k < 24; k++) hop[k] = 0;
-    hop_pair<T, 0, false>(f, V, g, x, i, 1, in, true, true, hop);
-    hop_pair<T, 1, false>(f, V, g, x, i, g.L[0], in, true, true, hop);
-    hop_pair<T, 2, false>(f, V, g, x, i, g.L[0] * g.L[1], in, true, true, hop);
-    hop_pair<T, 3, false>(f, V, g, x, i, g.L[0] * g.L[1] * g.L[2], in, true, true, hop);
-    T s[24], acc[24];
-    {
-        T cl[72];
-        load_spinor(in, V, i, s);
-        load_clover(f, V, i, cl);
-        clover_apply<T>(cl, s, acc);
+        for (int k = 0; k < 24; k++) hop[k] = 0;
+        hop_pair<T, 0, false>(f, V, g, x, i, 1, in, true, true, hop);
+        hop_pair<T, 1, false>(f, V, g, x, i, g.L[0], in, true, true, hop);
+        hop_pair<T, 2, false>(f, V, g, x, i, g.L[0] * g.L[1], in, true, true, hop);
+        hop_pair<T, 3, false>(f, V, g, x, i, g.L[0] * g.L[1] * g.L[2], in, true, true, hop);
+        T s[24], acc[24];
+        {
+            T cl[72];
+            load_spinor(in, V, i, s);
+            load_clover(f, V, i, cl);
+            clover_apply<T>(cl, s, acc);
+        }
+        if (XPAY) {
+            load_spinor(bsrc, V, i, s);
+#pragma unroll
+            for (int k = 0; k < 24; k++) acc[k] = s[k] - (acc[k] - kappa * hop[k]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < 24; k++) acc[k] -= kappa * hop[k];
+        }
+        store_spinor(out, V, i, acc);
+        if (DOT) {
+            load_spinor(dotv, V, i, s);
+            T d0 = 0, d1 = 0, d2 = 0;  // per-site sums in T, accumulated over sites in fp64
+#pragma unroll
+            for (int n = 0; n < 12; n++) {
+                const T ar = DOT == 1 ? s[2 * n] : acc[2 * n], ai = DOT == 1 ? s[2 * n + 1] : acc[2 * n + 1];
+                const T br = DOT == 1 ? acc[2 * n] : s[2 * n], bi = DOT == 1 ? acc[2 * n + 1] : s[2 * n + 1];
+                d0 = wc_fma(ar, br, d0); d0 = wc_fma(ai, bi, d0);   // Re conj(a) b
+                d1 = wc_fma(ar, bi, d1); d1 = wc_fma(-ai, br, d1);  // Im conj(a) b
+                d2 = wc_fma(acc[2 * n], acc[2 * n], d2); d2 = wc_fma(acc[2 * n + 1], acc[2 * n + 1], d2);
+            }
+            dsum[0] = d0; dsum[1] = d1; dsum[2] = d2;
+        }
     }
-    if (XPAY) {
-        load_spinor(bsrc, V, i, s);
-#pragma unroll
-        for (int k = 0; k < 24; k++) acc[k] = s[k] - (acc[k] - kappa * hop[k]);
-    } else {
-#pragma unroll
-        for (int k = 0; k < 24; k++) acc[k] -= kappa * hop[k];
+    if (DOT) {
+        double tot[3];
+        if (dslash_grid_reduce<TH>(dsum, part, gpart, tickets, tot)) {
+            if (DOT == 1) {
+                sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
+                const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
+                sc->alpha[0] = a.r; sc->alpha[1] = a.i;
+            } else {
+                sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
+                sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
+                sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
+            }
+        }
     }
-    store_spinor(out, V, i, acc);
 }
 
 struct Box {
@@ -129,7 +227,7 @@ __global__ void __launch_bounds__(128) dslash_box_kernel(Geom g, Fields<T> f, T 
 
 template <typename T>
 int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>::type* out,
-           const typename VecOf<T>::type* b_minus) {
+           const typename VecOf<T>::type* b_minus, int dot, const typename VecOf<T>::type* dotv, Scalars* sc) {
     TimedRegion tr(ctx, sizeof(T) == 4 ? TC_DSLASH : TC_DSLASH64);
     const int V = ctx->geom.V;
     // 64-thread CTAs with the full register budget (165 registers fp32, 252 fp64): the compiler then keeps all
@@ -137,10 +235,27 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
     // 32^4: 130 us (fp32) / 292 us (fp64) against 147 / 330 us at 96 / 186 registers with 128-thread CTAs.
     constexpr int TH = 64;
     const unsigned grid = (V + TH - 1) / TH;
-    if (b_minus)
-        dslash_kernel<T, true, TH, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, b_minus);
-    else
-        dslash_kernel<T, false, TH, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr);
+    if (dot) {
+        if (!ctx->dpart) {
+            const unsigned ngrp = (grid + DOT_GROUP - 1) / DOT_GROUP;
+            if (alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * 3 * grid)) return WCRAS_CUDA_ERROR;
+            if (alloc_dev(ctx, (void**)&ctx->dgpart, sizeof(double) * 3 * ngrp)) return WCRAS_CUDA_ERROR;
+            if (alloc_dev(ctx, (void**)&ctx->dtickets, sizeof(unsigned) * (ngrp + 1))) return WCRAS_CUDA_ERROR;
+            WC_CUDA(cudaMemsetAsync(ctx->dtickets, 0, sizeof(unsigned) * (ngrp + 1), ctx->stream));
+        }
+        if (dot == 1)
+            dslash_kernel<T, false, TH, 1, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
+                                                                            dotv, sc, ctx->dpart, ctx->dgpart, ctx->dtickets);
+        else
+            dslash_kernel<T, false, TH, 1, 2><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
+                                                                            dotv, sc, ctx->dpart, ctx->dgpart, ctx->dtickets);
+    } else if (b_minus) {
+        dslash_kernel<T, true, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, b_minus,
+                                                                       nullptr, nullptr, nullptr, nullptr, nullptr);
+    } else {
+        dslash_kernel<T, false, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
+                                                                        nullptr, nullptr, nullptr, nullptr, nullptr);
+    }
     ctx->launches++;
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;
     WC_CHECK_LAUNCH();
@@ -164,8 +279,8 @@ int dslash_box(wcras_ctx* ctx, const int start[4], const int ext[4], bool all_bl
     return WCRAS_OK;
 }
 
-template int dslash<float>(wcras_ctx*, const float4*, float4*, const float4*);
-template int dslash<double>(wcras_ctx*, const double2*, double2*, const double2*);
+template int dslash<float>(wcras_ctx*, const float4*, float4*, const float4*, int, const float4*, Scalars*);
+template int dslash<double>(wcras_ctx*, const double2*, double2*, const double2*, int, const double2*, Scalars*);
 template int dslash_box<float>(wcras_ctx*, const int*, const int*, bool, const float4*, float4*);
 template int dslash_box<double>(wcras_ctx*, const int*, const int*, bool, const double2*, double2*);
 

@@ -97,25 +97,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* _
     }
 }
 
-// rtv = <rt, v>; alpha = rho / rtv
-template <typename T, typename Vec>
-__global__ void __launch_bounds__(RED_THREADS) k_dot_rtv(size_t n, const Vec* __restrict__ rt, const Vec* __restrict__ v, Scalars* sc,
-                                                         double* partials, unsigned* ticket) {
-    constexpr int N = Cx<Vec>::N;
-    double acc[2] = {0, 0};
-    GRID_STRIDE(k, n) {
-        cpx<T> a[N], b[N];
-        unpack<T>(rt[k], a); unpack<T>(v[k], b);
-#pragma unroll
-        for (int j = 0; j < N; j++) dot_acc(a[j], b[j], acc[0], acc[1]);
-    }
-    double tot[2];
-    if (grid_reduce<2>(acc, partials, ticket, tot)) {
-        sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
-        const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
-        sc->alpha[0] = a.r; sc->alpha[1] = a.i;
-    }
-}
+// <rt,v> (alpha) and <t,s>, <t,t> (omega) are fused into the Dslash that produces v and t (dslash.cu, DOT = 1 / 2)
 
 // s = r - alpha v; ss = |s|^2
 template <typename T, typename Vec>
@@ -136,29 +118,6 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_s(size_t n, const Vec* _
     }
     double tot[1];
     if (grid_reduce<1>(acc, partials, ticket, tot)) sc->ss = tot[0];
-}
-
-// ts = <t,s>, tt = <t,t>; omega = ts/tt (0 if tt = 0)
-template <typename T, typename Vec>
-__global__ void __launch_bounds__(RED_THREADS) k_dot_ts(size_t n, const Vec* __restrict__ t, const Vec* __restrict__ s, Scalars* sc,
-                                                        double* partials, unsigned* ticket) {
-    constexpr int N = Cx<Vec>::N;
-    double acc[3] = {0, 0, 0};
-    GRID_STRIDE(k, n) {
-        cpx<T> a[N], b[N];
-        unpack<T>(t[k], a); unpack<T>(s[k], b);
-#pragma unroll
-        for (int j = 0; j < N; j++) {
-            dot_acc(a[j], b[j], acc[0], acc[1]);
-            acc[2] += (double)a[j].r * a[j].r + (double)a[j].i * a[j].i;
-        }
-    }
-    double tot[3];
-    if (grid_reduce<3>(acc, partials, ticket, tot)) {
-        sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
-        sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
-        sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
-    }
 }
 
 // x += alpha ph + omega sh; r = s - omega t; rho_old = rho; rho = <rt,r>; rr = |r|^2
@@ -309,10 +268,9 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
             LAUNCH((k_update_p<T, Vec>), n, w.r, w.p, w.v, w.sc);
         }
         if (!k_identity) if (int rc = K(w.p, ph)) return rc;
-        if (int rc = dslash<T>(ctx, ph, w.v)) return rc;
+        if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, w.rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
         {
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_dot_rtv<T, Vec>), n, w.rt, w.v, w.sc, part, tk);
             LAUNCH((k_update_s<T, Vec>), n, w.r, w.v, w.s, w.sc, part, tk);
         }
         if (half_exit) {
@@ -327,10 +285,9 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
             }
         }
         if (!k_identity) if (int rc = K(w.s, sh)) return rc;
-        if (int rc = dslash<T>(ctx, sh, w.t)) return rc;
+        if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
         {
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_dot_ts<T, Vec>), n, w.t, w.s, w.sc, part, tk);
             LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, w.rt, w.r, w.sc, part, tk);
         }
         it++;

@@ -178,6 +178,8 @@ struct wcras_ctx {
     wc::Scalars* sc_host = nullptr;  // pinned
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;
+    double *dpart = nullptr, *dgpart = nullptr;  // partials of the dots fused into the Dslash (per CTA, per group)
+    unsigned* dtickets = nullptr;
     // timing
     int timing = 0;
     std::vector<cudaEvent_t> ev_pool;
@@ -238,9 +240,11 @@ int from_internal(wcras_ctx* ctx, int prec, const void* internal, void* canonica
 int export_clover(wcras_ctx* ctx, double* out_dev);
 
 // dslash.cu : out = D in   or   out = b - D in (b may alias out)
+// dot = 1: also rtv = <dotv, out>, alpha = rho/rtv; dot = 2: also ts = <out, dotv>, tt = |out|^2, omega = ts/tt (sc)
 template <typename T>
 int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>::type* out,
-           const typename VecOf<T>::type* b_minus = nullptr);
+           const typename VecOf<T>::type* b_minus = nullptr, int dot = 0, const typename VecOf<T>::type* dotv = nullptr,
+           Scalars* sc = nullptr);
 template <typename T>
 int dslash_box(wcras_ctx* ctx, const int start[4], const int ext[4], bool all_blocks,
                const typename VecOf<T>::type* in, typename VecOf<T>::type* out);

@@ -292,6 +292,23 @@ def test_full_size_32_sampled(prec):
     assert err <= (2e-6 if prec == 32 else 1e-13)
 
 
+def test_full_size_32_ras_apply():
+    """K_RAS at full size in the launch configuration bench.py times (4^4 domains, overlap 0, N_dominv 2, NRAS 3:
+    persistent one-CTA-per-domain kernel, 4096 domains over 148 CTAs, chained cycles) against the oracle's Alg. 1 on
+    every site; the same with the cycles not chained (full-lattice D between them)."""
+    cs = case(3)
+    r = I.spinor(cs.dims, 77)
+    r32 = r.astype(np.complex64).astype(np.complex128)
+    want = cs.op.ras_apply((4, 4, 4, 4), 0, 2, 3, r32)
+    for tier in (0, 4):
+        cs.ctx.set_ras_tier(tier)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+        got = cs.ras_apply(r32)
+        assert rel(got, want) <= TOL_RAS
+        assert np.abs(got - want).max() / np.abs(want).max() <= 10 * TOL_RAS
+    cs.ctx.set_ras_tier(0)
+
+
 def test_full_size_32_solve():
     cs = case(3)
     cfg = I.CONFIGS[3]
