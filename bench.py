@@ -38,7 +38,7 @@ RAS_NAMED = [dict(domain=(8, 8, 4, 4), overlap=0, block_iters=3, nras=2),
 INNER_TOL = 5e-7
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
 # `ncu --set full` capture (profiles/r1b_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
-DSLASH_TRAFFIC_NCU_BYTES = 827.5e6
+DSLASH_TRAFFIC_NCU_BYTES = 826.4e6
 
 
 def peaks():
@@ -240,7 +240,11 @@ def main():
     ms_d64 = ctx.time_kernel(1, 50)
     ms_blk = ctx.time_kernel(2, 50)
     ms_blas = ctx.time_kernel(3, 100)
-    gbs_in_solve = 768.0 * V / (ms_dslash_in_solve * 1e-3) / 1e9
+    n_blk = sum(i["block_dv"] for i in infos) // RAS["block_iters"]
+    ms_blk_in_solve = sum(i["ms_blocksolve"] for i in infos) / max(1, n_blk)
+    # inside the solve every fp32 D launch is the variant with the fused dot (<rt,v> or <t,s>,<t,t>): it also reads
+    # the dot vector, 864 B/site, and its time includes the one-CTA dot_finish_kernel launched behind it
+    gbs_in_solve = 864.0 * V / (ms_dslash_in_solve * 1e-3) / 1e9
     gbs_burst = 768.0 * V / (ms_d32 * 1e-3) / 1e9
     true_resid = info["rel_resid_true"]
 
@@ -270,11 +274,20 @@ def main():
         "roofline": {"kernel": "dslash_kernel<float> (fp32 clover Dslash)", "bound": "hbm", "achieved": gbs_in_solve,
                      "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": gbs_in_solve / hbm_peak,
                      "traffic": DSLASH_TRAFFIC_NCU_BYTES if V == 1 << 20 else None, "algorithmic_bytes": 768.0 * V,
-                     "bytes_per_site": 768, "sites": V,
+                     "bytes_per_site": 768, "bytes_per_site_in_solve": 864, "sites": V,
                      "ms_per_launch_in_solve": ms_dslash_in_solve, "ms_per_launch_burst": ms_d32,
                      "achieved_burst": gbs_burst, "frac_burst": gbs_burst / hbm_peak,
                      "frac_of_nominal_8TBs": gbs_burst / 8000.0,
                      "gflops_1824_per_site": 1824.0 * V / (ms_d32 * 1e-3) / 1e9},
+        # the kernel the timed solve spends most of its time in (profiles/): one K_RAS cycle over all domains
+        "roofline_block_solve": {
+            "kernel": "ras_cta_kernel (persistent one-CTA-per-domain MR block solver, %d sweeps per launch)" % RAS["block_iters"],
+            "bound": "hbm", "unit": "GB/s", "bytes_per_site": 864, "sites": V, "peak": hbm_peak,
+            "ms_per_launch_in_solve": ms_blk_in_solve, "achieved": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9,
+            "frac": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9 / hbm_peak,
+            "ms_per_launch_burst": ms_blk, "frac_burst": 864.0 * V / (ms_blk * 1e-3) / 1e9 / hbm_peak,
+            "note": "HBM floor = operands 576 + r 96 + v 96 + phi/rho 96 B per site; the kernel is bound by fp32 issue "
+                    "latency at 2 warps per scheduler, see profiles/r1b_kernels.md"},
         "cpu_baseline": cpu,
         "solve": {"ras": {k: info[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv",
                                               "ras_applies", "rel_resid_true", "ms_total", "ms_dslash", "ms_dslash64",

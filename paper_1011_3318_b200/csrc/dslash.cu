@@ -27,66 +27,58 @@ __device__ __forceinline__ void hop_pair(const Fields<T>& f, size_t V, const Geo
     }
 }
 
-// Two-level deterministic grid reduction for the dots fused into the Dslash (north_star (d)): a CTA writes its
-// partial, the last CTA of each group of DOT_GROUP CTAs (atomic ticket) sums the group in a fixed order, the last
-// group to finish sums the group partials in a fixed order.  Returns true in thread 0 of that last CTA.
-constexpr int DOT_GROUP = 128;
+// Dots fused into the Dslash (north_star (d)): every CTA reduces its 3 sums (warp shuffle -> shared memory) and
+// stores one partial, with no fence or atomic on the way (a __threadfence per 64-thread CTA would wait for the
+// CTA's output stores and cost ~15 % of the kernel).  dot_finish_kernel, one 1024-thread CTA launched right
+// behind it, sums the partials in a fixed order and finishes the scalar recurrence: deterministic.
 template <int TH>
-__device__ __forceinline__ bool dslash_grid_reduce(double (&v)[3], double* __restrict__ part, double* __restrict__ gpart,
-                                                   unsigned* __restrict__ tickets, double (&tot)[3]) {
+__device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __restrict__ part) {
     constexpr int NW = TH / 32;
     __shared__ double sm[3][NW];
-    __shared__ int stage;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const unsigned nblk = gridDim.x, grp = blockIdx.x / DOT_GROUP, ngrp = (nblk + DOT_GROUP - 1) / DOT_GROUP;
-    const unsigned gsize = min((unsigned)DOT_GROUP, nblk - grp * DOT_GROUP);
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         const double t = warp_sum(v[k]);
         if (lane == 0) sm[k][w] = t;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (threadIdx.x < 3) {
+        double t = 0;
+        for (int j = 0; j < NW; j++) t += sm[threadIdx.x][j];
+        part[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = t;  // [3][nblk]: coalesced for the finish kernel
+    }
+}
+
+template <int DOT>
+__global__ void __launch_bounds__(1024) dot_finish_kernel(const double* __restrict__ part, unsigned nblk, Scalars* sc) {
+    __shared__ double sm[3][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double t[3] = {0, 0, 0};
+    for (unsigned j = threadIdx.x; j < nblk; j += 1024)
 #pragma unroll
-        for (int k = 0; k < 3; k++) {
-            double t = 0;
-            for (int j = 0; j < NW; j++) t += sm[k][j];
-            part[(size_t)blockIdx.x * 3 + k] = t;
-        }
-        __threadfence();
-        stage = atomicInc(&tickets[1 + grp], gsize - 1) == gsize - 1 ? 1 : 0;
+        for (int k = 0; k < 3; k++) t[k] += part[(size_t)k * nblk + j];
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const double u = warp_sum(t[k]);
+        if (lane == 0) sm[k][w] = u;
     }
     __syncthreads();
-    if (!stage) return false;
-    __threadfence();
-    // last CTA of the group: fixed-order sum of the group's partials (warp 0 only)
     if (w == 0) {
-        double t[3] = {0, 0, 0};
-        for (unsigned j = lane; j < gsize; j += 32)
+        double tot[3];
 #pragma unroll
-            for (int k = 0; k < 3; k++) t[k] += __ldcg(&part[((size_t)grp * DOT_GROUP + j) * 3 + k]);
-#pragma unroll
-        for (int k = 0; k < 3; k++) t[k] = warp_sum(t[k]);
+        for (int k = 0; k < 3; k++) tot[k] = warp_sum(sm[k][lane]);
         if (lane == 0) {
-#pragma unroll
-            for (int k = 0; k < 3; k++) gpart[(size_t)grp * 3 + k] = t[k];
-            __threadfence();
-            stage = atomicInc(&tickets[0], ngrp - 1) == ngrp - 1 ? 2 : 1;
+            if (DOT == 1) {
+                sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
+                const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
+                sc->alpha[0] = a.r; sc->alpha[1] = a.i;
+            } else {
+                sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
+                sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
+                sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
+            }
         }
     }
-    __syncthreads();
-    if (stage != 2) return false;
-    __threadfence();
-    if (w == 0) {
-        double t[3] = {0, 0, 0};
-        for (unsigned j = lane; j < ngrp; j += 32)
-#pragma unroll
-            for (int k = 0; k < 3; k++) t[k] += __ldcg(&gpart[(size_t)j * 3 + k]);
-#pragma unroll
-        for (int k = 0; k < 3; k++) tot[k] = warp_sum(t[k]);
-        return lane == 0;
-    }
-    return false;
 }
 
 // DOT = 0: out = D in (XPAY: out = bsrc - D in).
@@ -96,8 +88,7 @@ template <typename T, bool XPAY, int TH, int MINB, int DOT>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
                                                      typename VecOf<T>::type* __restrict__ out,
                                                      const typename VecOf<T>::type* bsrc,
-                                                     const typename VecOf<T>::type* __restrict__ dotv, Scalars* sc,
-                                                     double* part, double* gpart, unsigned* tickets) {
+                                                     const typename VecOf<T>::type* __restrict__ dotv, double* part) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < g.V;
     if (!DOT && !valid) return;
@@ -143,20 +134,7 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
             dsum[0] = d0; dsum[1] = d1; dsum[2] = d2;
         }
     }
-    if (DOT) {
-        double tot[3];
-        if (dslash_grid_reduce<TH>(dsum, part, gpart, tickets, tot)) {
-            if (DOT == 1) {
-                sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
-                const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
-                sc->alpha[0] = a.r; sc->alpha[1] = a.i;
-            } else {
-                sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
-                sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
-                sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
-            }
-        }
-    }
+    if (DOT) dslash_block_partial<TH>(dsum, part);
 }
 
 struct Box {
@@ -236,25 +214,23 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
     constexpr int TH = 64;
     const unsigned grid = (V + TH - 1) / TH;
     if (dot) {
-        if (!ctx->dpart) {
-            const unsigned ngrp = (grid + DOT_GROUP - 1) / DOT_GROUP;
-            if (alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * 3 * grid)) return WCRAS_CUDA_ERROR;
-            if (alloc_dev(ctx, (void**)&ctx->dgpart, sizeof(double) * 3 * ngrp)) return WCRAS_CUDA_ERROR;
-            if (alloc_dev(ctx, (void**)&ctx->dtickets, sizeof(unsigned) * (ngrp + 1))) return WCRAS_CUDA_ERROR;
-            WC_CUDA(cudaMemsetAsync(ctx->dtickets, 0, sizeof(unsigned) * (ngrp + 1), ctx->stream));
-        }
-        if (dot == 1)
+        if (!ctx->dpart && alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * 3 * grid)) return WCRAS_CUDA_ERROR;
+        if (dot == 1) {
             dslash_kernel<T, false, TH, 1, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                            dotv, sc, ctx->dpart, ctx->dgpart, ctx->dtickets);
-        else
+                                                                            dotv, ctx->dpart);
+            dot_finish_kernel<1><<<1, 1024, 0, ctx->stream>>>(ctx->dpart, grid, sc);
+        } else {
             dslash_kernel<T, false, TH, 1, 2><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                            dotv, sc, ctx->dpart, ctx->dgpart, ctx->dtickets);
+                                                                            dotv, ctx->dpart);
+            dot_finish_kernel<2><<<1, 1024, 0, ctx->stream>>>(ctx->dpart, grid, sc);
+        }
+        ctx->launches++;
     } else if (b_minus) {
         dslash_kernel<T, true, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, b_minus,
-                                                                       nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                       nullptr, nullptr);
     } else {
         dslash_kernel<T, false, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                        nullptr, nullptr, nullptr, nullptr, nullptr);
+                                                                        nullptr, nullptr);
     }
     ctx->launches++;
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;

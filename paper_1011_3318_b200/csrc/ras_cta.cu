@@ -318,15 +318,18 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
                     __stcs(rho_out + (size_t)c * V + gi, make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]));
             }
             if (phi_in) {
+                // phi += v as a fire-and-forget vector reduction (phi_in == phi_out; one writer per site, so the
+                // result is the same single rounding as load-add-store, without waiting for the load)
 #pragma unroll
-                for (int c = 0; c < 6; c++) {
-                    const float4 o = phi_in[(size_t)c * V + gi];
-                    v[4 * c] += o.x; v[4 * c + 1] += o.y; v[4 * c + 2] += o.z; v[4 * c + 3] += o.w;
-                }
+                for (int c = 0; c < 6; c++)
+                    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(phi_out + (size_t)c * V + gi), "f"(v[4 * c]),
+                                 "f"(v[4 * c + 1]), "f"(v[4 * c + 2]), "f"(v[4 * c + 3])
+                                 : "memory");
+            } else {
+#pragma unroll
+                for (int c = 0; c < 6; c++)
+                    phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
-#pragma unroll
-            for (int c = 0; c < 6; c++)
-                phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
         }
     }
 }

@@ -178,8 +178,7 @@ struct wcras_ctx {
     wc::Scalars* sc_host = nullptr;  // pinned
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;
-    double *dpart = nullptr, *dgpart = nullptr;  // partials of the dots fused into the Dslash (per CTA, per group)
-    unsigned* dtickets = nullptr;
+    double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][grid]
     // timing
     int timing = 0;
     std::vector<cudaEvent_t> ev_pool;
