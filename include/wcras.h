@@ -116,6 +116,27 @@ int wcras_solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double t
 /* Same, with HOST buffers: copies eta to the device, solves, copies phi back (end-to-end entry point). */
 int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, double tol, wcras_info* info);
 
+/* One row of the parameter survey of wcras_ras_autotune. */
+typedef struct {
+    int domain[4];      /* block shape; all zero = no preconditioner */
+    int overlap_s, block_iters, nras;
+    int status;         /* status of the timed solve (WCRAS_OK, NOT_CONVERGED, BREAKDOWN) or WCRAS_UNSUPPORTED */
+    int inner_iters, ras_applies;
+    double ms;          /* device time of the timed solve */
+    double rel_resid_true;
+} wcras_tune_row;
+
+/* The paper's parameter survey ("we survey the best parameters for NRAS and N_dominv ... we find the
+ * best parameter", and :83-85 on the trade-off), run on this lattice and GPU: solves D phi = eta to `tol` once
+ * untimed and once timed for every candidate (overlap 0; block shapes of <= 256 sites with extents 2/4/8 that
+ * divide the lattice, plus 8x4x4x4 and 8x8x4x4; (N_dominv, NRAS) in {(2,2),(2,3),(2,4),(3,2),(3,3),(4,1),(4,2)};
+ * and the unpreconditioned solver), at most max_rows candidates.  The fastest converged candidate is left
+ * configured (wcras_ras_precondition + use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.
+ * table_host (may be NULL) receives the rows tried, *nrows their number.  eta_dev: device, canonical fp64.
+ * Uses the workspace of wcras_solve plus one scratch solution vector. */
+int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int max_rows, wcras_tune_row* best,
+                       wcras_tune_row* table_host, int* nrows);
+
 /* Export the packed clover term for checking: out_dev = [V][2][36] doubles (packing: 6 real diagonal
  * entries, then the 15 strictly-lower entries (i>j, k = i(i-1)/2 + j) as {re,im}). */
 int wcras_export_clover(wcras_ctx* ctx, double* out_dev);

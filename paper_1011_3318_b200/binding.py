@@ -18,7 +18,7 @@ OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, 
 EXPORTS = [
     "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_ras_precondition", "wcras_set_ras_tier",
     "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_timing", "wcras_solve",
-    "wcras_solve_host", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
+    "wcras_solve_host", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
 ]
 
 
@@ -31,6 +31,17 @@ class WcrasInfo(C.Structure):
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class WcrasTuneRow(C.Structure):
+    _fields_ = [("domain", C.c_int * 4), ("overlap_s", C.c_int), ("block_iters", C.c_int), ("nras", C.c_int),
+                ("status", C.c_int), ("inner_iters", C.c_int), ("ras_applies", C.c_int), ("ms", C.c_double),
+                ("rel_resid_true", C.c_double)]
+
+    def asdict(self):
+        d = {k: getattr(self, k) for k, _ in self._fields_ if k != "domain"}
+        d["domain"] = tuple(self.domain)
+        return d
 
 
 class WcrasError(RuntimeError):
@@ -142,6 +153,15 @@ class Context:
                                         C.byref(info))
         self._chk(rc, allow=() if strict else (NOT_CONVERGED, BREAKDOWN))
         return info.asdict()
+
+    def ras_autotune(self, eta_dev, tol, max_rows=256):
+        """Parameter survey (wcras_ras_autotune): returns (best row, list of all rows) and leaves best configured."""
+        best = WcrasTuneRow()
+        table = (WcrasTuneRow * max_rows)()
+        n = C.c_int(0)
+        self._chk(self._lib.wcras_ras_autotune(self._h, _ptr(eta_dev), C.c_double(tol), C.c_int(max_rows), C.byref(best),
+                                               table, C.byref(n)))
+        return best.asdict(), [table[k].asdict() for k in range(n.value)]
 
     def export_clover(self, out_dev):
         self._chk(self._lib.wcras_export_clover(self._h, _ptr(out_dev)))

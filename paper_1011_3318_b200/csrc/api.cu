@@ -158,6 +158,70 @@ int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, d
     return rc;
 }
 
+int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int max_rows, wcras_tune_row* best,
+                       wcras_tune_row* table_host, int* nrows) {
+    NEED(ctx, "null ctx");
+    NEED(eta_dev && best && tol > 0 && max_rows >= 1, "ras_autotune: bad arguments");
+    if (int rc = ensure_io(ctx)) return rc;
+    const int* L = ctx->geom.L;
+    std::vector<wcras_tune_row> rows;
+    auto add = [&](int b0, int b1, int b2, int b3, int it, int nras) {
+        wcras_tune_row r = {};
+        r.domain[0] = b0; r.domain[1] = b1; r.domain[2] = b2; r.domain[3] = b3;
+        r.block_iters = it; r.nras = nras;
+        rows.push_back(r);
+    };
+    add(0, 0, 0, 0, 0, 0);  // no preconditioner
+    static const int par[7][2] = {{2, 3}, {2, 2}, {2, 4}, {3, 2}, {3, 3}, {4, 1}, {4, 2}};
+    std::vector<std::vector<int>> shapes;
+    for (int b3 : {8, 4, 2}) for (int b2 : {8, 4, 2}) for (int b1 : {8, 4, 2}) for (int b0 : {8, 4, 2}) {
+        const int b[4] = {b0, b1, b2, b3};
+        long ns = 1;
+        bool ok = true;
+        for (int mu = 0; mu < 4; mu++) { ns *= b[mu]; ok = ok && L[mu] % b[mu] == 0; }
+        // persistent tier (<= 256 sites, not tiny) with x >= y >= z >= t to skip permutations of the same cut,
+        // and the two cluster-tier shapes BASELINE.json:configs name
+        const bool sorted = b0 >= b1 && b1 >= b2 && b2 >= b3;
+        const bool named = (b0 == 8 && b1 == 4 && b2 == 4 && b3 == 4) || (b0 == 8 && b1 == 8 && b2 == 4 && b3 == 4);
+        if (ok && ((sorted && ns <= 256 && ns >= 64) || named)) shapes.push_back({b0, b1, b2, b3});
+    }
+    for (int p = 0; p < 7; p++)
+        for (const auto& sh : shapes) add(sh[0], sh[1], sh[2], sh[3], par[p][0], par[p][1]);
+    if ((int)rows.size() > max_rows) rows.resize(max_rows);
+    double* phi = (double*)ctx->io_b;
+    int ibest = -1;
+    for (size_t k = 0; k < rows.size(); k++) {
+        wcras_tune_row& r = rows[k];
+        if (r.block_iters == 0) {
+            ctx->use_ras = 0;
+        } else {
+            const int rc = ras_configure(ctx, r.domain, 0, r.block_iters, r.nras);
+            if (rc == WCRAS_CUDA_ERROR) return rc;
+            if (rc) { r.status = WCRAS_UNSUPPORTED; r.ms = 0; continue; }
+            ctx->use_ras = 1;
+        }
+        wcras_info info;
+        int rc = WCRAS_OK;
+        for (int pass = 0; pass < 2; pass++) {  // pass 0 = warm-up
+            rc = solve(ctx, eta_dev, phi, tol, &info);
+            if (rc == WCRAS_CUDA_ERROR) return rc;
+        }
+        r.status = rc; r.ms = info.ms_total; r.inner_iters = info.inner_iters; r.ras_applies = info.ras_applies;
+        r.rel_resid_true = info.rel_resid_true;
+        if (rc == WCRAS_OK && (ibest < 0 || r.ms < rows[ibest].ms)) ibest = (int)k;
+    }
+    if (table_host) for (size_t k = 0; k < rows.size(); k++) table_host[k] = rows[k];
+    if (nrows) *nrows = (int)rows.size();
+    if (ibest < 0) {
+        snprintf(ctx->err, sizeof ctx->err, "ras_autotune: no candidate converged");
+        return WCRAS_NOT_CONVERGED;
+    }
+    *best = rows[ibest];
+    if (best->block_iters == 0) { ctx->use_ras = 0; return WCRAS_OK; }
+    ctx->use_ras = 1;
+    return ras_configure(ctx, best->domain, 0, best->block_iters, best->nras);
+}
+
 int wcras_export_clover(wcras_ctx* ctx, double* out_dev) {
     NEED(ctx, "null ctx");
     NEED(out_dev, "export_clover: null buffer");

@@ -270,6 +270,24 @@ def test_ras_reduces_iterations():
     assert i1["inner_iters"] < i0["inner_iters"]
 
 
+def test_ras_autotune():
+    """Parameter survey: the fastest converged row is returned and left configured."""
+    cs = case(1)
+    eta = I.spinor(cs.dims, 2)
+    x = dev(eta, torch.float64)
+    best, rows = cs.ctx.ras_autotune(x, 1e-12, max_rows=12)
+    assert len(rows) == 12 and rows[0]["block_iters"] == 0           # first row = no preconditioner
+    ok = [r for r in rows if r["status"] == 0]
+    assert ok and best["ms"] == min(r["ms"] for r in ok)
+    assert all(r["rel_resid_true"] <= 1e-12 for r in ok)
+    for r in rows[1:]:
+        assert all(d in (2, 4, 8) for d in r["domain"]) and r["overlap_s"] == 0
+    phi, info = cs.solve(eta, 1e-12)                                  # solves with the configuration left behind
+    assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+    assert (info["ras_applies"] > 0) == (best["block_iters"] > 0)
+    cs.ctx.set_solver(use_ras=False)
+
+
 @pytest.mark.parametrize("prec", [32, 64])
 def test_full_size_32_sampled(prec):
     """BASELINE.json:configs[3] at full size, the launch configuration bench.py times: D checked on sampled
