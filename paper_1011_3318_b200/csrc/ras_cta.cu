@@ -44,6 +44,12 @@ __device__ __forceinline__ void ld_half_cta(const float4* __restrict__ slot, int
         h[4 * j] = v.x; h[4 * j + 1] = v.y; h[4 * j + 2] = v.z; h[4 * j + 3] = v.w;
     }
 }
+// 16-byte asynchronous global -> shared copy (LDGSTS); the issuing thread waits for its own copies with cp_async_wait
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(cta_smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
@@ -113,7 +119,8 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     float4* hbuf = smem;            // [8][3][nsp]
-    float4* red = smem + 24 * nsp;  // [nwarps]
+    float4* As = smem + 24 * nsp;   // [18][nsp] clover blocks of the current domain (each thread reads back its own column)
+    float4* red = smem + 42 * nsp;  // [nwarps]
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const bool active = k < fg.ns;
 
@@ -155,15 +162,31 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
 
     const size_t V = fg.V;
     const unsigned dm_bytes = 36u * (unsigned)nsp * 16u;
+    // clover blocks: global -> shared with cp.async, into the thread's own column (only the owner reads it back, so
+    // no barrier is involved); the copy for the NEXT domain is issued right after the last use in the current one
+    if ((int)blockIdx.x < nd) {
+        const float4* p0 = dm + ((size_t)blockIdx.x * 36 + 18) * nsp + k;
+#pragma unroll
+        for (int c = 0; c < 18; c++) cp_async16(As + c * nsp + k, p0 + (size_t)c * nsp);
+        cp_async_commit();
+    }
+    float U[72];
+#define WC_LOAD_U(DOM)                                                                            \
+    {                                                                                             \
+        const float4* pu = dm + (size_t)(DOM) * 36 * nsp + k;                                     \
+        for (int c = 0; c < 18; c++) {                                                            \
+            const float4 t = __ldcs(pu + (size_t)c * nsp);                                        \
+            U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;           \
+        }                                                                                         \
+    }
+    if ((int)blockIdx.x < nd) {
+#pragma unroll
+        WC_LOAD_U(blockIdx.x)
+    }
     for (int dom = blockIdx.x; dom < nd; dom += gridDim.x) {
         const size_t gi = cta_site(fg, dom, lc);
-        float U[72], A[72], rho[24], v[24];
-        const float4* p = dm + (size_t)dom * 36 * nsp + k;
-#pragma unroll
-        for (int c = 0; c < 18; c++) {
-            const float4 t = __ldcs(p + (size_t)c * nsp);
-            U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;
-        }
+        float rho[24], v[24];
+        bool u_early = false;  // links of the next domain already requested in the last sweep of this one
         if (active) {
 #pragma unroll
             for (int c = 0; c < 6; c++) {
@@ -201,11 +224,6 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
             WC_CROSS(0) WC_CROSS(1) WC_CROSS(2) WC_CROSS(3)
 #undef WC_CROSS
         }
-#pragma unroll
-        for (int c = 0; c < 18; c++) {
-            const float4 t = __ldcs(p + (size_t)(18 + c) * nsp);
-            A[4 * c] = t.x; A[4 * c + 1] = t.y; A[4 * c + 2] = t.z; A[4 * c + 3] = t.w;
-        }
         // ---- pull the next domain of this CTA towards L2 while this one is solved ----
         {
             const int nxt = dom + gridDim.x;
@@ -235,7 +253,23 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
 #undef WC_SCATTER
             }
             float q[24];
-            clover_apply<float>(A, rho, q);
+            if (it == 0) cp_async_wait();
+#pragma unroll
+            for (int ch = 0; ch < 2; ch++) {
+                float Ab[36];
+#pragma unroll
+                for (int c = 0; c < 9; c++) {
+                    const float4 t = As[(9 * ch + c) * nsp + k];
+                    Ab[4 * c] = t.x; Ab[4 * c + 1] = t.y; Ab[4 * c + 2] = t.z; Ab[4 * c + 3] = t.w;
+                }
+                herm6_mul<float>(Ab, rho + 12 * ch, q + 12 * ch);
+            }
+            if (it + 1 == fg.niter && dom + (int)gridDim.x < nd) {
+                const float4* pn = dm + ((size_t)(dom + gridDim.x) * 36 + 18) * nsp + k;
+#pragma unroll
+                for (int c = 0; c < 18; c++) cp_async16(As + c * nsp + k, pn + (size_t)c * nsp);
+                cp_async_commit();
+            }
             __syncthreads();
             {
                 float h[12], g[12];
@@ -247,6 +281,13 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
     reconstruct_add<float, MU, +1>(g, q);
                 WC_GATHER(0) WC_GATHER(1) WC_GATHER(2) WC_GATHER(3)
 #undef WC_GATHER
+            }
+            // the links are dead after the last gather unless the halo scatter still needs them: request those of
+            // the next domain now, their latency hides behind the dots, the update and the stores
+            if (it + 1 == fg.niter && hb_out == nullptr && dom + (int)gridDim.x < nd) {
+#pragma unroll
+                WC_LOAD_U(dom + gridDim.x)
+                u_early = true;
             }
             float d0 = 0.f, d1 = 0.f, d2 = 0.f;
 #pragma unroll
@@ -331,11 +372,16 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
+        if (!u_early && dom + (int)gridDim.x < nd) {
+#pragma unroll
+            WC_LOAD_U(dom + gridDim.x)
+        }
     }
+#undef WC_LOAD_U
 }
 
 // ---- host side ----
-static size_t cta_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)24 * fg.nsp + fg.nsp / 32); }
+static size_t cta_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)42 * fg.nsp + fg.nsp / 32); }
 
 // allocate and fill the domain-major operand copy; sets ctx->dm and the persistent grid size
 int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
