@@ -32,21 +32,18 @@ template <typename T> __device__ __forceinline__ cpx<T> ld_scalar(const double* 
 
 #define GRID_STRIDE(idx, n) for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (n); idx += (size_t)gridDim.x * blockDim.x)
 
-// r = b, rt = b, x = 0, p = v = 0; bb = |b|^2; scalars reset
+// bb = |b|^2; scalars reset.  No vector is written: the first iteration reads b in place of r (p = b, s = b - alpha v),
+// writes x instead of updating it, and the shadow residual rt is b itself ("first iteration").
 template <typename T, typename Vec>
-__global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __restrict__ b, Vec* r, Vec* rt, Vec* x, Vec* p, Vec* v,
-                                                      Scalars* sc, double* partials, unsigned* ticket) {
+__global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __restrict__ b, Scalars* sc, double* partials,
+                                                      unsigned* ticket) {
     constexpr int N = Cx<Vec>::N;
     double acc[1] = {0};
-    Vec zero;
-    memset(&zero, 0, sizeof zero);
     GRID_STRIDE(k, n) {
-        const Vec bv = b[k];
         cpx<T> c[N];
-        unpack<T>(bv, c);
+        unpack<T>(b[k], c);
 #pragma unroll
         for (int j = 0; j < N; j++) acc[0] += (double)c[j].r * c[j].r + (double)c[j].i * c[j].i;
-        r[k] = bv; rt[k] = bv; x[k] = zero; p[k] = zero; v[k] = zero;
     }
     double tot[1];
     if (grid_reduce<1>(acc, partials, ticket, tot)) {
@@ -83,8 +80,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_restart(size_t n, const Vec* __
 // p = r + beta (p - omega v), beta = (rho/rho_old)(alpha/omega)
 template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* __restrict__ r, Vec* __restrict__ p,
-                                                          const Vec* __restrict__ v, const Scalars* __restrict__ sc) {
+                                                          const Vec* __restrict__ v, const Scalars* __restrict__ sc, int first) {
     constexpr int N = Cx<Vec>::N;
+    if (first) {  // p = v = 0 before the first iteration: p = r (= b), nothing else is read
+        GRID_STRIDE(k, n) p[k] = r[k];
+        return;
+    }
     const cd b = cmul(cdiv({sc->rho[0], sc->rho[1]}, {sc->rho_old[0], sc->rho_old[1]}),
                       cdiv({sc->alpha[0], sc->alpha[1]}, {sc->omega[0], sc->omega[1]}));
     const cpx<T> beta = {(T)b.r, (T)b.i}, omega = ld_scalar<T>(sc->omega);
@@ -125,13 +126,19 @@ template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_update_xr(size_t n, Vec* __restrict__ x, const Vec* __restrict__ ph,
                                                            const Vec* __restrict__ sh, const Vec* __restrict__ s,
                                                            const Vec* __restrict__ t, const Vec* __restrict__ rt, Vec* __restrict__ r,
-                                                           Scalars* sc, double* partials, unsigned* ticket) {
+                                                           Scalars* sc, double* partials, unsigned* ticket, int first) {
     constexpr int N = Cx<Vec>::N;
     const cpx<T> alpha = ld_scalar<T>(sc->alpha), omega = ld_scalar<T>(sc->omega);
     double acc[3] = {0, 0, 0};
     GRID_STRIDE(k, n) {
         cpx<T> xc[N], pc[N], hc[N], sc_[N], tc[N], rc[N];
-        unpack<T>(x[k], xc); unpack<T>(ph[k], pc); unpack<T>(sh[k], hc);
+        if (first) {  // x = 0 before the first iteration
+#pragma unroll
+            for (int j = 0; j < N; j++) xc[j] = {0, 0};
+        } else {
+            unpack<T>(x[k], xc);
+        }
+        unpack<T>(ph[k], pc); unpack<T>(sh[k], hc);
         unpack<T>(s[k], sc_); unpack<T>(t[k], tc); unpack<T>(rt[k], rc);
 #pragma unroll
         for (int j = 0; j < N; j++) {
@@ -154,12 +161,18 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_xr(size_t n, Vec* __rest
 // x += alpha ph (half-step exit)
 template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_axpy_alpha(size_t n, Vec* __restrict__ x, const Vec* __restrict__ ph,
-                                                            const Scalars* __restrict__ sc) {
+                                                            const Scalars* __restrict__ sc, int first) {
     constexpr int N = Cx<Vec>::N;
     const cpx<T> alpha = ld_scalar<T>(sc->alpha);
     GRID_STRIDE(k, n) {
         cpx<T> xc[N], pc[N];
-        unpack<T>(x[k], xc); unpack<T>(ph[k], pc);
+        if (first) {
+#pragma unroll
+            for (int j = 0; j < N; j++) xc[j] = {0, 0};
+        } else {
+            unpack<T>(x[k], xc);
+        }
+        unpack<T>(ph[k], pc);
 #pragma unroll
         for (int j = 0; j < N; j++) xc[j] = xc[j] + alpha * pc[j];
         x[k] = pack(xc, (Vec*)nullptr);
@@ -243,16 +256,22 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
     unsigned* tk = ctx->ticket;
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH((k_init<T, Vec>), n, b, w.r, w.rt, x, w.p, w.v, w.sc, part, tk);
+        LAUNCH((k_init<T, Vec>), n, b, w.sc, part, tk);
     }
     if (int rc = read_scalars(ctx, w.sc)) return rc;
     const double bb = ctx->sc_host->bb;
     *iters = 0;
     *relres = 0;
-    if (bb == 0.0) return WCRAS_OK;
+    if (bb == 0.0) {
+        WC_CUDA(cudaMemsetAsync(x, 0, sizeof(Vec) * n, ctx->stream));
+        return WCRAS_OK;
+    }
     Vec* ph = k_identity ? w.p : w.ph;
     Vec* sh = k_identity ? w.s : w.sh;
     const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
+    const Vec* rt = b;    // shadow residual = initial residual = b (x0 = 0); a restart switches to the copy in w.rt
+    const Vec* rcur = b;  // residual read by the first iteration; w.r from the first r = s - omega t on
+    bool x_written = false;
     int it = 0, restarts = 0, status = WCRAS_NOT_CONVERGED;
     double rr = bb, best = bb;
     int it_best = 0;
@@ -261,23 +280,25 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
         if (hypot(h.rho[0], h.rho[1]) < tiny * bb || (it > 0 && hypot(h.omega[0], h.omega[1]) < tiny)) {
             if (restarts++) { status = WCRAS_BREAKDOWN; break; }
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_restart<T, Vec>), n, w.r, w.rt, w.p, w.v, w.sc, part, tk);
+            LAUNCH((k_restart<T, Vec>), n, rcur, w.rt, w.p, w.v, w.sc, part, tk);
+            rt = w.rt;
         }
         {
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_p<T, Vec>), n, w.r, w.p, w.v, w.sc);
+            LAUNCH((k_update_p<T, Vec>), n, rcur, w.p, w.v, w.sc, (it == 0 && restarts == 0) ? 1 : 0);
         }
         if (!k_identity) if (int rc = K(w.p, ph)) return rc;
-        if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, w.rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
+        if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
         {
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_s<T, Vec>), n, w.r, w.v, w.s, w.sc, part, tk);
+            LAUNCH((k_update_s<T, Vec>), n, rcur, w.v, w.s, w.sc, part, tk);
         }
         if (half_exit) {
             if (int rc = read_scalars(ctx, w.sc)) return rc;
             if (std::sqrt(ctx->sc_host->ss / bb) < tol) {
                 TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_axpy_alpha<T, Vec>), n, x, ph, w.sc);
+                LAUNCH((k_axpy_alpha<T, Vec>), n, x, ph, w.sc, x_written ? 0 : 1);
+                x_written = true;
                 rr = ctx->sc_host->ss;
                 it++;
                 status = WCRAS_OK;
@@ -288,7 +309,9 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
         if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
         {
             TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, w.rt, w.r, w.sc, part, tk);
+            LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, rt, w.r, w.sc, part, tk, x_written ? 0 : 1);
+            x_written = true;
+            rcur = w.r;
         }
         it++;
         if (int rc = read_scalars(ctx, w.sc)) return rc;
@@ -299,6 +322,7 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
         if (rr < best) { best = rr; it_best = it; }
         else if (it - it_best >= 10) break;
     }
+    if (!x_written) WC_CUDA(cudaMemsetAsync(x, 0, sizeof(Vec) * n, ctx->stream));  // left before the first update of x
     WC_CHECK_LAUNCH();
     *iters = it;
     *relres = std::sqrt(rr / bb);
@@ -397,14 +421,15 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
 
     double2 *eta = ctx->w64[8], *phi = ctx->w64[9], *res = ctx->w64[10], *dx = ctx->w64[11];
     if (int rc = to_internal(ctx, 64, eta_dev, eta)) return rc;
-    WC_CUDA(cudaMemsetAsync(phi, 0, sizeof(double2) * n64, ctx->stream));
-    WC_CUDA(cudaMemcpyAsync(res, eta, sizeof(double2) * n64, cudaMemcpyDeviceToDevice, ctx->stream));
     LAUNCH(k_norm2_d, n64, eta, ctx->sc64, ctx->partials, ctx->ticket);
     if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
     const double en2 = ctx->sc_host->nrm;
     double rn2 = en2, recur = 1.0;
     int outer = 0, inner_iters = 0, inner_solves = 0, status = WCRAS_NOT_CONVERGED;
-    if (en2 == 0.0) status = WCRAS_OK;
+    if (en2 == 0.0) {  // zero source: phi = 0
+        status = WCRAS_OK;
+        WC_CUDA(cudaMemsetAsync(phi, 0, sizeof(double2) * n64, ctx->stream));
+    }
     Work<double> w = work64(ctx);
     auto K = [&](const double2* in, double2* out) { return inner_solve(ctx, in, out, &inner_iters, &inner_solves); };
     for (int pass = 0; pass < 10 && status != WCRAS_OK && outer < ctx->outer_maxit; pass++) {
@@ -413,11 +438,14 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         // solve D dx = res to relative accuracy tol*|eta|/|res| so that the total residual meets tol
         const double tol_pass = 0.7 * tol * std::sqrt(en2 / rn2);
         ctx->outer_target = tol_pass * std::sqrt(rn2);  // absolute |r| this pass has to reach
-        int rc = bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel);
+        // pass 0: phi = 0 and res = eta, so the solver works on eta and writes phi directly; later passes solve
+        // D dx = res for the correction and add it
+        int rc = pass == 0 ? bicgstab<double>(ctx, w, eta, phi, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel)
+                           : bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel);
         if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
         outer += it;
         recur = rel * std::sqrt(rn2 / en2);
-        {
+        if (pass > 0) {
             TimedRegion tr(ctx, TC_BLAS);
             LAUNCH(k_add_d, n64, phi, dx);
         }
@@ -469,7 +497,7 @@ int time_blas(wcras_ctx* ctx, int reps, double* ms) {
     for (int k = 0; k < 8; k++) WC_CUDA(cudaMemsetAsync(ctx->w32[k], 0, sizeof(float4) * w.n, ctx->stream));
     WC_CUDA(cudaEventRecord(e0, ctx->stream));
     for (int k = 0; k < reps; k++)
-        LAUNCH((k_update_xr<float, float4>), w.n, ctx->w32[9], w.ph, w.sh, w.s, w.t, w.rt, w.r, w.sc, ctx->partials, ctx->ticket);
+        LAUNCH((k_update_xr<float, float4>), w.n, ctx->w32[9], w.ph, w.sh, w.s, w.t, w.rt, w.r, w.sc, ctx->partials, ctx->ticket, 0);
     WC_CUDA(cudaEventRecord(e1, ctx->stream));
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
     float t = 0;
