@@ -29,8 +29,8 @@ __device__ __forceinline__ void hop_pair(const Fields<T>& f, size_t V, const Geo
 
 // Dots fused into the Dslash (north_star (d)): every CTA reduces its 3 sums (warp shuffle -> shared memory) and
 // stores one partial, with no fence or atomic on the way (a __threadfence per 64-thread CTA would wait for the
-// CTA's output stores and cost ~15 % of the kernel).  dot_finish_kernel, one 1024-thread CTA launched right
-// behind it, sums the partials in a fixed order and finishes the scalar recurrence: deterministic.
+// CTA's output stores and cost ~15 % of the kernel).  dot_finish_kernel, 16 CTAs launched right behind it, sums
+// the partials in a fixed order and finishes the scalar recurrence: deterministic.
 template <int TH>
 __device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __restrict__ part) {
     constexpr int NW = TH / 32;
@@ -49,12 +49,18 @@ __device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __r
     }
 }
 
+// FIN_CTAS CTAs each sum a contiguous slice of the partials in a fixed order; the last one to finish (atomic ticket)
+// sums the FIN_CTAS slice sums in a fixed order and finishes the scalar recurrence.
+constexpr int FIN_CTAS = 16;
 template <int DOT>
-__global__ void __launch_bounds__(1024) dot_finish_kernel(const double* __restrict__ part, unsigned nblk, Scalars* sc) {
-    __shared__ double sm[3][32];
+__global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restrict__ part, unsigned nblk, double* __restrict__ slice,
+                                                         unsigned* ticket, Scalars* sc) {
+    __shared__ double sm[3][16];
+    __shared__ bool last;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned per = (nblk + FIN_CTAS - 1) / FIN_CTAS, lo = blockIdx.x * per, hi = min(nblk, lo + per);
     double t[3] = {0, 0, 0};
-    for (unsigned j = threadIdx.x; j < nblk; j += 1024)
+    for (unsigned j = lo + threadIdx.x; j < hi; j += 512)
 #pragma unroll
         for (int k = 0; k < 3; k++) t[k] += part[(size_t)k * nblk + j];
 #pragma unroll
@@ -64,20 +70,31 @@ __global__ void __launch_bounds__(1024) dot_finish_kernel(const double* __restri
     }
     __syncthreads();
     if (w == 0) {
-        double tot[3];
 #pragma unroll
-        for (int k = 0; k < 3; k++) tot[k] = warp_sum(sm[k][lane]);
-        if (lane == 0) {
-            if (DOT == 1) {
-                sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
-                const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
-                sc->alpha[0] = a.r; sc->alpha[1] = a.i;
-            } else {
-                sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
-                sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
-                sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
-            }
+        for (int k = 0; k < 3; k++) {
+            const double u = warp_sum(lane < 16 ? sm[k][lane] : 0.0);
+            if (lane == 0) slice[blockIdx.x * 3 + k] = u;
         }
+        if (lane == 0) {
+            __threadfence();
+            last = atomicInc(ticket, FIN_CTAS - 1) == FIN_CTAS - 1;
+        }
+    }
+    __syncthreads();
+    if (!last || threadIdx.x != 0) return;
+    __threadfence();
+    double tot[3] = {0, 0, 0};
+    for (int j = 0; j < FIN_CTAS; j++)
+#pragma unroll
+        for (int k = 0; k < 3; k++) tot[k] += __ldcg(&slice[j * 3 + k]);
+    if (DOT == 1) {
+        sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
+        const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
+        sc->alpha[0] = a.r; sc->alpha[1] = a.i;
+    } else {
+        sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
+        sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
+        sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
     }
 }
 
@@ -214,15 +231,20 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
     constexpr int TH = 64;
     const unsigned grid = (V + TH - 1) / TH;
     if (dot) {
-        if (!ctx->dpart && alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * 3 * grid)) return WCRAS_CUDA_ERROR;
+        if (!ctx->dpart) {  // [3][grid] per-CTA partials, then [FIN_CTAS][3] slice sums and one ticket
+            if (alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * (3 * (size_t)grid + 3 * FIN_CTAS + 1))) return WCRAS_CUDA_ERROR;
+            WC_CUDA(cudaMemsetAsync(ctx->dpart + 3 * (size_t)grid + 3 * FIN_CTAS, 0, sizeof(double), ctx->stream));
+        }
+        double* slice = ctx->dpart + 3 * (size_t)grid;
+        unsigned* fticket = (unsigned*)(slice + 3 * FIN_CTAS);
         if (dot == 1) {
             dslash_kernel<T, false, TH, 1, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
                                                                             dotv, ctx->dpart);
-            dot_finish_kernel<1><<<1, 1024, 0, ctx->stream>>>(ctx->dpart, grid, sc);
+            dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, grid, slice, fticket, sc);
         } else {
             dslash_kernel<T, false, TH, 1, 2><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
                                                                             dotv, ctx->dpart);
-            dot_finish_kernel<2><<<1, 1024, 0, ctx->stream>>>(ctx->dpart, grid, sc);
+            dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, grid, slice, fticket, sc);
         }
         ctx->launches++;
     } else if (b_minus) {
