@@ -138,6 +138,15 @@ class Operator:
             raise ValueError("invalid domain decomposition")
         return out
 
+    def sap_apply(self, block, niter, ncycle, eta):
+        """Multiplicative Schwarz (SAP, PAPER.md:33 ref [5]), overlap 0, red-black domains."""
+        eta = _c(eta)
+        out = np.empty((self.V, 4, 3), np.complex128)
+        rc = _load().wco_sap_apply(*self._args(), _i4(block), C.c_int(niter), C.c_int(ncycle), _p(eta), _p(out))
+        if rc:
+            raise ValueError("invalid or not two-colourable domain decomposition")
+        return out
+
     def bicgstab(self, eta, tol=1e-12, maxit=10000, ras=None):
         """Flat fp64 BiCGStab; ras = None or dict(domain, overlap, block_iters, nras)."""
         eta = _c(eta)

@@ -179,6 +179,54 @@ def test_alg1_equals_eq21(small, s, nras):
         assert np.abs(S[np.ix_(comp, rest)]).max() == 0
 
 
+@pytest.mark.parametrize("ncycle", [1, 2])
+def test_sap_equals_block_gauss_seidel(small, ncycle):
+    """Multiplicative Schwarz (SAP, PAPER.md:33 ref [5]) with exact block solves == the dense
+    red-black block Gauss-Seidel iteration phi += S_c r, r -= D S_c r over the colours c = 0, 1; a black half step
+    leaves a zero residual on the black domains; and SAP reduces the residual further than RAS with the same number
+    of cycles."""
+    dims = (4, 4, 2, 2)  # 2 x 2 x 1 x 1 blocks: even in every cut direction
+    op = O.Operator(dims, I.gauge_exp(dims, 0.5, 7), 0.12, 1.0)
+    D = dense_from(op.apply_D, 12 * op.V)
+    block = (2, 2, 2, 2)
+    n = D.shape[0]
+    nblk = [dims[mu] // block[mu] for mu in range(4)]
+    Sc = [np.zeros((n, n), complex), np.zeros((n, n), complex)]
+    comps = [[], []]
+    for idx in range(op.domain_count(block)):
+        bc, par = idx, 0
+        for mu in range(4):
+            par += bc % nblk[mu]
+            bc //= nblk[mu]
+        origin, start, ext = op.domain_box(block, 0, idx)
+        sites = box_sites(dims, start, ext)
+        comp = (12 * sites[:, None] + np.arange(12)[None]).reshape(-1)
+        Sc[par & 1][np.ix_(comp, comp)] = np.linalg.inv(D[np.ix_(comp, comp)])
+        comps[par & 1].append(comp)
+    eta = I.spinor(dims, 8)
+    r = eta.reshape(-1).copy()
+    phi = np.zeros(n, complex)
+    for cyc in range(ncycle):
+        for c in (0, 1):
+            v = Sc[c] @ r
+            phi += v
+            r = r - D @ v
+            assert np.abs(r[np.concatenate(comps[c])]).max() < 1e-12   # exact solve: residual vanishes there
+    got = op.sap_apply(block, 400, ncycle, eta).reshape(-1)
+    assert np.abs(got - phi).max() < 1e-10 * np.abs(phi).max()
+    res_sap = np.linalg.norm(eta.reshape(-1) - D @ got)
+    ras = op.ras_apply(block, 0, 400, ncycle, eta).reshape(-1)
+    assert res_sap < np.linalg.norm(eta.reshape(-1) - D @ ras)
+
+
+def test_sap_needs_two_colourable_decomposition(small):
+    dims, op, D = small
+    with pytest.raises(ValueError):
+        op.sap_apply(dims, 3, 1, I.spinor(dims, 1))           # a single domain cannot be coloured
+    with pytest.raises(ValueError):
+        op.sap_apply((2, 2, 2, 2), 3, 1, I.spinor(dims, 1))   # 3 blocks in x: neighbours across the wrap share a colour
+
+
 def test_ras_single_domain_is_inverse(small):
     """north_star self-check 5: one domain covering the whole lattice + exact block solve => phi = D^-1 eta."""
     dims, op, D = small
