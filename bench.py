@@ -35,6 +35,7 @@ TOL = 1e-12
 RAS = dict(domain=(4, 4, 4, 4), overlap=0, block_iters=2, nras=3)
 RAS_NAMED = [dict(domain=(8, 8, 4, 4), overlap=0, block_iters=3, nras=2),
              dict(domain=(8, 8, 8, 8), overlap=0, block_iters=5, nras=1)]
+SAP = dict(domain=(4, 4, 4, 4), block_iters=3, ncycle=2)
 INNER_TOL = 5e-7
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
 # `ncu --set full` capture (profiles/r1b_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
@@ -200,6 +201,17 @@ def main():
         named["ras_%s_it%d_nras%d" % ("x".join(map(str, rp["domain"])), rp["block_iters"], rp["nras"])] = {
             k: i[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies",
                               "rel_resid_true", "ms_total")}
+
+    # ---- multiplicative Schwarz (SAP) beside it: same kernel, red-black half steps ----
+    ctx.set_schwarz(True)
+    ctx.ras_precondition(SAP["domain"], 0, SAP["block_iters"], SAP["ncycle"])
+    ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+    ctx.solve(eta_d, phi_d, TOL)
+    i = ctx.solve(eta_d, phi_d, TOL)
+    named["sap_%s_it%d_ncycle%d" % ("x".join(map(str, SAP["domain"])), SAP["block_iters"], SAP["ncycle"])] = {
+        k: i[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies",
+                          "rel_resid_true", "ms_total")}
+    ctx.set_schwarz(False)
 
     # ---- the timed step: RAS-preconditioned nested solve ----
     ctx.ras_precondition(RAS["domain"], RAS["overlap"], RAS["block_iters"], RAS["nras"])

@@ -88,6 +88,14 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
  * Call before wcras_ras_precondition. */
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
 
+/* Schwarz variant applied by wcras_ras_apply and the solver: 0 = additive with restriction (RAS, Alg. 1 -- the paper's
+ * method and the default), 1 = multiplicative (SAP, the related method PAPER.md:33 names, ref. [5]; SURVEY.md 8(f)
+ * NEXT-4): the domains are coloured red/black by the parity of their block coordinates and `nras` cycles of (black
+ * half step, red half step) are run, each half step solving with the residual left by the previous one.  Needs
+ * overlap 0, domains of <= 256 sites (persistent-CTA tier) and an even number of blocks in every cut direction;
+ * otherwise wcras_ras_apply / wcras_solve return WCRAS_UNSUPPORTED. */
+int wcras_set_schwarz(wcras_ctx* ctx, int multiplicative);
+
 /* out = P'^T D_Omega' P' in : the principal sub-matrix of D on the extended domain Omega'_index of the
  * current decomposition ("restriction of D ... with the Dirichlet boundary condition"; reading
  * Q7), on full-lattice canonical vectors; out = 0 outside Omega'.  domain_index = -1 applies all domains at

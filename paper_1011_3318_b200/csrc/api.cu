@@ -85,6 +85,13 @@ int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     return WCRAS_OK;
 }
 
+int wcras_set_schwarz(wcras_ctx* ctx, int multiplicative) {
+    NEED(ctx, "null ctx");
+    NEED(multiplicative == 0 || multiplicative == 1, "set_schwarz: 0 (additive, RAS) or 1 (multiplicative, SAP)");
+    ctx->schwarz = multiplicative;
+    return WCRAS_OK;
+}
+
 int wcras_apply_D_restricted(wcras_ctx* ctx, int prec, int domain_index, const void* in_dev, void* out_dev) {
     NEED(ctx, "null ctx");
     NEED(in_dev && out_dev && in_dev != out_dev, "apply_D_restricted: null or aliased buffers");

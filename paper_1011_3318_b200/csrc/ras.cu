@@ -204,6 +204,8 @@ int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool ac
 int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_cta_sap_pdir(const FusedGeom& fg);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
     RasConfig rc;
@@ -242,6 +244,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         ctx->dm = nullptr;
     }
     if (rc.tier == 2) {
+        fgeom.pdir = ras_cta_sap_pdir(fgeom);
         ctx->fused = fgeom;
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
     }
@@ -291,6 +294,13 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     const RasConfig& rc = ctx->ras;
     if (!rc.set) { snprintf(ctx->err, sizeof ctx->err, "ras_apply: call wcras_ras_precondition first"); return WCRAS_INVALID_ARG; }
     ctx->ras_applies++;
+    if (ctx->schwarz == 1) {
+        if (!(rc.tier == 2 && rc.cta && rc.s == 0 && ctx->fused.pdir >= 0)) {
+            snprintf(ctx->err, sizeof ctx->err, "multiplicative Schwarz needs overlap 0, domains of <= 256 sites and an even number of blocks in every cut direction");
+            return WCRAS_UNSUPPORTED;
+        }
+        return ras_cta_apply_sap(ctx, r, v);
+    }
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);

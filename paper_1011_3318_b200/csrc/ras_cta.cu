@@ -74,6 +74,24 @@ __device__ __forceinline__ size_t cta_site(const FusedGeom& fg, int dom, const i
     return cta_site(fg, dom, lc, x);
 }
 
+// domain handled as the h-th of a launch: all domains (colour < 0), or the domains of one colour of the red-black
+// (checkerboard) colouring by the parity of the block coordinates (multiplicative Schwarz).  fg.pdir is a direction
+// with an even number >= 2 of blocks; h enumerates the lattice of blocks with that direction halved.
+__device__ __forceinline__ int launch_dom(const FusedGeom& fg, int h, int colour) {
+    if (colour < 0) return h;
+    int dom = 0, stride = 1, par = 0, cp = 0, sp = 1;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        const int nb = fg.nblk[mu], n = mu == fg.pdir ? nb / 2 : nb;
+        const int c = h % n;
+        h /= n;
+        if (mu == fg.pdir) { cp = c; sp = stride; }
+        else { par += c; dom += c * stride; }
+        stride *= nb;
+    }
+    return dom + (2 * cp + ((colour + par) & 1)) * sp;
+}
+
 // pack the domain-major operand copy: one thread per (domain, local site)
 __global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, float mkappa, float4* __restrict__ dm) {
     const int dom = blockIdx.x, k = threadIdx.x;
@@ -113,7 +131,7 @@ __global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, 
 //   rho_out rho_fin of this cycle, or nullptr (then the last MR residual update is skipped, Q12)
 template <bool CHAIN>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
-ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, const float4* __restrict__ r_src,
+ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __restrict__ dm, const float4* __restrict__ r_src,
                const float4* __restrict__ hb_in, float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out,
                float4* rho_out) {
     extern __shared__ float4 smem[];
@@ -164,8 +182,9 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
     const unsigned dm_bytes = 36u * (unsigned)nsp * 16u;
     // clover blocks: global -> shared with cp.async, into the thread's own column (only the owner reads it back, so
     // no barrier is involved); the copy for the NEXT domain is issued right after the last use in the current one
-    if ((int)blockIdx.x < nd) {
-        const float4* p0 = dm + ((size_t)blockIdx.x * 36 + 18) * nsp + k;
+    const int dom0 = launch_dom(fg, blockIdx.x, colour);
+    if ((int)blockIdx.x < ndl) {
+        const float4* p0 = dm + ((size_t)dom0 * 36 + 18) * nsp + k;
 #pragma unroll
         for (int c = 0; c < 18; c++) cp_async16(As + c * nsp + k, p0 + (size_t)c * nsp);
         cp_async_commit();
@@ -179,11 +198,14 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
             U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;           \
         }                                                                                         \
     }
-    if ((int)blockIdx.x < nd) {
+    if ((int)blockIdx.x < ndl) {
 #pragma unroll
-        WC_LOAD_U(blockIdx.x)
+        WC_LOAD_U(dom0)
     }
-    for (int dom = blockIdx.x; dom < nd; dom += gridDim.x) {
+    for (int h = blockIdx.x; h < ndl; h += gridDim.x) {
+        const int dom = launch_dom(fg, h, colour);
+        const bool has_next = h + (int)gridDim.x < ndl;
+        const int nxt = launch_dom(fg, has_next ? h + gridDim.x : h, colour);
         const size_t gi = cta_site(fg, dom, lc);
         float rho[24], v[24];
         bool u_early = false;  // links of the next domain already requested in the last sweep of this one
@@ -226,8 +248,7 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
         }
         // ---- pull the next domain of this CTA towards L2 while this one is solved ----
         {
-            const int nxt = dom + gridDim.x;
-            if (nxt < nd) {
+            if (has_next) {
                 if (k == 0) prefetch_l2_bulk(dm + (size_t)nxt * 36 * nsp, dm_bytes);
                 if (CHAIN && k == 32) prefetch_l2_bulk(hb_in + (size_t)nxt * 24 * nface, 24u * (unsigned)nface * 16u);
                 if (active) {
@@ -264,8 +285,8 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
                 }
                 herm6_mul<float>(Ab, rho + 12 * ch, q + 12 * ch);
             }
-            if (it + 1 == fg.niter && dom + (int)gridDim.x < nd) {
-                const float4* pn = dm + ((size_t)(dom + gridDim.x) * 36 + 18) * nsp + k;
+            if (it + 1 == fg.niter && has_next) {
+                const float4* pn = dm + ((size_t)nxt * 36 + 18) * nsp + k;
 #pragma unroll
                 for (int c = 0; c < 18; c++) cp_async16(As + c * nsp + k, pn + (size_t)c * nsp);
                 cp_async_commit();
@@ -284,9 +305,9 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
             }
             // the links are dead after the last gather unless the halo scatter still needs them: request those of
             // the next domain now, their latency hides behind the dots, the update and the stores
-            if (it + 1 == fg.niter && hb_out == nullptr && dom + (int)gridDim.x < nd) {
+            if (it + 1 == fg.niter && hb_out == nullptr && has_next) {
 #pragma unroll
-                WC_LOAD_U(dom + gridDim.x)
+                WC_LOAD_U(nxt)
                 u_early = true;
             }
             float d0 = 0.f, d1 = 0.f, d2 = 0.f;
@@ -372,9 +393,9 @@ ras_cta_kernel(FusedGeom fg, int nd, int nface, const float4* __restrict__ dm, c
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
-        if (!u_early && dom + (int)gridDim.x < nd) {
+        if (!u_early && has_next) {
 #pragma unroll
-            WC_LOAD_U(dom + gridDim.x)
+            WC_LOAD_U(nxt)
         }
     }
 #undef WC_LOAD_U
@@ -425,7 +446,7 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
     ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(
-        fg, ctx->ras.nd, ctx->nface, ctx->dm, r, nullptr, nullptr, accum ? vout : nullptr, vout, nullptr);
+        fg, ctx->ras.nd, -1, ctx->nface, ctx->dm, r, nullptr, nullptr, accum ? vout : nullptr, vout, nullptr);
     ctx->launches++;
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
@@ -444,11 +465,54 @@ int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
         TimedRegion tr(ctx, TC_BLOCK);
         ctx->block_dv += ctx->ras.niter;
         if (j == 0)
-            ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, nface, ctx->dm, r, nullptr, last ? nullptr : hb[0],
+            ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, r, nullptr, last ? nullptr : hb[0],
                                                                                 nullptr, v, last ? nullptr : rf);
         else
-            ras_cta_kernel<true><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, nface, ctx->dm, rf, hb[(j - 1) & 1],
+            ras_cta_kernel<true><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, rf, hb[(j - 1) & 1],
                                                                                last ? nullptr : hb[j & 1], v, v, last ? nullptr : rf);
+        ctx->launches++;
+    }
+    WC_CHECK_LAUNCH();
+    return WCRAS_OK;
+}
+
+// Can the decomposition be two-coloured (multiplicative Schwarz)?  Needs a cut direction and an even number of
+// blocks in every cut direction; returns the pairing direction or -1.
+int ras_cta_sap_pdir(const FusedGeom& fg) {
+    int pdir = -1;
+    for (int mu = 0; mu < 4; mu++) {
+        if (fg.nblk[mu] > 1 && fg.nblk[mu] % 2) return -1;
+        if (fg.nblk[mu] > 1 && pdir < 0) pdir = mu;
+    }
+    return pdir;
+}
+
+// v = K_SAP r: multiplicative Schwarz (SAP; PAPER.md:33 ref [5]), overlap 0, NRAS cycles of
+// (black half step, red half step).  Each half step is one launch over the domains of one colour: rho = r_store -
+// (hops of the other colour's latest v across the boundary, from the halo buffer), N_dominv MR sweeps, phi += v,
+// r_store = rho_fin, halo out for the other colour.  One halo buffer suffices: a launch reads the slots of its own
+// colour and writes those of the other.
+int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v) {
+    const FusedGeom& fg = ctx->fused;
+    const int ncyc = ctx->ras.nras, ndl = ctx->ras.nd / 2, nface = ctx->nface;
+    float4* rf = ctx->ras32[0];
+    float4* hb = ctx->hb;
+    const size_t smem = cta_smem_bytes(fg);
+    const int grid = ndl < ctx->cta_grid ? ndl : ctx->cta_grid;
+    for (int step = 0; step < 2 * ncyc; step++) {
+        const int colour = step & 1;
+        const bool first_visit = step < 2, last_step = step == 2 * ncyc - 1, last_visit = step >= 2 * ncyc - 2;
+        TimedRegion tr(ctx, TC_BLOCK);
+        if (colour == 0) ctx->block_dv += ctx->ras.niter;  // one sweep count per full cycle over all domains
+        const float4* src = first_visit ? r : rf;
+        float4* rho_out = last_visit ? nullptr : rf;          // the residual of this colour is dead after its last visit
+        float4* halo_out = last_step ? nullptr : hb;
+        if (step == 0)
+            ras_cta_kernel<false><<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, nullptr, halo_out, nullptr,
+                                                                        v, rho_out);
+        else
+            ras_cta_kernel<true><<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, hb, halo_out,
+                                                                       first_visit ? nullptr : v, v, rho_out);
         ctx->launches++;
     }
     WC_CHECK_LAUNCH();

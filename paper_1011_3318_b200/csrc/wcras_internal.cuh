@@ -124,6 +124,7 @@ struct FusedGeom {
     int split[4];  // b < L: direction is cut, Omega' extended by s per side, Dirichlet unless ext == L
     int wrap[4];   // ext == L: hops across the domain edge stay inside Omega' (Q7)
     int V, s, ns, nsp, C, niter;
+    int pdir;        // multiplicative Schwarz: pairing direction of the red-black domain enumeration, -1 = not colourable
 };
 
 struct RasConfig {
@@ -154,6 +155,7 @@ struct wcras_ctx {
     // RAS
     RasConfig ras;
     int tier_request = 0;
+    int schwarz = 0;               // 0 additive (RAS, the paper's method), 1 multiplicative (SAP, red-black domains)
     int chain_cycles = 1;          // overlap 0, persistent-CTA tier: NRAS cycles chained through rho_fin (ras_cta.cu)
     FusedGeom fused;               // valid when ras.tier == 2
     float4* dm = nullptr;          // domain-major operand copy of the persistent-CTA tier: [nd][36][nsp]

@@ -189,6 +189,49 @@ def test_ras_apply(which, block, s, nit, nras, tier):
     cs.ctx.set_ras_tier(0)
 
 
+SAP_CASES = [
+    (0, (2, 2, 2, 2), 4, 1), (0, (2, 2, 2, 2), 4, 3), (1, (4, 4, 4, 4), 3, 1), (1, (4, 4, 4, 4), 2, 2),
+    (1, (8, 4, 4, 2), 2, 3), ("ragged", (3, 2, 5, 2), 3, 2),
+]
+
+
+@pytest.mark.parametrize("which,block,nit,ncycle", SAP_CASES)
+def test_sap_apply(which, block, nit, ncycle):
+    """Multiplicative Schwarz (wcras_set_schwarz(1)): red-black half steps on the persistent-CTA
+    kernel against the oracle's SAP, element by element."""
+    cs = ragged_case() if which == "ragged" else case(which)
+    cs.ctx.set_ras_tier(0)
+    cs.ctx.ras_precondition(block, 0, nit, ncycle)
+    cs.ctx.set_schwarz(True)
+    try:
+        r = I.spinor(cs.dims, 56)
+        r32 = r.astype(np.complex64).astype(np.complex128)
+        want = cs.op.sap_apply(block, nit, ncycle, r32)
+        got = cs.ras_apply(r32)
+        assert rel(got, want) <= TOL_RAS
+    finally:
+        cs.ctx.set_schwarz(False)
+
+
+def test_sap_unsupported_and_solve():
+    cs = ragged_case()                                    # 6 x 4 x 10 x 4
+    cs.ctx.set_schwarz(True)
+    try:
+        cs.ctx.ras_precondition((2, 2, 5, 4), 0, 3, 1)    # 3 blocks in x: cannot be two-coloured
+        r = dev(I.spinor(cs.dims, 1), torch.float32)
+        with pytest.raises(binding.WcrasError) as e:
+            cs.ctx.ras_apply(r, torch.empty_like(r))
+        assert e.value.code == binding.UNSUPPORTED
+        cs.ctx.ras_precondition((3, 2, 5, 2), 0, 3, 2)
+        cs.ctx.set_solver(use_ras=True)
+        eta = I.spinor(cs.dims, 4)
+        phi, info = cs.solve(eta, 1e-12)
+        assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+    finally:
+        cs.ctx.set_schwarz(False)
+        cs.ctx.set_solver(use_ras=False)
+
+
 def test_ras_zero_residual_domain():
     """alpha := 0 when <q,q> = 0 in a domain (Q9): input supported on one block leaves the others exactly zero."""
     cs = case(0)
