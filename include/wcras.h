@@ -121,6 +121,17 @@ int wcras_set_timing(wcras_ctx* ctx, int enable);
  * eta_dev / phi_dev: device, canonical fp64, 24*V doubles.  info: host struct, may be NULL. */
 int wcras_solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info);
 
+/* Multi-right-hand-side solve (BASELINE.json:configs[4] "4 Gaussian sources"): solves
+ * D phi_k = eta_k, k < nrhs (1..4), as one block-diagonal system with the same nested BiCGStab on stacked vectors, so
+ * that the links and the clover term are loaded once per nrhs spinors in the fp32 Dslash (336 instead of 768 B per
+ * site and right-hand side at nrhs = 4) and in the persistent block solver.  One set of Krylov scalars serves the
+ * stack: every eta_k is scaled to unit norm, the stack is solved to tol/sqrt(nrhs), and the true residual
+ * |eta_k - D phi_k|/|eta_k| <= tol is checked for every k (written to rel_resid_host[k], host, may be NULL;
+ * info->rel_resid_true is the worst one).  eta_dev / phi_dev: device, canonical fp64, nrhs vectors of 24*V doubles
+ * one after the other.  The workspace grows to nrhs times its size and stays that large. */
+int wcras_solve_multi(wcras_ctx* ctx, int nrhs, const double* eta_dev, double* phi_dev, double tol, wcras_info* info,
+                      double* rel_resid_host);
+
 /* Same, with HOST buffers: copies eta to the device, solves, copies phi back (end-to-end entry point). */
 int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, double tol, wcras_info* info);
 

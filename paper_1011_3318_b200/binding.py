@@ -18,7 +18,7 @@ OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, 
 EXPORTS = [
     "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_ras_precondition", "wcras_set_ras_tier", "wcras_set_schwarz",
     "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_timing", "wcras_solve",
-    "wcras_solve_host", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
+    "wcras_solve_host", "wcras_solve_multi", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
 ]
 
 
@@ -148,6 +148,15 @@ class Context:
         rc = self._lib.wcras_solve(self._h, _ptr(eta_dev), _ptr(phi_dev), C.c_double(tol), C.byref(info))
         self._chk(rc, allow=() if strict else (NOT_CONVERGED, BREAKDOWN))
         return info.asdict()
+
+    def solve_multi(self, nrhs, eta_dev, phi_dev, tol, strict=True):
+        """nrhs stacked systems (wcras_solve_multi); returns (info, per-system true residuals)."""
+        info = WcrasInfo()
+        res = (C.c_double * nrhs)()
+        rc = self._lib.wcras_solve_multi(self._h, C.c_int(nrhs), _ptr(eta_dev), _ptr(phi_dev), C.c_double(tol),
+                                         C.byref(info), res)
+        self._chk(rc, allow=() if strict else (NOT_CONVERGED, BREAKDOWN))
+        return info.asdict(), list(res)
 
     def solve_host(self, eta_host_ptr, phi_host_ptr, tol, strict=True):
         """eta/phi: host buffers (numpy arrays via .ctypes.data, or pinned torch CPU tensors)."""

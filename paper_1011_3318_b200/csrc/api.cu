@@ -150,6 +150,19 @@ int wcras_solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double t
     return solve(ctx, eta_dev, phi_dev, tol, info);
 }
 
+int wcras_solve_multi(wcras_ctx* ctx, int nrhs, const double* eta_dev, double* phi_dev, double tol, wcras_info* info,
+                      double* rel_resid_host) {
+    NEED(ctx, "null ctx");
+    NEED(eta_dev && phi_dev && eta_dev != phi_dev, "solve_multi: null or aliased buffers");
+    NEED(nrhs >= 1 && nrhs <= 4, "solve_multi: nrhs must be 1..4");
+    NEED(tol > 0, "solve_multi: tol must be positive");
+    NEED(!ctx->use_ras || ctx->ras.set, "solve_multi: use_ras is set but wcras_ras_precondition was not called");
+    ctx->nrhs = nrhs;
+    const int rc = solve(ctx, eta_dev, phi_dev, tol, info, rel_resid_host);
+    ctx->nrhs = 1;
+    return rc;
+}
+
 int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, double tol, wcras_info* info) {
     NEED(ctx, "null ctx");
     NEED(eta_host && phi_host, "solve_host: null buffers");

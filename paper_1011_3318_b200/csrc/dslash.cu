@@ -32,20 +32,20 @@ __device__ __forceinline__ void hop_pair(const Fields<T>& f, size_t V, const Geo
 // CTA's output stores and cost ~15 % of the kernel).  dot_finish_kernel, 16 CTAs launched right behind it, sums
 // the partials in a fixed order and finishes the scalar recurrence: deterministic.
 template <int TH>
-__device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __restrict__ part) {
+__device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __restrict__ part, unsigned pstride, unsigned poff) {
     constexpr int NW = TH / 32;
     __shared__ double sm[3][NW];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x, lane = tid & 31, w = tid >> 5;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
         const double t = warp_sum(v[k]);
         if (lane == 0) sm[k][w] = t;
     }
     __syncthreads();
-    if (threadIdx.x < 3) {
+    if (tid < 3) {
         double t = 0;
-        for (int j = 0; j < NW; j++) t += sm[threadIdx.x][j];
-        part[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = t;  // [3][nblk]: coalesced for the finish kernel
+        for (int j = 0; j < NW; j++) t += sm[tid][j];
+        part[(size_t)tid * pstride + poff + blockIdx.x] = t;  // [3][pstride]: coalesced for the finish kernel
     }
 }
 
@@ -105,8 +105,18 @@ template <typename T, bool XPAY, int TH, int MINB, int DOT>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
                                                      typename VecOf<T>::type* __restrict__ out,
                                                      const typename VecOf<T>::type* bsrc,
-                                                     const typename VecOf<T>::type* __restrict__ dotv, double* part) {
+                                                     const typename VecOf<T>::type* __restrict__ dotv, double* part,
+                                                     unsigned pstride, unsigned poff, size_t rstride) {
+    // blockDim = (sites, right-hand sides): the threads threadIdx.y = 0..nrhs-1 of a site work on the vectors of a
+    // stack rstride apart and load the same links and clover term, which L1 serves after the first warp has
+    // fetched them (576/nrhs + 192 bytes of DRAM traffic per site and right-hand side)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    {
+        const size_t ro = threadIdx.y * rstride;
+        in += ro; out += ro;
+        if (XPAY) bsrc += ro;
+        if (DOT) dotv += ro;
+    }
     const bool valid = i < g.V;
     if (!DOT && !valid) return;
     double dsum[3] = {0, 0, 0};
@@ -151,7 +161,7 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
             dsum[0] = d0; dsum[1] = d1; dsum[2] = d2;
         }
     }
-    if (DOT) dslash_block_partial<TH>(dsum, part);
+    if (DOT) dslash_block_partial<TH>(dsum, part, pstride, poff);
 }
 
 struct Box {
@@ -220,41 +230,61 @@ __global__ void __launch_bounds__(128) dslash_box_kernel(Geom g, Fields<T> f, T 
     store_spinor(out, V, i, acc);
 }
 
+// in / out / b_minus / dotv are stacks of ctx->nrhs vectors (one vector when nrhs = 1)
 template <typename T>
 int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>::type* out,
            const typename VecOf<T>::type* b_minus, int dot, const typename VecOf<T>::type* dotv, Scalars* sc) {
+    typedef typename VecOf<T>::type Vec;
     TimedRegion tr(ctx, sizeof(T) == 4 ? TC_DSLASH : TC_DSLASH64);
-    const int V = ctx->geom.V;
+    const int V = ctx->geom.V, nr = ctx->nrhs;
+    const size_t rstride = (size_t)VecOf<T>::CHUNKS * V;
     // 64-thread CTAs with the full register budget (165 registers fp32, 252 fp64): the compiler then keeps all
     // loads of a site in flight at once, which is what an HBM latency-bound stencil needs -- measured on B200 at
     // 32^4: 130 us (fp32) / 292 us (fp64) against 147 / 330 us at 96 / 186 registers with 128-thread CTAs.
-    constexpr int TH = 64;
-    const unsigned grid = (V + TH - 1) / TH;
+    // fp32, nrhs 2..4: one launch covers the whole stack with CTAs of 32 sites x nrhs right-hand sides; otherwise
+    // (nrhs = 1, fp64) one launch of 64-site CTAs per vector of the stack
+    const bool stacked = sizeof(T) == 4 && nr >= 2 && nr <= 4;
+    const unsigned grid = stacked ? (V + 31) / 32 : (V + 63) / 64;
+    const unsigned nblk = stacked ? grid : grid * (unsigned)nr;  // partials of the fused dots
+    double* slice = nullptr;
+    unsigned* fticket = nullptr;
     if (dot) {
-        if (!ctx->dpart) {  // [3][grid] per-CTA partials, then [FIN_CTAS][3] slice sums and one ticket
-            if (alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * (3 * (size_t)grid + 3 * FIN_CTAS + 1))) return WCRAS_CUDA_ERROR;
-            WC_CUDA(cudaMemsetAsync(ctx->dpart + 3 * (size_t)grid + 3 * FIN_CTAS, 0, sizeof(double), ctx->stream));
+        if (!ctx->dpart || ctx->dpart_blocks < nblk) {  // [3][nblk] per-CTA partials, then [FIN_CTAS][3] slice sums and one ticket
+            if (alloc_dev(ctx, (void**)&ctx->dpart, sizeof(double) * (3 * (size_t)nblk + 3 * FIN_CTAS + 1))) return WCRAS_CUDA_ERROR;
+            ctx->dpart_blocks = nblk;
+            WC_CUDA(cudaMemsetAsync(ctx->dpart + 3 * (size_t)nblk + 3 * FIN_CTAS, 0, sizeof(double), ctx->stream));
         }
-        double* slice = ctx->dpart + 3 * (size_t)grid;
-        unsigned* fticket = (unsigned*)(slice + 3 * FIN_CTAS);
-        if (dot == 1) {
-            dslash_kernel<T, false, TH, 1, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                            dotv, ctx->dpart);
-            dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, grid, slice, fticket, sc);
-        } else {
-            dslash_kernel<T, false, TH, 1, 2><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                            dotv, ctx->dpart);
-            dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, grid, slice, fticket, sc);
-        }
-        ctx->launches++;
-    } else if (b_minus) {
-        dslash_kernel<T, true, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, b_minus,
-                                                                       nullptr, nullptr);
-    } else {
-        dslash_kernel<T, false, TH, 1, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, in, out, nullptr,
-                                                                        nullptr, nullptr);
+        slice = ctx->dpart + 3 * (size_t)ctx->dpart_blocks;
+        fticket = (unsigned*)(slice + 3 * FIN_CTAS);
     }
-    ctx->launches++;
+#define WC_DSL(TH, BLOCK, INP, OUTP, BM, DV, POFF)                                                                                    \
+    {                                                                                                                              \
+        if (dot == 1)                                                                                                              \
+            dslash_kernel<T, false, TH, 1, 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                               nullptr, DV, ctx->dpart, nblk, POFF, rstride);      \
+        else if (dot == 2)                                                                                                         \
+            dslash_kernel<T, false, TH, 1, 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                               nullptr, DV, ctx->dpart, nblk, POFF, rstride);      \
+        else if (b_minus)                                                                                                          \
+            dslash_kernel<T, true, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP,  \
+                                                                              BM, nullptr, nullptr, 0, 0, rstride);                \
+        else                                                                                                                       \
+            dslash_kernel<T, false, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                               nullptr, nullptr, nullptr, 0, 0, rstride);          \
+        ctx->launches++;                                                                                                           \
+    }
+    if (stacked) {
+        if (nr == 2) WC_DSL(64, dim3(32, 2), in, out, b_minus, dotv, 0)
+        else if (nr == 3) WC_DSL(96, dim3(32, 3), in, out, b_minus, dotv, 0)
+        else WC_DSL(128, dim3(32, 4), in, out, b_minus, dotv, 0)
+    } else {
+        for (int r = 0; r < nr; r++)
+            WC_DSL(64, dim3(64, 1), in + r * rstride, out + r * rstride, b_minus + r * rstride, dotv + r * rstride, r * grid)
+    }
+#undef WC_DSL
+    if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc);
+    if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc);
+    if (dot) ctx->launches++;
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;
     WC_CHECK_LAUNCH();
     return WCRAS_OK;

@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_add_f(size_t n, float4* __restr
     }
 }
 int add_f(wcras_ctx* ctx, float4* x, const float4* y) {
-    k_add_f<<<RED_BLOCKS, RED_THREADS, 0, ctx->stream>>>((size_t)6 * ctx->geom.V, x, y);
+    k_add_f<<<RED_BLOCKS, RED_THREADS, 0, ctx->stream>>>((size_t)6 * ctx->geom.V * ctx->nrhs, x, y);
     ctx->launches++;
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
@@ -281,9 +281,14 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
 static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     TimedRegion tr(ctx, TC_BLOCK);
     ctx->block_dv += ctx->ras.niter;
-    if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);
-    if (ctx->ras.tier == 2) return ras_fused_block_solve(ctx, r, vout, accum);
-    return generic_block_solve(ctx, r, vout, accum);
+    if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
+    const size_t rstride = (size_t)6 * ctx->geom.V;
+    for (int k = 0; k < ctx->nrhs; k++) {  // cluster and generic tiers: one right-hand side of the stack at a time
+        const int e = ctx->ras.tier == 2 ? ras_fused_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
+                                         : generic_block_solve(ctx, r + k * rstride, vout + k * rstride, accum);
+        if (e) return e;
+    }
+    return WCRAS_OK;
 }
 
 int ras_block_solve(wcras_ctx* ctx, const float4* r, float4* v) { return block_solve(ctx, r, v, false); }

@@ -129,11 +129,13 @@ __global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, 
 //   phi_in  own-site value added to v before the store (phi += v, Alg.1 line 9), or nullptr
 //   phi_out where R_Omega (v [+ phi_in]) is stored
 //   rho_out rho_fin of this cycle, or nullptr (then the last MR residual update is skipped, Q12)
-template <bool CHAIN>
+template <bool CHAIN, bool MULTI>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
 ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __restrict__ dm, const float4* __restrict__ r_src,
                const float4* __restrict__ hb_in, float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out,
-               float4* rho_out) {
+               float4* rho_out, int nrhs, size_t rstride, size_t hstride) {
+    // nrhs > 1 (wcras_solve_multi): every vector argument is a stack of nrhs vectors rstride apart (halo buffers:
+    // hstride); the right-hand sides of a domain are solved one after the other with the operands loaded once
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     float4* hbuf = smem;            // [8][3][nsp]
@@ -202,17 +204,33 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
 #pragma unroll
         WC_LOAD_U(dom0)
     }
-    for (int h = blockIdx.x; h < ndl; h += gridDim.x) {
+    // Work items of this CTA: (domain, right-hand side) pairs, the nr right-hand sides of a domain one after the other
+    // with the operands (links in registers, clover in shared memory) loaded once.  MULTI = false is the
+    // single-right-hand-side instantiation: nr = 1 and the offsets fold away (the kernel sits at the 255-register limit).
+    const int nr = MULTI ? nrhs : 1;
+    for (int j = 0;; j++) {
+        const int h = blockIdx.x + (j / nr) * gridDim.x;
+        if (h >= ndl) break;
+        const int rr = MULTI ? j % nr : 0;
+        const bool last_rhs = rr + 1 == nr;                     // the next item is a new domain (or the end)
+        const bool has_next = last_rhs ? h + (int)gridDim.x < ndl : true;
         const int dom = launch_dom(fg, h, colour);
-        const bool has_next = h + (int)gridDim.x < ndl;
-        const int nxt = launch_dom(fg, has_next ? h + gridDim.x : h, colour);
+        const int nxt = last_rhs ? launch_dom(fg, has_next ? h + gridDim.x : h, colour) : dom;  // domain of the next item
+        const int rrn = last_rhs ? 0 : rr + 1;
         const size_t gi = cta_site(fg, dom, lc);
-        float rho[24], v[24];
         bool u_early = false;  // links of the next domain already requested in the last sweep of this one
+      {
+        const size_t roff = MULTI ? rr * rstride : 0, hoff = MULTI ? rr * hstride : 0;
+#define r_src_r (r_src + roff)
+#define hb_in_r (hb_in + hoff)
+#define hb_out_r (hb_out + hoff)
+#define phi_out_r (phi_out + roff)
+#define rho_out_r (rho_out + roff)
+        float rho[24], v[24];
         if (active) {
 #pragma unroll
             for (int c = 0; c < 6; c++) {
-                const float4 t = r_src[(size_t)c * V + gi];
+                const float4 t = r_src_r[(size_t)c * V + gi];
                 rho[4 * c] = t.x; rho[4 * c + 1] = t.y; rho[4 * c + 2] = t.z; rho[4 * c + 3] = t.w;
             }
         } else {
@@ -223,7 +241,7 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
             // ---- boundary coupling: rho -= D-terms of v_{j-1} that cross the domain boundary.  A lane whose
             // in-domain slot 2mu+1 (2mu) has no receiver sits on the upper (lower) face and receives the
             // outside forward (backward) hop from halo slot 2mu (2mu+1).  All loads are issued first. ----
-            const float4* hin = hb_in + (size_t)dom * 24 * nface;
+            const float4* hin = hb_in_r + (size_t)dom * 24 * nface;
             float hh[8][12];
 #pragma unroll
             for (int sl = 0; sl < 8; sl++) {
@@ -249,12 +267,13 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
         // ---- pull the next domain of this CTA towards L2 while this one is solved ----
         {
             if (has_next) {
-                if (k == 0) prefetch_l2_bulk(dm + (size_t)nxt * 36 * nsp, dm_bytes);
-                if (CHAIN && k == 32) prefetch_l2_bulk(hb_in + (size_t)nxt * 24 * nface, 24u * (unsigned)nface * 16u);
+                const size_t roffn = MULTI ? rrn * rstride : 0, hoffn = MULTI ? rrn * hstride : 0;
+                if (k == 0 && last_rhs) prefetch_l2_bulk(dm + (size_t)nxt * 36 * nsp, dm_bytes);
+                if (CHAIN && k == 32) prefetch_l2_bulk(hb_in + hoffn + (size_t)nxt * 24 * nface, 24u * (unsigned)nface * 16u);
                 if (active) {
                     const size_t gn = cta_site(fg, nxt, lc);
 #pragma unroll
-                    for (int c = 0; c < 6; c++) prefetch_l2(r_src + (size_t)c * V + gn);
+                    for (int c = 0; c < 6; c++) prefetch_l2(r_src + roffn + (size_t)c * V + gn);
                 }
             }
         }
@@ -285,7 +304,7 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
                 }
                 herm6_mul<float>(Ab, rho + 12 * ch, q + 12 * ch);
             }
-            if (it + 1 == fg.niter && has_next) {
+            if (it + 1 == fg.niter && has_next && last_rhs) {
                 const float4* pn = dm + ((size_t)nxt * 36 + 18) * nsp + k;
 #pragma unroll
                 for (int c = 0; c < 18; c++) cp_async16(As + c * nsp + k, pn + (size_t)c * nsp);
@@ -305,7 +324,7 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
             }
             // the links are dead after the last gather unless the halo scatter still needs them: request those of
             // the next domain now, their latency hides behind the dots, the update and the stores
-            if (it + 1 == fg.niter && hb_out == nullptr && has_next) {
+            if (it + 1 == fg.niter && hb_out == nullptr && has_next && last_rhs) {
 #pragma unroll
                 WC_LOAD_U(nxt)
                 u_early = true;
@@ -356,13 +375,13 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
         dd /= nb;                                                                                                \
         if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the domain at -mu */            \
             const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                              \
+            float4* o = hb_out_r + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                            \
             project<float, MU, -1>(v, h);                                                                        \
             for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(h[4 * j], h[4 * j + 1], h[4 * j + 2], h[4 * j + 3]); \
         }                                                                                                        \
         if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the domain at +mu */      \
             const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                          \
+            float4* o = hb_out_r + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                        \
             project<float, MU, +1>(v, h);                                                                        \
             su3_adj_mul<float>(U + 18 * MU, h, g);                                                               \
             for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(g[4 * j], g[4 * j + 1], g[4 * j + 2], g[4 * j + 3]); \
@@ -377,23 +396,29 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
             if (rho_out) {
 #pragma unroll
                 for (int c = 0; c < 6; c++)
-                    __stcs(rho_out + (size_t)c * V + gi, make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]));
+                    __stcs(rho_out_r + (size_t)c * V + gi, make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]));
             }
             if (phi_in) {
                 // phi += v as a fire-and-forget vector reduction (phi_in == phi_out; one writer per site, so the
                 // result is the same single rounding as load-add-store, without waiting for the load)
 #pragma unroll
                 for (int c = 0; c < 6; c++)
-                    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(phi_out + (size_t)c * V + gi), "f"(v[4 * c]),
+                    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(phi_out_r + (size_t)c * V + gi), "f"(v[4 * c]),
                                  "f"(v[4 * c + 1]), "f"(v[4 * c + 2]), "f"(v[4 * c + 3])
                                  : "memory");
             } else {
 #pragma unroll
                 for (int c = 0; c < 6; c++)
-                    phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+                    phi_out_r[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
-        if (!u_early && has_next) {
+      }  // right-hand sides of this domain
+#undef r_src_r
+#undef hb_in_r
+#undef hb_out_r
+#undef phi_out_r
+#undef rho_out_r
+        if (!u_early && has_next && last_rhs) {
 #pragma unroll
             WC_LOAD_U(nxt)
         }
@@ -402,20 +427,28 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
 }
 
 // ---- host side ----
+typedef void (*cta_kernel_t)(FusedGeom, int, int, int, const float4*, const float4*, const float4*, float4*, const float4*, float4*,
+                             float4*, int, size_t, size_t);
+static cta_kernel_t cta_kernel(bool chain, bool multi) {
+    if (chain) return multi ? ras_cta_kernel<true, true> : ras_cta_kernel<true, false>;
+    return multi ? ras_cta_kernel<false, true> : ras_cta_kernel<false, false>;
+}
 static size_t cta_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)42 * fg.nsp + fg.nsp / 32); }
 
 // allocate and fill the domain-major operand copy; sets ctx->dm and the persistent grid size
 int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
     if (fg.C != 1 || fg.nsp > FUSED_CTA_MAX_THREADS) return 0;
     const size_t smem = cta_smem_bytes(fg);
-    if (cudaFuncSetAttribute(ras_cta_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-        cudaFuncSetAttribute(ras_cta_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(ras_cta_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        cudaFuncSetAttribute(ras_cta_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        cudaFuncSetAttribute(ras_cta_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        cudaFuncSetAttribute(ras_cta_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
     int per_sm = 0, per_sm_chain = 0, dev = 0, sms = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta_kernel<false>, fg.nsp, smem) != cudaSuccess || per_sm < 1 ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_chain, ras_cta_kernel<true>, fg.nsp, smem) != cudaSuccess ||
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta_kernel<false, false>, fg.nsp, smem) != cudaSuccess || per_sm < 1 ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_chain, ras_cta_kernel<true, true>, fg.nsp, smem) != cudaSuccess ||
         per_sm_chain < 1) {
         cudaGetLastError();
         return 0;
@@ -426,14 +459,12 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
     if (ctx->dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm); ctx->dm = nullptr; }
     const size_t bytes = sizeof(float4) * 36 * (size_t)fg.nsp * nd;
     if (cudaMalloc((void**)&ctx->dm, bytes) != cudaSuccess) { cudaGetLastError(); ctx->dm = nullptr; return 0; }
-    // halo buffers of the chained cycles (two parities): float4 [2][nd][8][3][nface]
+    // face size of the halo buffers of the chained cycles (allocated on first use, ensure_halo)
     int nface = 1;
     for (int mu = 0; mu < 4; mu++) nface = fg.ns / fg.ext[mu] > nface ? fg.ns / fg.ext[mu] : nface;
     nface = (nface + 7) / 8 * 8;
     if (ctx->hb) { cudaFree(ctx->hb); ctx->hb = nullptr; }
-    if (cudaMalloc((void**)&ctx->hb, sizeof(float4) * 2 * 24 * (size_t)nface * nd) != cudaSuccess) {
-        cudaGetLastError(); ctx->hb = nullptr; cudaFree(ctx->dm); ctx->dm = nullptr; return 0;
-    }
+    ctx->hb_nrhs = 0;
     ctx->nface = nface;
     pack_domain_major_kernel<<<nd, fg.nsp, 0, ctx->stream>>>(fg, nd, ctx->fields<float>(), -(float)ctx->kappa, ctx->dm);
     ctx->launches++;
@@ -443,10 +474,20 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
     return 1;
 }
 
+// halo buffers: float4 [2 parities][nrhs][nd][8][3][nface], grown when a deeper stack of right-hand sides arrives
+static int ensure_halo(wcras_ctx* ctx, int nrhs) {
+    if (ctx->hb && ctx->hb_nrhs >= nrhs) return WCRAS_OK;
+    if (ctx->hb) { WC_CUDA(cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->hb); ctx->hb = nullptr; }
+    WC_CUDA(cudaMalloc((void**)&ctx->hb, sizeof(float4) * 2 * 24 * (size_t)ctx->nface * ctx->ras.nd * nrhs));
+    ctx->hb_nrhs = nrhs;
+    return WCRAS_OK;
+}
+
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
-    ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(
-        fg, ctx->ras.nd, -1, ctx->nface, ctx->dm, r, nullptr, nullptr, accum ? vout : nullptr, vout, nullptr);
+    const size_t rstride = (size_t)6 * fg.V;
+    cta_kernel(false, ctx->nrhs > 1)<<<ctx->cta_grid, fg.nsp, cta_smem_bytes(fg), ctx->stream>>>(
+        fg, ctx->ras.nd, -1, ctx->nface, ctx->dm, r, nullptr, nullptr, accum ? vout : nullptr, vout, nullptr, ctx->nrhs, rstride, 0);
     ctx->launches++;
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
@@ -456,20 +497,23 @@ int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accu
 // rf = rho_fin (updated in place, own sites only); the halo buffer alternates between its two parities.
 int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
     const FusedGeom& fg = ctx->fused;
-    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;
+    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface, nr = ctx->nrhs;
+    if (int rc = ensure_halo(ctx, nr)) return rc;
     float4* rf = ctx->ras32[0];
-    float4* hb[2] = {ctx->hb, ctx->hb + (size_t)24 * nface * nd};
+    const size_t rstride = (size_t)6 * fg.V, hstride = (size_t)24 * nface * nd;
+    float4* hb[2] = {ctx->hb, ctx->hb + hstride * ctx->hb_nrhs};
     const size_t smem = cta_smem_bytes(fg);
     for (int j = 0; j < nras; j++) {
         const bool last = j == nras - 1;
         TimedRegion tr(ctx, TC_BLOCK);
         ctx->block_dv += ctx->ras.niter;
         if (j == 0)
-            ras_cta_kernel<false><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, r, nullptr, last ? nullptr : hb[0],
-                                                                                nullptr, v, last ? nullptr : rf);
+            cta_kernel(false, ctx->nrhs > 1)<<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, r, nullptr, last ? nullptr : hb[0],
+                                                                                nullptr, v, last ? nullptr : rf, nr, rstride, hstride);
         else
-            ras_cta_kernel<true><<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, rf, hb[(j - 1) & 1],
-                                                                               last ? nullptr : hb[j & 1], v, v, last ? nullptr : rf);
+            cta_kernel(true, ctx->nrhs > 1)<<<ctx->cta_grid, fg.nsp, smem, ctx->stream>>>(fg, nd, -1, nface, ctx->dm, rf, hb[(j - 1) & 1],
+                                                                               last ? nullptr : hb[j & 1], v, v, last ? nullptr : rf, nr,
+                                                                               rstride, hstride);
         ctx->launches++;
     }
     WC_CHECK_LAUNCH();
@@ -494,9 +538,11 @@ int ras_cta_sap_pdir(const FusedGeom& fg) {
 // colour and writes those of the other.
 int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v) {
     const FusedGeom& fg = ctx->fused;
-    const int ncyc = ctx->ras.nras, ndl = ctx->ras.nd / 2, nface = ctx->nface;
+    const int ncyc = ctx->ras.nras, ndl = ctx->ras.nd / 2, nface = ctx->nface, nr = ctx->nrhs;
+    if (int rc = ensure_halo(ctx, nr)) return rc;
     float4* rf = ctx->ras32[0];
     float4* hb = ctx->hb;
+    const size_t rstride = (size_t)6 * fg.V, hstride = (size_t)24 * nface * ctx->ras.nd;
     const size_t smem = cta_smem_bytes(fg);
     const int grid = ndl < ctx->cta_grid ? ndl : ctx->cta_grid;
     for (int step = 0; step < 2 * ncyc; step++) {
@@ -508,11 +554,11 @@ int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v) {
         float4* rho_out = last_visit ? nullptr : rf;          // the residual of this colour is dead after its last visit
         float4* halo_out = last_step ? nullptr : hb;
         if (step == 0)
-            ras_cta_kernel<false><<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, nullptr, halo_out, nullptr,
-                                                                        v, rho_out);
+            cta_kernel(false, ctx->nrhs > 1)<<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, nullptr, halo_out, nullptr,
+                                                                        v, rho_out, nr, rstride, hstride);
         else
-            ras_cta_kernel<true><<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, hb, halo_out,
-                                                                       first_visit ? nullptr : v, v, rho_out);
+            cta_kernel(true, ctx->nrhs > 1)<<<grid, fg.nsp, smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->dm, src, hb, halo_out,
+                                                                       first_visit ? nullptr : v, v, rho_out, nr, rstride, hstride);
         ctx->launches++;
     }
     WC_CHECK_LAUNCH();

@@ -193,24 +193,34 @@ __global__ void __launch_bounds__(RED_THREADS) k_norm2_d(size_t n, const double2
 
 // out32 = in64 / sqrt(nrm).  fp32 SoA chunk c4 of site i (float4 [6][V]) holds the complex components 2*c4 and
 // 2*c4+1, which live in fp64 SoA chunks 2*c4 and 2*c4+1 of the same site (double2 [12][V]).
-__global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, const double2* __restrict__ in, float4* __restrict__ out,
-                                                                const Scalars* __restrict__ sc) {
+__global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, int nr, const double2* __restrict__ in,
+                                                                float4* __restrict__ out, const Scalars* __restrict__ sc) {
     const double inv = sc->nrm > 0 ? rsqrt(sc->nrm) : 0.0;
-    GRID_STRIDE(k, 6 * V) {
-        const size_t c4 = k / V, i = k - c4 * V;
-        const double2 a = in[(2 * c4) * V + i], b = in[(2 * c4 + 1) * V + i];
+    GRID_STRIDE(k, 6 * V * nr) {
+        const size_t r = k / (6 * V), kk = k - r * 6 * V, c4 = kk / V, i = kk - c4 * V;
+        const double2* inr = in + r * 12 * V;
+        const double2 a = inr[(2 * c4) * V + i], b = inr[(2 * c4 + 1) * V + i];
         out[k] = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
     }
 }
 // out64 = in32 * sqrt(nrm)
-__global__ void __launch_bounds__(RED_THREADS) k_f2d_scaled(size_t V, const float4* __restrict__ in, double2* __restrict__ out,
-                                                            const Scalars* __restrict__ sc) {
+__global__ void __launch_bounds__(RED_THREADS) k_f2d_scaled(size_t V, int nr, const float4* __restrict__ in,
+                                                            double2* __restrict__ out, const Scalars* __restrict__ sc) {
     const double sc_ = sqrt(sc->nrm);
-    GRID_STRIDE(k, 6 * V) {
-        const size_t c4 = k / V, i = k - c4 * V;
+    GRID_STRIDE(k, 6 * V * nr) {
+        const size_t r = k / (6 * V), kk = k - r * 6 * V, c4 = kk / V, i = kk - c4 * V;
+        double2* outr = out + r * 12 * V;
         const float4 a = in[k];
-        out[(2 * c4) * V + i] = make_double2(a.x * sc_, a.y * sc_);
-        out[(2 * c4 + 1) * V + i] = make_double2(a.z * sc_, a.w * sc_);
+        outr[(2 * c4) * V + i] = make_double2(a.x * sc_, a.y * sc_);
+        outr[(2 * c4 + 1) * V + i] = make_double2(a.z * sc_, a.w * sc_);
+    }
+}
+// a *= f (fp64)
+__global__ void __launch_bounds__(RED_THREADS) k_scale_d(size_t n, double2* __restrict__ a, double f) {
+    GRID_STRIDE(k, n) {
+        double2 v = a[k];
+        v.x *= f; v.y *= f;
+        a[k] = v;
     }
 }
 // x += dx (fp64)
@@ -329,21 +339,36 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
     return status;
 }
 
+static void free_owned(wcras_ctx* ctx, void* p) {
+    if (!p) return;
+    for (size_t k = 0; k < ctx->owned.size(); k++)
+        if (ctx->owned[k] == p) { ctx->owned.erase(ctx->owned.begin() + k); break; }
+    cudaFree(p);
+}
+
+// solver vectors, each a stack of ctx->nrhs lattice vectors; grown when a deeper stack arrives
 int ensure_workspace(wcras_ctx* ctx) {
     const size_t V = ctx->geom.V;
-    if (!ctx->w32[0]) {
-        for (int k = 0; k < 12; k++)
-            if (alloc_dev(ctx, (void**)&ctx->w32[k], sizeof(float4) * 6 * V)) return WCRAS_CUDA_ERROR;
-        for (int k = 0; k < 12; k++)
-            if (alloc_dev(ctx, (void**)&ctx->w64[k], sizeof(double2) * 12 * V)) return WCRAS_CUDA_ERROR;
-        for (int k = 0; k < 3; k++)
-            if (alloc_dev(ctx, (void**)&ctx->ras32[k], sizeof(float4) * 6 * V)) return WCRAS_CUDA_ERROR;
+    if (!ctx->sc32) {
         if (alloc_dev(ctx, (void**)&ctx->sc32, sizeof(Scalars))) return WCRAS_CUDA_ERROR;
         if (alloc_dev(ctx, (void**)&ctx->sc64, sizeof(Scalars))) return WCRAS_CUDA_ERROR;
         if (alloc_dev(ctx, (void**)&ctx->partials, sizeof(double) * RED_BLOCKS * 8)) return WCRAS_CUDA_ERROR;
         if (alloc_dev(ctx, (void**)&ctx->ticket, sizeof(unsigned))) return WCRAS_CUDA_ERROR;
         WC_CUDA(cudaMemsetAsync(ctx->ticket, 0, sizeof(unsigned), ctx->stream));
         WC_CUDA(cudaMallocHost((void**)&ctx->sc_host, sizeof(Scalars)));
+    }
+    if (ctx->ws_nrhs < ctx->nrhs) {
+        WC_CUDA(cudaStreamSynchronize(ctx->stream));
+        for (int k = 0; k < 12; k++) { free_owned(ctx, ctx->w32[k]); free_owned(ctx, ctx->w64[k]); ctx->w32[k] = nullptr; ctx->w64[k] = nullptr; }
+        for (int k = 0; k < 3; k++) { free_owned(ctx, ctx->ras32[k]); ctx->ras32[k] = nullptr; }
+        const size_t nr = ctx->nrhs;
+        for (int k = 0; k < 12; k++)
+            if (alloc_dev(ctx, (void**)&ctx->w32[k], sizeof(float4) * 6 * V * nr)) return WCRAS_CUDA_ERROR;
+        for (int k = 0; k < 12; k++)
+            if (alloc_dev(ctx, (void**)&ctx->w64[k], sizeof(double2) * 12 * V * nr)) return WCRAS_CUDA_ERROR;
+        for (int k = 0; k < 3; k++)
+            if (alloc_dev(ctx, (void**)&ctx->ras32[k], sizeof(float4) * 6 * V * nr)) return WCRAS_CUDA_ERROR;
+        ctx->ws_nrhs = ctx->nrhs;
     }
     return WCRAS_OK;
 }
@@ -352,14 +377,14 @@ static Work<float> work32(wcras_ctx* ctx) {
     Work<float> w;
     w.r = ctx->w32[0]; w.rt = ctx->w32[1]; w.p = ctx->w32[2]; w.v = ctx->w32[3]; w.s = ctx->w32[4];
     w.t = ctx->w32[5]; w.ph = ctx->w32[6]; w.sh = ctx->w32[7];
-    w.sc = ctx->sc32; w.n = (size_t)6 * ctx->geom.V;
+    w.sc = ctx->sc32; w.n = (size_t)6 * ctx->geom.V * ctx->nrhs;
     return w;
 }
 static Work<double> work64(wcras_ctx* ctx) {
     Work<double> w;
     w.r = ctx->w64[0]; w.rt = ctx->w64[1]; w.p = ctx->w64[2]; w.v = ctx->w64[3]; w.s = ctx->w64[4];
     w.t = ctx->w64[5]; w.ph = ctx->w64[6]; w.sh = ctx->w64[7];
-    w.sc = ctx->sc64; w.n = (size_t)12 * ctx->geom.V;
+    w.sc = ctx->sc64; w.n = (size_t)12 * ctx->geom.V * ctx->nrhs;
     return w;
 }
 
@@ -370,8 +395,8 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
     float4* x32 = ctx->w32[9];
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH(k_norm2_d, (size_t)12 * V, in64, ctx->sc64, ctx->partials, ctx->ticket);
-        LAUNCH(k_d2f_normalised, V, in64, b32, ctx->sc64);
+        LAUNCH(k_norm2_d, (size_t)12 * V * ctx->nrhs, in64, ctx->sc64, ctx->partials, ctx->ticket);
+        LAUNCH(k_d2f_normalised, V, ctx->nrhs, in64, b32, ctx->sc64);
     }
     // Tolerance of this inner solve (reading A2): the outer residual after this preconditioner call is
     // about (inner accuracy) x |in|, so the reduction still missing is R = target/|in|.  It is spread evenly over
@@ -403,14 +428,20 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
     // an unconverged or broken-down inner solve is still a usable (flexible) preconditioner
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH(k_f2d_scaled, V, x32, out64, ctx->sc64);
+        LAUNCH(k_f2d_scaled, V, ctx->nrhs, x32, out64, ctx->sc64);
     }
     return WCRAS_OK;
 }
 
-int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info) {
+// ctx->nrhs = 1: one system.  ctx->nrhs = N > 1 (wcras_solve_multi): the N systems D phi_k = eta_k
+// are solved as ONE block-diagonal system diag(D,...,D) by the same nested BiCGStab on stacked vectors -- one set of
+// Krylov scalars for the stack, links and clover loaded once per N spinors in the Dslash and in the block solver.
+// Every eta_k is scaled to unit norm first so that all systems weigh equally, the stack is solved to tol/sqrt(N)
+// (then |r_k| <= |r_stack| <= tol for every k), and the true residual of every system is checked on its own.
+int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info, double* resid_per_rhs) {
     if (int rc = ensure_workspace(ctx)) return rc;
-    const size_t V = ctx->geom.V, n64 = 12 * V;
+    const int nr = ctx->nrhs;
+    const size_t V = ctx->geom.V, n1 = 12 * V, n64 = n1 * nr;
     cudaEvent_t e0, e1;
     WC_CUDA(cudaEventCreate(&e0));
     WC_CUDA(cudaEventCreate(&e1));
@@ -420,10 +451,18 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
     for (int k = 0; k < TC_COUNT; k++) ctx->ms_class[k] = 0;
 
     double2 *eta = ctx->w64[8], *phi = ctx->w64[9], *res = ctx->w64[10], *dx = ctx->w64[11];
-    if (int rc = to_internal(ctx, 64, eta_dev, eta)) return rc;
-    LAUNCH(k_norm2_d, n64, eta, ctx->sc64, ctx->partials, ctx->ticket);
-    if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
-    const double en2 = ctx->sc_host->nrm;
+    double norm_k[8], rel_k[8];
+    double en2 = 0;
+    for (int k = 0; k < nr; k++) {
+        if (int rc = to_internal(ctx, 64, eta_dev + (size_t)k * 24 * V, eta + k * n1)) return rc;
+        LAUNCH(k_norm2_d, n1, eta + k * n1, ctx->sc64, ctx->partials, ctx->ticket);
+        if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
+        norm_k[k] = std::sqrt(ctx->sc_host->nrm);
+        rel_k[k] = norm_k[k] > 0 ? 1.0 : 0.0;
+        if (nr > 1 && norm_k[k] > 0) LAUNCH(k_scale_d, n1, eta + k * n1, 1.0 / norm_k[k]);
+        en2 += nr > 1 ? (norm_k[k] > 0 ? 1.0 : 0.0) : ctx->sc_host->nrm;
+    }
+    const double tol_stack = nr > 1 ? tol / std::sqrt((double)nr) : tol;
     double rn2 = en2, recur = 1.0;
     int outer = 0, inner_iters = 0, inner_solves = 0, status = WCRAS_NOT_CONVERGED;
     if (en2 == 0.0) {  // zero source: phi = 0
@@ -436,7 +475,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         int it = 0;
         double rel = 0;
         // solve D dx = res to relative accuracy tol*|eta|/|res| so that the total residual meets tol
-        const double tol_pass = 0.7 * tol * std::sqrt(en2 / rn2);
+        const double tol_pass = 0.7 * tol_stack * std::sqrt(en2 / rn2);
         ctx->outer_target = tol_pass * std::sqrt(rn2);  // absolute |r| this pass has to reach
         // pass 0: phi = 0 and res = eta, so the solver works on eta and writes phi directly; later passes solve
         // D dx = res for the correction and add it
@@ -450,16 +489,30 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
             LAUNCH(k_add_d, n64, phi, dx);
         }
         if (int r2 = dslash<double>(ctx, phi, res, eta)) return r2;  // res = eta - D phi (true residual, fp64)
-        {
-            TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH(k_norm2_d, n64, res, ctx->sc64, ctx->partials, ctx->ticket);
+        rn2 = 0;
+        double worst = 0;
+        for (int k = 0; k < nr; k++) {  // the true residual of every system on its own
+            {
+                TimedRegion tr(ctx, TC_BLAS);
+                LAUNCH(k_norm2_d, n1, res + k * n1, ctx->sc64, ctx->partials, ctx->ticket);
+            }
+            if (int r3 = read_scalars(ctx, ctx->sc64)) return r3;
+            const double nk = ctx->sc_host->nrm;
+            rn2 += nk;
+            const double ek = nr > 1 ? 1.0 : en2;  // |eta_k|^2 (unit after scaling)
+            rel_k[k] = norm_k[k] > 0 ? std::sqrt(nk / ek) : 0.0;
+            worst = rel_k[k] > worst ? rel_k[k] : worst;
         }
-        if (int r3 = read_scalars(ctx, ctx->sc64)) return r3;
-        rn2 = ctx->sc_host->nrm;
-        if (std::sqrt(rn2 / en2) <= tol) status = WCRAS_OK;
+        if (worst <= tol) status = WCRAS_OK;
         else if (rc == WCRAS_BREAKDOWN) { status = WCRAS_BREAKDOWN; break; }
     }
-    if (int rc = from_internal(ctx, 64, phi, phi_dev)) return rc;
+    double worst = 0;
+    for (int k = 0; k < nr; k++) {
+        if (nr > 1 && norm_k[k] > 0) LAUNCH(k_scale_d, n1, phi + k * n1, norm_k[k]);
+        if (int rc = from_internal(ctx, 64, phi + k * n1, phi_dev + (size_t)k * 24 * V)) return rc;
+        if (resid_per_rhs) resid_per_rhs[k] = rel_k[k];
+        worst = rel_k[k] > worst ? rel_k[k] : worst;
+    }
     WC_CUDA(cudaEventRecord(e1, ctx->stream));
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
     float ms = 0;
@@ -477,7 +530,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         info->outer_iters = outer; info->inner_iters = inner_iters; info->inner_solves = inner_solves;
         info->dv_fp32 = ctx->dv32; info->dv_fp64 = ctx->dv64; info->block_dv = ctx->block_dv;
         info->ras_applies = ctx->ras_applies; info->status = status;
-        info->rel_resid_recur = recur; info->rel_resid_true = en2 > 0 ? std::sqrt(rn2 / en2) : 0.0;
+        info->rel_resid_recur = recur; info->rel_resid_true = worst;
         info->ms_total = ms;
         info->ms_dslash = ctx->ms_class[TC_DSLASH]; info->ms_dslash64 = ctx->ms_class[TC_DSLASH64];
         info->ms_blocksolve = ctx->ms_class[TC_BLOCK]; info->ms_blas = ctx->ms_class[TC_BLAS];

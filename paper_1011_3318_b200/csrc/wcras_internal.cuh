@@ -162,6 +162,7 @@ struct wcras_ctx {
     int cta_grid = 0;              // its persistent grid size
     float4* hb = nullptr;          // halo buffers of the chained K_RAS cycles: [2][nd][8][3][nface]
     int nface = 0;
+    int hb_nrhs = 0;               // stack depth the halo buffers are allocated for
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
     double* mr_scal = nullptr;                                     // [niter][nd][4]
     // solver parameters
@@ -180,7 +181,10 @@ struct wcras_ctx {
     wc::Scalars* sc_host = nullptr;  // pinned
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;
-    double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][grid]
+    double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][blocks], slice sums, ticket
+    unsigned dpart_blocks = 0;
+    int nrhs = 1;                  // right-hand sides stacked in every solver vector (wcras_solve_multi)
+    int ws_nrhs = 0;               // stack depth the workspace is allocated for
     // timing
     int timing = 0;
     std::vector<cudaEvent_t> ev_pool;
@@ -256,6 +260,6 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v);  // v = K_RAS r, inte
 int ras_block_solve(wcras_ctx* ctx, const float4* r, float4* v);
 
 // solver.cu
-int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info);
+int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wcras_info* info, double* resid_per_rhs = nullptr);
 int time_blas(wcras_ctx* ctx, int reps, double* ms);
 }  // namespace wc

@@ -313,6 +313,40 @@ def test_ras_reduces_iterations():
     assert i1["inner_iters"] < i0["inner_iters"]
 
 
+@pytest.mark.parametrize("mode", ["noprec", "ras", "sap", "cluster", "generic"])
+@pytest.mark.parametrize("nrhs", [2, 4])
+def test_solve_multi(mode, nrhs):
+    """wcras_solve_multi: nrhs stacked systems solved as one block-diagonal system; the true
+    residual of every system, recomputed by the oracle, is <= 1e-12 and the solutions agree with single solves."""
+    cs = case(1)
+    ctx = cs.ctx
+    ctx.set_ras_tier(1 if mode == "generic" else 0)
+    if mode == "noprec":
+        ctx.set_solver(use_ras=False)
+    else:
+        dom, it, nras = {"ras": ((4, 4, 4, 4), 2, 3), "sap": ((4, 4, 4, 4), 3, 2), "cluster": ((8, 4, 4, 4), 2, 2),
+                         "generic": ((4, 4, 4, 4), 2, 2)}[mode]
+        ctx.ras_precondition(dom, 0, it, nras)
+        ctx.set_solver(use_ras=True)
+        ctx.set_schwarz(mode == "sap")
+    try:
+        etas = [I.spinor(cs.dims, 2, stream=k) * (10.0 ** k) for k in range(nrhs)]   # very different norms
+        x = dev(np.stack(etas), torch.float64)
+        y = torch.empty_like(x)
+        info, res = ctx.solve_multi(nrhs, x, y, 1e-12)
+        assert info["status"] == 0 and len(res) == nrhs and max(res) <= 1e-12
+        phis = host(y, (nrhs, cs.V, 4, 3))
+        for k in range(nrhs):
+            true = cs.op.true_residual(etas[k], phis[k])
+            assert true <= 1e-12 and abs(true - res[k]) <= 1e-13
+        single, _ = cs.solve(etas[nrhs - 1], 1e-12)
+        assert rel(phis[nrhs - 1], single) < 1e-9
+    finally:
+        ctx.set_schwarz(False)
+        ctx.set_ras_tier(0)
+        ctx.set_solver(use_ras=False)
+
+
 def test_ras_autotune():
     """Parameter survey: the fastest converged row is returned and left configured."""
     cs = case(1)
