@@ -135,6 +135,30 @@ def test_apply_D_special_inputs():
     assert len(np.unique(np.nonzero(np.abs(got) > 0)[0])) == 9
 
 
+def test_extent_two_lattice():
+    """Reading Q19: with L_mu = 2 the forward and the backward neighbour coincide and both hops are added -- D, K_RAS
+    (one domain spanning the lattice in three directions, chained cycles and SAP across the cut one) and the solve."""
+    dims = (2, 2, 4, 2)
+    cs = Case(dims, 0.12, 1.0, I.gauge_exp(dims, 0.5, 21))
+    psi = I.spinor(dims, 22)
+    assert rel(cs.apply_D(32, psi), cs.op.apply_D(psi)) <= TOL32
+    assert rel(cs.apply_D(64, psi), cs.op.apply_D(psi)) <= TOL64
+    r32 = psi.astype(np.complex64).astype(np.complex128)
+    for tier in (0, 1, 4):
+        cs.ctx.set_ras_tier(tier)
+        for block, nras in (((2, 2, 2, 2), 2), ((2, 2, 4, 2), 1), ((2, 2, 1, 2), 3)):
+            cs.ctx.ras_precondition(block, 0, 3, nras)
+            assert rel(cs.ras_apply(r32), cs.op.ras_apply(block, 0, 3, nras, r32)) <= TOL_RAS
+    cs.ctx.set_ras_tier(0)
+    cs.ctx.ras_precondition((2, 2, 2, 2), 0, 3, 2)
+    cs.ctx.set_schwarz(True)
+    assert rel(cs.ras_apply(r32), cs.op.sap_apply((2, 2, 2, 2), 3, 2, r32)) <= TOL_RAS
+    cs.ctx.set_schwarz(False)
+    cs.ctx.set_solver(use_ras=True)
+    phi, info = cs.solve(psi, 1e-12)
+    assert info["status"] == 0 and cs.op.true_residual(psi, phi) <= 1e-12
+
+
 @pytest.mark.parametrize("prec", [32, 64])
 @pytest.mark.parametrize("s", [0, 1])
 def test_apply_D_restricted(prec, s):
@@ -161,6 +185,9 @@ RAS_CASES = [
     (0, (2, 2, 2, 2), 0, 4, 1), (0, (2, 2, 2, 2), 0, 4, 3), (0, (2, 2, 2, 2), 1, 3, 2), (0, (4, 4, 4, 4), 0, 6, 1),
     (1, (4, 4, 4, 4), 0, 4, 1), (1, (4, 4, 4, 4), 1, 4, 1), (1, (4, 4, 4, 4), 0, 5, 3), (1, (8, 4, 4, 4), 1, 2, 2),
     ("ragged", (2, 2, 5, 4), 1, 3, 2), ("ragged", (3, 4, 5, 2), 0, 1, 1),
+    # BASELINE.json:configs[2] shapes: 4^4 with overlap 2 (8^4 = 4096-site extended domains: 16-CTA cluster) and
+    # 8x4x4x4 with overlap 2 (12x8x8x8 = 6144 sites: fits no on-chip tier, generic tier), overlap 1 (cluster)
+    (2, (4, 4, 4, 4), 2, 2, 1), (2, (8, 4, 4, 4), 2, 2, 1), (2, (8, 4, 4, 4), 1, 3, 2),
     # chained cycles (overlap 0, NRAS > 1): plain, with a wrap-around direction (block = L in x), ragged
     (1, (4, 4, 4, 4), 0, 2, 2), (1, (8, 4, 4, 2), 0, 3, 3), ("ragged", (3, 4, 5, 2), 0, 2, 3),
 ]
