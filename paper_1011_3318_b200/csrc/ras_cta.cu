@@ -254,13 +254,16 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
                     hh[sl][4 * j] = t.x; hh[sl][4 * j + 1] = t.y; hh[sl][4 * j + 2] = t.z; hh[sl][4 * j + 3] = t.w;
                 }
             }
+            // a warp none of whose lanes sits on the face in question skips that hop (z and t faces are warp-uniform
+            // for x-fastest local indices)
             float g[12];
-#define WC_CROSS(MU)                                                   \
-    su3_mul<float>(U + 18 * MU, hh[2 * MU], g);                        \
-    for (int n = 0; n < 12; n++) g[n] = -g[n];                         \
-    reconstruct_add<float, MU, -1>(g, rho);                            \
-    for (int n = 0; n < 12; n++) g[n] = -hh[2 * MU + 1][n];            \
-    reconstruct_add<float, MU, +1>(g, rho);
+#define WC_CROSS(MU)                                                                              \
+    if (__any_sync(0xffffffffu, active && dst[2 * MU + 1] == 0xffffffffu)) {                      \
+        su3_mul<float>(U + 18 * MU, hh[2 * MU], g);                                               \
+        reconstruct_sub<float, MU, -1>(g, rho);                                                   \
+    }                                                                                             \
+    if (__any_sync(0xffffffffu, active && dst[2 * MU] == 0xffffffffu))                            \
+        reconstruct_sub<float, MU, +1>(hh[2 * MU + 1], rho);
             WC_CROSS(0) WC_CROSS(1) WC_CROSS(2) WC_CROSS(3)
 #undef WC_CROSS
         }

@@ -52,32 +52,39 @@ WC_HD void project(const T* __restrict__ s, T* __restrict__ h) {
     }
 }
 
-// acc += full spinor whose upper rows are g and whose rows 2,3 follow from (1 + SIGN*gamma_MU)
-template <typename T, int MU, int SIGN>
-WC_HD void reconstruct_add(const T* __restrict__ g, T* __restrict__ acc) {
+// acc += sg * (full spinor whose upper rows are g and whose rows 2,3 follow from (1 + SIGN*gamma_MU)), sg = +1 or,
+// with NEG, -1 (a compile-time sign: it folds into the operand negation of the adds)
+template <typename T, int MU, int SIGN, int NEG>
+WC_HD void reconstruct_acc(const T* __restrict__ g, T* __restrict__ acc) {
+    const T sg = NEG ? T(-1) : T(1);
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const T g0r = g[2 * c], g0i = g[2 * c + 1];
         const T g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
-        acc[2 * c] += g0r; acc[2 * c + 1] += g0i;
-        acc[6 + 2 * c] += g1r; acc[6 + 2 * c + 1] += g1i;
+        acc[2 * c] += sg * g0r; acc[2 * c + 1] += sg * g0i;
+        acc[6 + 2 * c] += sg * g1r; acc[6 + 2 * c + 1] += sg * g1i;
         T* a2 = acc + 12 + 2 * c;
         T* a3 = acc + 18 + 2 * c;
         if (MU == 0) {
-            if (SIGN < 0) { a2[0] += g1i; a2[1] -= g1r; a3[0] += g0i; a3[1] -= g0r; }   // r2 = -i g1, r3 = -i g0
-            else          { a2[0] -= g1i; a2[1] += g1r; a3[0] -= g0i; a3[1] += g0r; }   // r2 =  i g1, r3 =  i g0
+            if (SIGN < 0) { a2[0] += sg * g1i; a2[1] -= sg * g1r; a3[0] += sg * g0i; a3[1] -= sg * g0r; }   // r2 = -i g1, r3 = -i g0
+            else          { a2[0] -= sg * g1i; a2[1] += sg * g1r; a3[0] -= sg * g0i; a3[1] += sg * g0r; }   // r2 =  i g1, r3 =  i g0
         } else if (MU == 1) {
-            if (SIGN < 0) { a2[0] -= g1r; a2[1] -= g1i; a3[0] += g0r; a3[1] += g0i; }   // r2 = -g1, r3 = g0
-            else          { a2[0] += g1r; a2[1] += g1i; a3[0] -= g0r; a3[1] -= g0i; }   // r2 = g1, r3 = -g0
+            if (SIGN < 0) { a2[0] -= sg * g1r; a2[1] -= sg * g1i; a3[0] += sg * g0r; a3[1] += sg * g0i; }   // r2 = -g1, r3 = g0
+            else          { a2[0] += sg * g1r; a2[1] += sg * g1i; a3[0] -= sg * g0r; a3[1] -= sg * g0i; }   // r2 = g1, r3 = -g0
         } else if (MU == 2) {
-            if (SIGN < 0) { a2[0] += g0i; a2[1] -= g0r; a3[0] -= g1i; a3[1] += g1r; }   // r2 = -i g0, r3 = i g1
-            else          { a2[0] -= g0i; a2[1] += g0r; a3[0] += g1i; a3[1] -= g1r; }   // r2 = i g0, r3 = -i g1
+            if (SIGN < 0) { a2[0] += sg * g0i; a2[1] -= sg * g0r; a3[0] -= sg * g1i; a3[1] += sg * g1r; }   // r2 = -i g0, r3 = i g1
+            else          { a2[0] -= sg * g0i; a2[1] += sg * g0r; a3[0] += sg * g1i; a3[1] -= sg * g1r; }   // r2 = i g0, r3 = -i g1
         } else {
-            if (SIGN < 0) { a2[0] -= g0r; a2[1] -= g0i; a3[0] -= g1r; a3[1] -= g1i; }   // r2 = -g0, r3 = -g1
-            else          { a2[0] += g0r; a2[1] += g0i; a3[0] += g1r; a3[1] += g1i; }
+            if (SIGN < 0) { a2[0] -= sg * g0r; a2[1] -= sg * g0i; a3[0] -= sg * g1r; a3[1] -= sg * g1i; }   // r2 = -g0, r3 = -g1
+            else          { a2[0] += sg * g0r; a2[1] += sg * g0i; a3[0] += sg * g1r; a3[1] += sg * g1i; }
         }
     }
 }
+
+template <typename T, int MU, int SIGN>
+WC_HD void reconstruct_add(const T* __restrict__ g, T* __restrict__ acc) { reconstruct_acc<T, MU, SIGN, 0>(g, acc); }
+template <typename T, int MU, int SIGN>
+WC_HD void reconstruct_sub(const T* __restrict__ g, T* __restrict__ acc) { reconstruct_acc<T, MU, SIGN, 1>(g, acc); }
 
 // Explicit fused multiply-add chains: written out because the compiler may not re-associate
 // "re += ur*hr - ui*hi" into two FMAs on the accumulator (it emits FMUL + FFMA + FADD instead).
