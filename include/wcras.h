@@ -88,6 +88,12 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
  * Call before wcras_ras_precondition. */
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
 
+/* Order in which the full-lattice Dslash visits the sites (a traversal order only; no layout changes, results are
+ * identical): ztile = -1 automatic (default: plain order x,y,z,t; above ~60 MB of operands per t-slice the order
+ * x, y, z within a tile, t, z tile, with the largest tile whose slab stays under 30 MB, so that the t-neighbours are
+ * still in L2), 0 plain order, z > 0 that tile size (a proper divisor of Lz). */
+int wcras_set_traversal(wcras_ctx* ctx, int ztile);
+
 /* Schwarz variant applied by wcras_ras_apply and the solver: 0 = additive with restriction (RAS, Alg. 1 -- the paper's
  * method and the default), 1 = multiplicative (SAP, the related method PAPER.md:33 names, ref. [5]; SURVEY.md 8(f)
  * NEXT-4): the domains are coloured red/black by the parity of their block coordinates and `nras` cycles of (black

@@ -85,6 +85,14 @@ int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     return WCRAS_OK;
 }
 
+int wcras_set_traversal(wcras_ctx* ctx, int ztile) {
+    NEED(ctx, "null ctx");
+    NEED(ztile >= -1 && ztile < ctx->geom.L[2] && (ztile <= 0 || ctx->geom.L[2] % ztile == 0),
+         "set_traversal: ztile must be -1 (automatic), 0 (off) or a proper divisor of Lz");
+    ctx->ztile_request = ztile;
+    return WCRAS_OK;
+}
+
 int wcras_set_schwarz(wcras_ctx* ctx, int multiplicative) {
     NEED(ctx, "null ctx");
     NEED(multiplicative == 0 || multiplicative == 1, "set_schwarz: 0 (additive, RAS) or 1 (multiplicative, SAP)");

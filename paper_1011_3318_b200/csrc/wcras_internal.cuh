@@ -155,6 +155,7 @@ struct wcras_ctx {
     // RAS
     RasConfig ras;
     int tier_request = 0;
+    int ztile_request = -1;        // z-tile size of the Dslash traversal: -1 automatic, 0 off (wcras_set_traversal)
     int schwarz = 0;               // 0 additive (RAS, the paper's method), 1 multiplicative (SAP, red-black domains)
     int chain_cycles = 1;          // overlap 0, persistent-CTA tier: NRAS cycles chained through rho_fin (ras_cta.cu)
     FusedGeom fused;               // valid when ras.tier == 2

@@ -135,6 +135,32 @@ def test_apply_D_special_inputs():
     assert len(np.unique(np.nonzero(np.abs(got) > 0)[0])) == 9
 
 
+@pytest.mark.parametrize("ztile", [1, 2, 5])
+def test_dslash_z_tiled_traversal(ztile):
+    """wcras_set_traversal: the z-tiled visiting order used on large lattices gives the same D v (fp32, fp64, the
+    r - D v and fused-dot variants through a solve, and the stacked multi-right-hand-side launch)."""
+    cs = ragged_case()                                    # 6 x 4 x 10 x 4: Lz = 10
+    psi = I.spinor(cs.dims, 31)
+    want = cs.op.apply_D(psi)
+    cs.ctx.set_traversal(ztile)
+    try:
+        assert rel(cs.apply_D(32, psi), want) <= TOL32
+        assert rel(cs.apply_D(64, psi), want) <= TOL64
+        cs.ctx.set_solver(use_ras=False)
+        phi, info = cs.solve(psi, 1e-12)
+        assert info["status"] == 0 and cs.op.true_residual(psi, phi) <= 1e-12
+        etas = [I.spinor(cs.dims, 32, stream=k) for k in range(3)]
+        x = dev(np.stack(etas), torch.float64)
+        y = torch.empty_like(x)
+        info, res = cs.ctx.solve_multi(3, x, y, 1e-12)
+        phis = host(y, (3, cs.V, 4, 3))
+        assert info["status"] == 0 and all(cs.op.true_residual(etas[k], phis[k]) <= 1e-12 for k in range(3))
+        with pytest.raises(binding.WcrasError):
+            cs.ctx.set_traversal(3)                       # 3 does not divide 10
+    finally:
+        cs.ctx.set_traversal(-1)
+
+
 def test_extent_two_lattice():
     """Reading Q19: with L_mu = 2 the forward and the backward neighbour coincide and both hops are added -- D, K_RAS
     (one domain spanning the lattice in three directions, chained cycles and SAP across the cut one) and the solve."""
