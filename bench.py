@@ -38,8 +38,8 @@ RAS_NAMED = [dict(domain=(8, 8, 4, 4), overlap=0, block_iters=3, nras=2),
 SAP = dict(domain=(4, 4, 4, 4), block_iters=3, ncycle=2)
 INNER_TOL = 5e-7
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
-# `ncu --set full` capture (profiles/r1b_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
-DSLASH_TRAFFIC_NCU_BYTES = 826.4e6
+# `ncu --set full` capture (profiles/r1j_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
+DSLASH_TRAFFIC_NCU_BYTES = 810.3e6
 
 
 def peaks():
@@ -312,7 +312,7 @@ def main():
             "frac": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9 / hbm_peak,
             "ms_per_launch_burst": ms_blk, "frac_burst": 864.0 * V / (ms_blk * 1e-3) / 1e9 / hbm_peak,
             "note": "HBM floor = operands 576 + r 96 + v 96 + phi/rho 96 B per site; the kernel is bound by fp32 issue "
-                    "latency at 2 warps per scheduler, see profiles/r1b_kernels.md"},
+                    "latency at 2 warps per scheduler, see profiles/r1j_kernels.md"},
         "cpu_baseline": cpu,
         "solve": {"ras": {k: info[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv",
                                               "ras_applies", "rel_resid_true", "ms_total", "ms_dslash", "ms_dslash64",
