@@ -457,6 +457,31 @@ def test_full_size_32_ras_apply():
     cs.ctx.set_ras_tier(0)
 
 
+def test_full_size_32_sap_and_multi():
+    """Full size, the configurations bench.py reports beside the timed step: K_SAP (4^4, N_dominv 3, 2 cycles) against
+    the oracle on every site, and the stacked 2-right-hand-side RAS solve with the oracle's residual per system."""
+    cs = case(3)
+    r32 = I.spinor(cs.dims, 78).astype(np.complex64).astype(np.complex128)
+    cs.ctx.set_ras_tier(0)
+    cs.ctx.ras_precondition((4, 4, 4, 4), 0, 3, 2)
+    cs.ctx.set_schwarz(True)
+    try:
+        assert rel(cs.ras_apply(r32), cs.op.sap_apply((4, 4, 4, 4), 3, 2, r32)) <= TOL_RAS
+    finally:
+        cs.ctx.set_schwarz(False)
+    cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+    cs.ctx.set_solver(use_ras=True)
+    etas = [I.spinor(cs.dims, 4, stream=k) for k in range(2)]
+    x = dev(np.stack(etas), torch.float64)
+    y = torch.empty_like(x)
+    info, res = cs.ctx.solve_multi(2, x, y, 1e-12)
+    phis = host(y, (2, cs.V, 4, 3))
+    assert info["status"] == 0
+    for k in range(2):
+        assert cs.op.true_residual(etas[k], phis[k]) <= 1e-12
+    cs.ctx.set_solver(use_ras=False)
+
+
 def test_full_size_32_solve():
     cs = case(3)
     cfg = I.CONFIGS[3]
