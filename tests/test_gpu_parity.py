@@ -400,6 +400,30 @@ def test_solve_multi(mode, nrhs):
         ctx.set_solver(use_ras=False)
 
 
+def test_hard_regime_smooth_field():
+    """A smooth, near-critical field (links exp(i 0.2 H), kappa = 0.13: an order of magnitude more iterations than the
+    BASELINE configs, the regime of the paper's Table 1): every variant still meets the true-residual target, and the
+    paper's best point (NRAS 3, N_dominv 5) cuts the number of fp32 D applications of the Krylov solver."""
+    dims = (8, 8, 8, 8)
+    cs = Case(dims, 0.13, 1.0, I.gauge_exp(dims, 0.2, 17))
+    eta = I.spinor(dims, 18)
+    cs.ctx.set_solver(use_ras=False)
+    phi, i0 = cs.solve(eta, 1e-12)
+    assert i0["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+    cs.ctx.ras_precondition((4, 4, 4, 4), 0, 5, 3)
+    cs.ctx.set_solver(use_ras=True)
+    phi, i1 = cs.solve(eta, 1e-12)
+    assert i1["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+    cs.ctx.set_schwarz(True)
+    phi, i2 = cs.solve(eta, 1e-12)
+    cs.ctx.set_schwarz(False)
+    assert i2["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+    print("\ninner iterations: no preconditioner %d, RAS(5,3) %d, SAP(5,3) %d" % (i0["inner_iters"], i1["inner_iters"], i2["inner_iters"]))
+    assert i0["inner_iters"] > 60                       # the system really is harder than the BASELINE configs
+    assert i1["inner_iters"] < i0["inner_iters"] / 2 and i2["inner_iters"] <= i1["inner_iters"]
+    cs.ctx.set_solver(use_ras=False)
+
+
 def test_ras_autotune():
     """Parameter survey: the fastest converged row is returned and left configured."""
     cs = case(1)
