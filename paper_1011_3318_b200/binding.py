@@ -139,7 +139,7 @@ class Context:
     def ras_apply(self, r_dev, v_dev):
         self._chk(self._lib.wcras_ras_apply(self._h, _ptr(r_dev), _ptr(v_dev)))
 
-    def set_solver(self, inner_tol=1e-5, inner_maxit=1000, outer_maxit=50, use_ras=True):
+    def set_solver(self, inner_tol=5e-7, inner_maxit=1000, outer_maxit=50, use_ras=True):
         self._chk(self._lib.wcras_set_solver(self._h, C.c_double(inner_tol), C.c_int(inner_maxit),
                                              C.c_int(outer_maxit), C.c_int(1 if use_ras else 0)))
 
