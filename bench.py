@@ -299,6 +299,10 @@ def main():
         ch.set_solver(inner_tol=INNER_TOL, use_ras=True)
         ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)     # the paper's best point: NRAS 3, N_dominv 5
         hrun("ras_4x4x4x4_it5_nras3")
+        for dom in ((8, 8, 4, 4), (8, 8, 8, 8)):        # the domain shapes configs[3] names (cluster tier)
+            ch.ras_precondition(dom, 0, 5, 3)
+            hrun("ras_%s_it5_nras3" % "x".join(map(str, dom)))
+        ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)
         ch.set_schwarz(True)
         hrun("sap_4x4x4x4_it5_ncycle3")
         del ch, eh, ph
