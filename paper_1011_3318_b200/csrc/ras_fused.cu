@@ -7,7 +7,7 @@
 //   * The extended domain Omega' (extents ext[mu]) is cut into c[0] x c[1] x c[2] x c[3] sub-blocks of shape
 //     sb[mu] = ext[mu]/c[mu] with at most 256 sites each; one CTA per sub-block, one thread per site, and the
 //     C = prod c[mu] <= 16 CTAs of a domain form one thread-block cluster (C = 1: a plain CTA).
-//   * Per thread, for the whole solve, IN REGISTERS: its 4 forward links U_mu(x) (72 reals), its clover
+//   * Per thread, for the whole solve, IN REGISTERS (clover: shared memory): its 4 forward links U_mu(x) (72 reals), its clover
 //     blocks A(x) (72 reals), the MR residual rho(x) and the iterate v(x) (24 reals each).  Links and clover
 //     are read from HBM exactly once per block solve.
 //   * Only projected half spinors (12 reals) travel between sites, through shared memory: in every MR
@@ -18,7 +18,8 @@
 //   * The domain-local dots <q,rho>, <q,q> go warp shuffle -> one float4 per warp pushed to every CTA of the
 //     cluster -> summed in a fixed order by every warp after the barrier (deterministic, no atomics).
 //   * Two barriers per MR iteration (barrier.cluster arrive/wait when C > 1, bar.sync when C = 1).
-// Shared memory per CTA: 8 x 3 float4 x 256 = 96 KB of half-spinor slots + 2 KB of dot partials.
+// Shared memory per CTA: 8 x 3 float4 x 256 = 96 KB of half-spinor slots + 72 KB of clover blocks (own column per
+// thread, read back one chiral block at a time) + 2 KB of dot partials.
 // Roofline: HBM floor = (96 + 576) B per extended site in + 96 B per bulk site out; the N_dominv sweeps are bound
 // by fp32 issue (~1.3 k instructions per site-sweep) and shared-memory traffic (768 B per site-sweep).
 #include "wcras_internal.cuh"
@@ -79,7 +80,8 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;                 // threads per CTA = slots per chunk
     float4* hbuf = smem;                    // [8][3][nsp]
-    float4* red = smem + 24 * nsp;          // [C * nwarps]
+    float4* As = smem + 24 * nsp;           // [18][nsp] clover blocks, each thread its own column (as in ras_cta.cu)
+    float4* red = smem + 42 * nsp;          // [C * nwarps]
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const unsigned rank = CL ? cluster_rank() : 0u;
     const int dom = CL ? blockIdx.x / fg.C : blockIdx.x;
@@ -154,15 +156,18 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
     // ---- zero the slots (Dirichlet faces are never written), load the site data ----
 #pragma unroll
     for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    float U[72], A[72], rho[24], v[24];
+    float U[72], rho[24], v[24];
     if (active) {
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) load_link(f, (size_t)fg.V, gi, mu, U + 18 * mu);
-        load_clover(f, (size_t)fg.V, gi, A);
+#pragma unroll
+        for (int c = 0; c < 18; c++) As[c * nsp + k] = f.cl[(size_t)c * fg.V + gi];
         load_spinor(r, (size_t)fg.V, gi, rho);  // projection P_Omega' r
     } else {
 #pragma unroll
-        for (int n = 0; n < 72; n++) { U[n] = 0.f; A[n] = 0.f; }
+        for (int n = 0; n < 72; n++) U[n] = 0.f;
+#pragma unroll
+        for (int c = 0; c < 18; c++) As[c * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
         for (int n = 0; n < 24; n++) rho[n] = 0.f;
     }
@@ -186,7 +191,17 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
         }
         barrier_arrive<CL>();
         float q[24];
-        clover_apply<float>(A, rho, q);  // independent of the exchange: overlaps the barrier
+        // q = A rho from the shared-memory copy, one chiral block at a time; independent of the exchange: overlaps the barrier
+#pragma unroll
+        for (int ch = 0; ch < 2; ch++) {
+            float Ab[36];
+#pragma unroll
+            for (int c = 0; c < 9; c++) {
+                const float4 t = As[(9 * ch + c) * nsp + k];
+                Ab[4 * c] = t.x; Ab[4 * c + 1] = t.y; Ab[4 * c + 2] = t.z; Ab[4 * c + 3] = t.w;
+            }
+            herm6_mul<float>(Ab, rho + 12 * ch, q + 12 * ch);
+        }
         barrier_wait<CL>();
         // ---- gather: q = A rho - kappa * hop ----
         {
@@ -308,7 +323,7 @@ static FusedGeom make_fused_geom(const wcras_ctx* ctx, const int b[4], const int
     return fg;
 }
 
-static size_t fused_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)24 * fg.nsp + (size_t)fg.C * (fg.nsp / 32)); }
+static size_t fused_smem_bytes(const FusedGeom& fg) { return sizeof(float4) * ((size_t)42 * fg.nsp + (size_t)fg.C * (fg.nsp / 32)); }
 
 template <bool CL>
 static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
