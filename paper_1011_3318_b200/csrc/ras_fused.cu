@@ -17,6 +17,8 @@
 //     never written and its slot stays zero = Dirichlet boundary.  Wrap-around inside Omega' (ext = L) is kept.
 //   * The domain-local dots <q,rho>, <q,q> go warp shuffle -> one float4 per warp pushed to every CTA of the
 //     cluster -> summed in a fixed order by every warp after the barrier (deterministic, no atomics).
+//   * PERSISTENT: the grid holds as many clusters as fit on the chip (cudaOccupancyMaxActiveClusters); a cluster walks
+//     over its domains and prefetches the operands and the residual of the next one into L2 while it solves one.
 //   * Two barriers per MR iteration (barrier.cluster arrive/wait when C > 1, bar.sync when C = 1).
 // Shared memory per CTA: 8 x 3 float4 x 256 = 96 KB of half-spinor slots + 72 KB of clover blocks (own column per
 // thread, read back one chiral block at a time) + 2 KB of dot partials.
@@ -76,7 +78,7 @@ __device__ __forceinline__ void ld_half(const float4* __restrict__ slot, int nsp
 
 template <bool CL>
 __global__ void __launch_bounds__(FUSED_MAX_THREADS, 1)
-ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum) {
+ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum) {
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;                 // threads per CTA = slots per chunk
     float4* hbuf = smem;                    // [8][3][nsp]
@@ -84,7 +86,9 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
     float4* red = smem + 42 * nsp;          // [C * nwarps]
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const unsigned rank = CL ? cluster_rank() : 0u;
-    const int dom = CL ? blockIdx.x / fg.C : blockIdx.x;
+    // PERSISTENT: a cluster (or CTA) walks over the domains dom0, dom0 + nclus, ...; while it solves one, the operands
+    // and the residual of its next one are pulled from HBM into L2 (prefetch.global.L2)
+    const int dom0 = CL ? blockIdx.x / fg.C : blockIdx.x, nclus = CL ? gridDim.x / fg.C : gridDim.x;
     const bool active = k < fg.ns;
 
     // ---- geometry of this thread's site ----
@@ -98,10 +102,12 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
             ec[mu] = sc[mu] * fg.sb[mu] + lc[mu];
         }
     }
-    size_t gi;       // global site index
     bool bulk = active;
-    {
-        int d = dom, x[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++)
+        if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
+    auto site_of = [&](int d) -> size_t {  // global site index of this thread's site in domain d
+        int x[4];
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
             const int bc = d % fg.nblk[mu];
@@ -110,10 +116,9 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
             if (st < 0) st += fg.L[mu];
             if (st >= fg.L[mu]) st -= fg.L[mu];
             x[mu] = st;
-            if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
         }
-        gi = x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3]));
-    }
+        return x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3]));
+    };
     // destination slot of the half spinor sent in direction (mu, -) [index 2mu: receiver x-mu uses it for its
     // forward hop] and (mu, +) [index 2mu+1: receiver x+mu, backward hop]
     const unsigned chunk_bytes = (unsigned)nsp * 16u;
@@ -156,6 +161,10 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
     // ---- zero the slots (Dirichlet faces are never written), load the site data ----
 #pragma unroll
     for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    barrier_arrive<CL>();
+    barrier_wait<CL>();  // every CTA of the cluster has zeroed its slots before anybody scatters into them
+    for (int dom = dom0; dom < nd; dom += nclus) {
+    const size_t gi = site_of(dom);
     float U[72], rho[24], v[24];
     if (active) {
 #pragma unroll
@@ -173,8 +182,17 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
     }
 #pragma unroll
     for (int n = 0; n < 24; n++) v[n] = 0.f;
-    barrier_arrive<CL>();
-    barrier_wait<CL>();
+    if (dom + nclus < nd && active) {  // next domain of this cluster towards L2
+        const size_t gn = site_of(dom + nclus), V = fg.V;
+#pragma unroll
+        for (int c = 0; c < 16; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.ga + (size_t)c * V + gn));
+#pragma unroll
+        for (int c = 0; c < 4; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.gb + (size_t)c * V + gn));
+#pragma unroll
+        for (int c = 0; c < 18; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.cl + (size_t)c * V + gn));
+#pragma unroll
+        for (int c = 0; c < 6; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(r + (size_t)c * V + gn));
+    }
 
     for (int it = 0; it < fg.niter; it++) {
         // ---- scatter: projected half spinors to the 8 neighbours ----
@@ -280,6 +298,7 @@ ras_fused_kernel(FusedGeom fg, Fields<float> f, float kappa, const float4* __res
         }
         store_spinor(vout, (size_t)fg.V, gi, v);
     }
+    }  // domains of this cluster
 }
 
 // ---- host side ----
@@ -331,7 +350,15 @@ static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
     const size_t smem = fused_smem_bytes(fg);
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    if (!CL) { *max_clusters = 1; return cudaSuccess; }
+    if (!CL) {  // plain CTAs: resident CTAs per SM x SMs
+        int per_sm = 0, dev = 0, sms = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, fg.nsp, smem);
+        if (e != cudaSuccess) return e;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        *max_clusters = per_sm * sms;
+        return cudaSuccess;
+    }
     e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, fg.C > 8 ? 1 : 0);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
@@ -347,10 +374,10 @@ static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
 }
 
 template <bool CL>
-static cudaError_t launch_fused(const FusedGeom& fg, int nd, cudaStream_t stream, const Fields<float>& f, float kappa,
+static cudaError_t launch_fused(const FusedGeom& fg, int nd, int nclus, cudaStream_t stream, const Fields<float>& f, float kappa,
                                 const float4* r, float4* vout, int accum) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)nd * fg.C);
+    cfg.gridDim = dim3((unsigned)nclus * fg.C);
     cfg.blockDim = dim3((unsigned)fg.nsp);
     cfg.dynamicSmemBytes = fused_smem_bytes(fg);
     cfg.stream = stream;
@@ -359,7 +386,7 @@ static cudaError_t launch_fused(const FusedGeom& fg, int nd, cudaStream_t stream
     at[0].val.clusterDim.x = (unsigned)fg.C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = CL ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, f, kappa, r, vout, accum);
+    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, nd, f, kappa, r, vout, accum);
 }
 
 // Fill *out and return 1 if the extended domain fits the fused tier on this device: a cut into <= 16 sub-blocks of
@@ -372,15 +399,17 @@ int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], in
     const cudaError_t e = fg.C > 1 ? prepare_fused<true>(fg, &nclusters) : prepare_fused<false>(fg, &nclusters);
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     if (nclusters < 1) return 0;
-    *out = fg;
+    FusedGeom fgo = fg;
+    fgo.nclus = nclusters;
+    *out = fgo;
     return 1;
 }
 
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
     const Fields<float> f = ctx->fields<float>();
-    if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
-    else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
+    if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
+    else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
     ctx->launches++;
     return WCRAS_OK;
 }

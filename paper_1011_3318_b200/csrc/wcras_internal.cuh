@@ -124,6 +124,7 @@ struct FusedGeom {
     int split[4];  // b < L: direction is cut, Omega' extended by s per side, Dirichlet unless ext == L
     int wrap[4];   // ext == L: hops across the domain edge stay inside Omega' (Q7)
     int V, s, ns, nsp, C, niter;
+    int nclus;       // tier 2b: clusters (or CTAs) resident at once = persistent grid size in clusters
     int pdir;        // multiplicative Schwarz: pairing direction of the red-black domain enumeration, -1 = not colourable
 };
 
