@@ -205,6 +205,7 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_cta_sap_pdir(const FusedGeom& fg);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
@@ -247,6 +248,13 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         fgeom.pdir = ras_cta_sap_pdir(fgeom);
         ctx->fused = fgeom;
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
+        if (!rc.cta) {  // halo geometry of the chained cycles on the cluster tier (buffers allocated on first use)
+            int nface = 1;
+            for (int mu = 0; mu < 4; mu++) nface = rc.nloc / rc.ext[mu] > nface ? rc.nloc / rc.ext[mu] : nface;
+            if (ctx->hb) { WC_CUDA(cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->hb); ctx->hb = nullptr; }
+            ctx->hb_nrhs = 0;
+            ctx->nface = (nface + 7) / 8 * 8;
+        }
     }
     ctx->ras = rc;
     return WCRAS_OK;
@@ -309,6 +317,7 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
+    if (rc.tier == 2 && !rc.cta && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];
     const float4* rcur = r;

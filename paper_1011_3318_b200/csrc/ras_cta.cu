@@ -478,7 +478,7 @@ int ras_cta_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
 }
 
 // halo buffers: float4 [2 parities][nrhs][nd][8][3][nface], grown when a deeper stack of right-hand sides arrives
-static int ensure_halo(wcras_ctx* ctx, int nrhs) {
+int ensure_halo(wcras_ctx* ctx, int nrhs) {
     if (ctx->hb && ctx->hb_nrhs >= nrhs) return WCRAS_OK;
     if (ctx->hb) { WC_CUDA(cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->hb); ctx->hb = nullptr; }
     WC_CUDA(cudaMalloc((void**)&ctx->hb, sizeof(float4) * 2 * 24 * (size_t)ctx->nface * ctx->ras.nd * nrhs));

@@ -78,7 +78,11 @@ __device__ __forceinline__ void ld_half(const float4* __restrict__ slot, int nsp
 
 template <bool CL>
 __global__ void __launch_bounds__(FUSED_MAX_THREADS, 1)
-ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum) {
+ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum,
+                 int nface, const float4* __restrict__ hb_in, float4* __restrict__ hb_out, float4* rho_out) {
+    // Chained cycles (overlap 0; same scheme as ras_cta.cu, reading A3): hb_in != nullptr: r is rho_fin of the
+    // previous cycle and the hops of the previous v that cross the domain boundary are subtracted from it (halo slots
+    // filled by the neighbouring domains); hb_out: halo scatter of this cycle's v; rho_out: rho_fin of this cycle.
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;                 // threads per CTA = slots per chunk
     float4* hbuf = smem;                    // [8][3][nsp]
@@ -106,6 +110,18 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
 #pragma unroll
     for (int mu = 0; mu < 4; mu++)
         if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
+    int fidx[4];  // index of the site within the mu-face of Omega' (coordinate mu removed), unique over the cluster
+    {
+        int E = 0, es = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) { E += ec[mu] * es; es *= fg.ext[mu]; }
+        es = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            fidx[mu] = (E % es) + (E / (es * fg.ext[mu])) * es;
+            es *= fg.ext[mu];
+        }
+    }
     auto site_of = [&](int d) -> size_t {  // global site index of this thread's site in domain d
         int x[4];
 #pragma unroll
@@ -179,6 +195,35 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
         for (int c = 0; c < 18; c++) As[c * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
         for (int n = 0; n < 24; n++) rho[n] = 0.f;
+    }
+    if (hb_in) {
+        // boundary coupling: rho += kappa [ recon^-(U h_2mu) + recon^+(h_2mu+1) ] over the halo slots of this domain; a
+        // lane whose in-domain slot 2mu+1 (2mu) has no receiver sits on the upper (lower) face and receives slot 2mu (2mu+1)
+        const float4* hin = hb_in + (size_t)dom * 24 * nface;
+        float g[12], hh[12];
+#define WC_CROSS(MU)                                                                                   \
+    {                                                                                                  \
+        const bool up = active && dst[2 * MU + 1] == NO_DST, lo = active && dst[2 * MU] == NO_DST;     \
+        if (__any_sync(0xffffffffu, up)) {                                                             \
+            for (int j = 0; j < 3; j++) {                                                              \
+                float4 t = make_float4(0.f, 0.f, 0.f, 0.f);                                            \
+                if (up) t = hin[((size_t)(2 * MU) * 3 + j) * nface + fidx[MU]];                        \
+                hh[4 * j] = kappa * t.x; hh[4 * j + 1] = kappa * t.y; hh[4 * j + 2] = kappa * t.z; hh[4 * j + 3] = kappa * t.w; \
+            }                                                                                          \
+            su3_mul<float>(U + 18 * MU, hh, g);                                                        \
+            reconstruct_add<float, MU, -1>(g, rho);                                                    \
+        }                                                                                              \
+        if (__any_sync(0xffffffffu, lo)) {                                                             \
+            for (int j = 0; j < 3; j++) {                                                              \
+                float4 t = make_float4(0.f, 0.f, 0.f, 0.f);                                            \
+                if (lo) t = hin[((size_t)(2 * MU + 1) * 3 + j) * nface + fidx[MU]];                    \
+                hh[4 * j] = kappa * t.x; hh[4 * j + 1] = kappa * t.y; hh[4 * j + 2] = kappa * t.z; hh[4 * j + 3] = kappa * t.w; \
+            }                                                                                          \
+            reconstruct_add<float, MU, +1>(hh, rho);                                                   \
+        }                                                                                              \
+    }
+        WC_CROSS(0) WC_CROSS(1) WC_CROSS(2) WC_CROSS(3)
+#undef WC_CROSS
     }
 #pragma unroll
     for (int n = 0; n < 24; n++) v[n] = 0.f;
@@ -276,7 +321,7 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
         }
         // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9); v += alpha rho; rho -= alpha q
         const float ar = s2 > 0.f ? s0 / s2 : 0.f, ai = s2 > 0.f ? s1 / s2 : 0.f;
-        const bool last = it + 1 == fg.niter;
+        const bool last = it + 1 == fg.niter && rho_out == nullptr;  // rho_fin is needed by the next chained cycle
 #pragma unroll
         for (int n = 0; n < 12; n++) {
             const float rr = rho[2 * n], ri = rho[2 * n + 1];
@@ -288,8 +333,35 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
             }
         }
     }
+    if (hb_out) {
+        // halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors
+        int dd = dom, dstride = 1;
+        float h[12], g[12];
+#define WC_HALO(MU)                                                                                              \
+    {                                                                                                            \
+        const int nb = fg.nblk[MU], bc = dd % nb;                                                                \
+        dd /= nb;                                                                                                \
+        if (active && dst[2 * MU] == NO_DST) { /* lower face -> slot 2mu of the domain at -mu */                 \
+            const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                              \
+            project<float, MU, -1>(v, h);                                                                        \
+            for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(h[4 * j], h[4 * j + 1], h[4 * j + 2], h[4 * j + 3]); \
+        }                                                                                                        \
+        if (active && dst[2 * MU + 1] == NO_DST) { /* upper face -> slot 2mu+1 of the domain at +mu */           \
+            const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                          \
+            project<float, MU, +1>(v, h);                                                                        \
+            su3_adj_mul<float>(U + 18 * MU, h, g);                                                               \
+            for (int j = 0; j < 3; j++) o[(size_t)j * nface] = make_float4(g[4 * j], g[4 * j + 1], g[4 * j + 2], g[4 * j + 3]); \
+        }                                                                                                        \
+        dstride *= nb;                                                                                           \
+    }
+        WC_HALO(0) WC_HALO(1) WC_HALO(2) WC_HALO(3)
+#undef WC_HALO
+    }
     // ---- restriction R_Omega: bulk sites only; disjoint over domains, so a plain store (or phi += v) ----
     if (bulk) {
+        if (rho_out) store_spinor(rho_out, (size_t)fg.V, gi, rho);
         if (accum) {
             float o[24];
             load_spinor(vout, (size_t)fg.V, gi, o);
@@ -375,7 +447,8 @@ static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
 
 template <bool CL>
 static cudaError_t launch_fused(const FusedGeom& fg, int nd, int nclus, cudaStream_t stream, const Fields<float>& f, float kappa,
-                                const float4* r, float4* vout, int accum) {
+                                const float4* r, float4* vout, int accum, int nface = 0, const float4* hb_in = nullptr,
+                                float4* hb_out = nullptr, float4* rho_out = nullptr) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)nclus * fg.C);
     cfg.blockDim = dim3((unsigned)fg.nsp);
@@ -386,7 +459,7 @@ static cudaError_t launch_fused(const FusedGeom& fg, int nd, int nclus, cudaStre
     at[0].val.clusterDim.x = (unsigned)fg.C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = CL ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, nd, f, kappa, r, vout, accum);
+    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, nd, f, kappa, r, vout, accum, nface, hb_in, hb_out, rho_out);
 }
 
 // Fill *out and return 1 if the extended domain fits the fused tier on this device: a cut into <= 16 sub-blocks of
@@ -403,6 +476,33 @@ int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], in
     fgo.nclus = nclusters;
     *out = fgo;
     return 1;
+}
+
+int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu
+
+// v = K_RAS r with NRAS chained cycles on the cluster tier (overlap 0, one right-hand side): as ras_cta_apply_chained
+int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
+    const FusedGeom& fg = ctx->fused;
+    const Fields<float> f = ctx->fields<float>();
+    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;
+    const int nclus = nd < fg.nclus ? nd : fg.nclus;
+    if (int rc = ensure_halo(ctx, 1)) return rc;
+    float4* rf = ctx->ras32[0];
+    const size_t hstride = (size_t)24 * nface * nd;
+    float4* hb[2] = {ctx->hb, ctx->hb + hstride * ctx->hb_nrhs};
+    for (int j = 0; j < nras; j++) {
+        const bool last = j == nras - 1;
+        TimedRegion tr(ctx, TC_BLOCK);
+        ctx->block_dv += ctx->ras.niter;
+        const float4* src = j == 0 ? r : rf;
+        const float4* hin = j == 0 ? nullptr : hb[(j - 1) & 1];
+        float4* hout = last ? nullptr : hb[j & 1];
+        float4* rout = last ? nullptr : rf;
+        if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout));
+        else WC_CUDA(launch_fused<false>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout));
+        ctx->launches++;
+    }
+    return WCRAS_OK;
 }
 
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {

@@ -214,6 +214,8 @@ RAS_CASES = [
     # BASELINE.json:configs[2] shapes: 4^4 with overlap 2 (8^4 = 4096-site extended domains: 16-CTA cluster) and
     # 8x4x4x4 with overlap 2 (12x8x8x8 = 6144 sites: fits no on-chip tier, generic tier), overlap 1 (cluster)
     (2, (4, 4, 4, 4), 2, 2, 1), (2, (8, 4, 4, 4), 2, 2, 1), (2, (8, 4, 4, 4), 1, 3, 2),
+    # the domain shapes of configs[3] on the cluster tier, overlap 0, NRAS > 1: chained cycles across clusters
+    (2, (8, 8, 4, 4), 0, 2, 3), (2, (8, 8, 8, 8), 0, 2, 2), (2, (8, 4, 4, 4), 0, 3, 2),
     # chained cycles (overlap 0, NRAS > 1): plain, with a wrap-around direction (block = L in x), ragged
     (1, (4, 4, 4, 4), 0, 2, 2), (1, (8, 4, 4, 2), 0, 3, 3), ("ragged", (3, 4, 5, 2), 0, 2, 3),
 ]
