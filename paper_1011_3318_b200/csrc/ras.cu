@@ -206,6 +206,7 @@ int ras_cta_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accu
 int ras_cta_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
+void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_sap_pdir(const FusedGeom& fg);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
@@ -248,6 +249,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         fgeom.pdir = ras_cta_sap_pdir(fgeom);
         ctx->fused = fgeom;
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
+        if (!rc.cta) ras_fused_pack(ctx, ctx->fused, rc.nd);
         if (!rc.cta) {  // halo geometry of the chained cycles on the cluster tier (buffers allocated on first use)
             int nface = 1;
             for (int mu = 0; mu < 4; mu++) nface = rc.nloc / rc.ext[mu] > nface ? rc.nloc / rc.ext[mu] : nface;

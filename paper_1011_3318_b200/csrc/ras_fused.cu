@@ -79,7 +79,10 @@ __device__ __forceinline__ void ld_half(const float4* __restrict__ slot, int nsp
 template <bool CL>
 __global__ void __launch_bounds__(FUSED_MAX_THREADS, 1)
 ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum,
-                 int nface, const float4* __restrict__ hb_in, float4* __restrict__ hb_out, float4* rho_out) {
+                 int nface, const float4* __restrict__ hb_in, float4* __restrict__ hb_out, float4* rho_out,
+                 const float4* __restrict__ dmc) {
+    // dmc (overlap 0 only): domain-major operand copy float4 [nd][C][36][nsp] -- the 72 link reals, then the 72 clover
+    // reals of the sites of one CTA contiguous (147 KB), as in ras_cta.cu but with the links unscaled
     // Chained cycles (overlap 0; same scheme as ras_cta.cu, reading A3): hb_in != nullptr: r is rho_fin of the
     // previous cycle and the hops of the previous v that cross the domain boundary are subtracted from it (halo slots
     // filled by the neighbouring domains); hb_out: halo scatter of this cycle's v; rho_out: rho_fin of this cycle.
@@ -182,7 +185,22 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
     for (int dom = dom0; dom < nd; dom += nclus) {
     const size_t gi = site_of(dom);
     float U[72], rho[24], v[24];
-    if (active) {
+    if (dmc) {
+        const float4* p = dmc + ((size_t)dom * fg.C + rank) * 36 * nsp + k;  // zero-filled for the inactive lanes
+#pragma unroll
+        for (int c = 0; c < 18; c++) {
+            const float4 t = __ldcs(p + (size_t)c * nsp);
+            U[4 * c] = t.x; U[4 * c + 1] = t.y; U[4 * c + 2] = t.z; U[4 * c + 3] = t.w;
+        }
+#pragma unroll
+        for (int c = 0; c < 18; c++) As[c * nsp + k] = __ldcs(p + (size_t)(18 + c) * nsp);
+        if (active) {
+            load_spinor(r, (size_t)fg.V, gi, rho);
+        } else {
+#pragma unroll
+            for (int n = 0; n < 24; n++) rho[n] = 0.f;
+        }
+    } else if (active) {
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) load_link(f, (size_t)fg.V, gi, mu, U + 18 * mu);
 #pragma unroll
@@ -227,14 +245,19 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
     }
 #pragma unroll
     for (int n = 0; n < 24; n++) v[n] = 0.f;
+    if (dom + nclus < nd && dmc && k == 0)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(dmc + ((size_t)(dom + nclus) * fg.C + rank) * 36 * nsp),
+                     "r"(36u * (unsigned)nsp * 16u) : "memory");
     if (dom + nclus < nd && active) {  // next domain of this cluster towards L2
         const size_t gn = site_of(dom + nclus), V = fg.V;
+        if (!dmc) {
 #pragma unroll
-        for (int c = 0; c < 16; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.ga + (size_t)c * V + gn));
+            for (int c = 0; c < 16; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.ga + (size_t)c * V + gn));
 #pragma unroll
-        for (int c = 0; c < 4; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.gb + (size_t)c * V + gn));
+            for (int c = 0; c < 4; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.gb + (size_t)c * V + gn));
 #pragma unroll
-        for (int c = 0; c < 18; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.cl + (size_t)c * V + gn));
+            for (int c = 0; c < 18; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(f.cl + (size_t)c * V + gn));
+        }
 #pragma unroll
         for (int c = 0; c < 6; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(r + (size_t)c * V + gn));
     }
@@ -373,6 +396,31 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
     }  // domains of this cluster
 }
 
+// pack the domain-major operand copy of the cluster tier: one CTA per (domain, cluster rank), one thread per site
+__global__ void pack_cluster_dm_kernel(FusedGeom fg, Fields<float> f, float4* __restrict__ dmc) {
+    const int dom = blockIdx.x / fg.C, rank = blockIdx.x % fg.C, k = threadIdx.x;
+    float4* out = dmc + (size_t)blockIdx.x * 36 * fg.nsp + k;
+    if (k >= fg.ns) {
+        for (int c = 0; c < 36; c++) out[(size_t)c * fg.nsp] = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    int kk = k, rr = rank, d = dom, x[4];
+    for (int mu = 0; mu < 4; mu++) {
+        const int lc = kk % fg.sb[mu]; kk /= fg.sb[mu];
+        const int sc = rr % fg.c[mu]; rr /= fg.c[mu];
+        const int bc = d % fg.nblk[mu]; d /= fg.nblk[mu];
+        int st = bc * fg.b[mu] - (fg.split[mu] ? fg.s : 0) + sc * fg.sb[mu] + lc;
+        if (st < 0) st += fg.L[mu];
+        if (st >= fg.L[mu]) st -= fg.L[mu];
+        x[mu] = st;
+    }
+    const size_t gi = x[0] + fg.L[0] * (x[1] + fg.L[1] * (x[2] + (size_t)fg.L[2] * x[3])), V = fg.V;
+    float u[72];
+    for (int mu = 0; mu < 4; mu++) load_link(f, V, gi, mu, u + 18 * mu);
+    for (int c = 0; c < 18; c++) out[(size_t)c * fg.nsp] = make_float4(u[4 * c], u[4 * c + 1], u[4 * c + 2], u[4 * c + 3]);
+    for (int c = 0; c < 18; c++) out[(size_t)(18 + c) * fg.nsp] = f.cl[(size_t)c * V + gi];
+}
+
 // ---- host side ----
 // Choose the cut of Omega' into sub-blocks: minimal cluster size, then the most cubic sub-block.
 static bool choose_cut(const int ext[4], int c[4], int sb[4]) {
@@ -448,7 +496,7 @@ static cudaError_t prepare_fused(const FusedGeom& fg, int* max_clusters) {
 template <bool CL>
 static cudaError_t launch_fused(const FusedGeom& fg, int nd, int nclus, cudaStream_t stream, const Fields<float>& f, float kappa,
                                 const float4* r, float4* vout, int accum, int nface = 0, const float4* hb_in = nullptr,
-                                float4* hb_out = nullptr, float4* rho_out = nullptr) {
+                                float4* hb_out = nullptr, float4* rho_out = nullptr, const float4* dmc = nullptr) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)nclus * fg.C);
     cfg.blockDim = dim3((unsigned)fg.nsp);
@@ -459,7 +507,7 @@ static cudaError_t launch_fused(const FusedGeom& fg, int nd, int nclus, cudaStre
     at[0].val.clusterDim.x = (unsigned)fg.C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at;
     cfg.numAttrs = CL ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, nd, f, kappa, r, vout, accum, nface, hb_in, hb_out, rho_out);
+    return cudaLaunchKernelEx(&cfg, ras_fused_kernel<CL>, fg, nd, f, kappa, r, vout, accum, nface, hb_in, hb_out, rho_out, dmc);
 }
 
 // Fill *out and return 1 if the extended domain fits the fused tier on this device: a cut into <= 16 sub-blocks of
@@ -480,6 +528,18 @@ int ras_fused_prepare(const wcras_ctx* ctx, const int b[4], const int ext[4], in
 
 int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu
 
+// overlap 0: build the domain-major operand copy of the cluster tier in ctx->dm (shared slot with tier 2a); on failure
+// (memory) the kernel falls back to the SoA fields
+void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
+    if (ctx->dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm); ctx->dm = nullptr; }
+    if (fg.s != 0) return;
+    const size_t bytes = sizeof(float4) * 36 * (size_t)fg.nsp * fg.C * nd;
+    if (cudaMalloc((void**)&ctx->dm, bytes) != cudaSuccess) { cudaGetLastError(); ctx->dm = nullptr; return; }
+    pack_cluster_dm_kernel<<<nd * fg.C, fg.nsp, 0, ctx->stream>>>(fg, ctx->fields<float>(), ctx->dm);
+    ctx->launches++;
+    if (cudaGetLastError() != cudaSuccess) { cudaFree(ctx->dm); ctx->dm = nullptr; }
+}
+
 // v = K_RAS r with NRAS chained cycles on the cluster tier (overlap 0, one right-hand side): as ras_cta_apply_chained
 int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
     const FusedGeom& fg = ctx->fused;
@@ -498,8 +558,8 @@ int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
         const float4* hin = j == 0 ? nullptr : hb[(j - 1) & 1];
         float4* hout = last ? nullptr : hb[j & 1];
         float4* rout = last ? nullptr : rf;
-        if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout));
-        else WC_CUDA(launch_fused<false>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout));
+        if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout, ctx->dm));
+        else WC_CUDA(launch_fused<false>(fg, nd, nclus, ctx->stream, f, (float)ctx->kappa, src, v, j > 0, nface, hin, hout, rout, ctx->dm));
         ctx->launches++;
     }
     return WCRAS_OK;
@@ -508,8 +568,9 @@ int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
     const Fields<float> f = ctx->fields<float>();
-    if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
-    else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0));
+    const int nclus = ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus;
+    if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0, 0, nullptr, nullptr, nullptr, ctx->dm));
+    else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0, 0, nullptr, nullptr, nullptr, ctx->dm));
     ctx->launches++;
     return WCRAS_OK;
 }
