@@ -154,7 +154,7 @@ typedef struct {
 /* The paper's parameter survey ("we survey the best parameters for NRAS and N_dominv ... we find the
  * best parameter", and :83-85 on the trade-off), run on this lattice and GPU: solves D phi = eta to `tol` once
  * untimed and once timed for every candidate (overlap 0; block shapes of <= 256 sites with extents 2/4/8 that
- * divide the lattice, plus 8x4x4x4 and 8x8x4x4; (N_dominv, NRAS) in {(2,2),(2,3),(2,4),(3,2),(3,3),(4,1),(4,2)};
+ * divide the lattice, plus 8x4x4x4 and 8x8x4x4; (N_dominv, NRAS) in {(2,2),(2,3),(2,4),(3,2),(3,3),(4,1),(4,2),(4,3),(5,3)} -- (5,3) is the paper's best point;
  * and the unpreconditioned solver), at most max_rows candidates.  The fastest converged candidate is left
  * configured (wcras_ras_precondition + use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.
  * table_host (may be NULL) receives the rows tried, *nrows their number.  eta_dev: device, canonical fp64.

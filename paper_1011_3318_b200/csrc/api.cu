@@ -200,7 +200,7 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
         rows.push_back(r);
     };
     add(0, 0, 0, 0, 0, 0);  // no preconditioner
-    static const int par[7][2] = {{2, 3}, {2, 2}, {2, 4}, {3, 2}, {3, 3}, {4, 1}, {4, 2}};
+    static const int par[9][2] = {{2, 3}, {2, 2}, {2, 4}, {3, 2}, {3, 3}, {4, 1}, {4, 2}, {4, 3}, {5, 3}};
     std::vector<std::vector<int>> shapes;
     for (int b3 : {8, 4, 2}) for (int b2 : {8, 4, 2}) for (int b1 : {8, 4, 2}) for (int b0 : {8, 4, 2}) {
         const int b[4] = {b0, b1, b2, b3};
@@ -213,7 +213,7 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
         const bool named = (b0 == 8 && b1 == 4 && b2 == 4 && b3 == 4) || (b0 == 8 && b1 == 8 && b2 == 4 && b3 == 4);
         if (ok && ((sorted && ns <= 256 && ns >= 64) || named)) shapes.push_back({b0, b1, b2, b3});
     }
-    for (int p = 0; p < 7; p++)
+    for (int p = 0; p < 9; p++)
         for (const auto& sh : shapes) add(sh[0], sh[1], sh[2], sh[3], par[p][0], par[p][1]);
     if ((int)rows.size() > max_rows) rows.resize(max_rows);
     double* phi = (double*)ctx->io_b;
