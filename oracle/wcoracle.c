@@ -27,6 +27,15 @@
  * coefficient, taken literally from north_star) -- the implementation of the
  * literal formula is pinned by the closed-form clover matrix test.
  *
+ * Reduced-precision operand storage (DESIGN.md reading
+ * R1): the same algorithms applied to an operator whose links and site-diagonal
+ * matrices A(x) were rounded entry by entry (fp64 -> fp32 -> fp16, round to
+ * nearest even).  wco_clover_matrix writes A(x) out as a dense 12x12 matrix,
+ * wco_round_half rounds, wco_set_explicit_clover makes every routine below use
+ * the given A(x) instead of forming it from F.  Pins: the explicit path with
+ * unrounded A reproduces the formula path; A(x) against the test's Kronecker
+ * construction; the rounding against numpy's IEEE binary16 and closed-form ties.
+ *
  * Layouts (row-major C arrays of double complex):
  *   site index i = x + Lx*(y + Ly*(z + Lz*t)); mu = 0..3 = x,y,z,t
  *   U   [V][4][3][3]   (U psi)_a = sum_b U[a][b] psi_b
@@ -203,13 +212,29 @@ void wco_field_strength(const int L[4], const cplx* U, cplx* F) {
 /* NULL when that hop is dropped (Dirichlet boundary of a restricted   */
 /* operator).  link_bwd[mu] = U_mu(x-mu).                 */
 /* ------------------------------------------------------------------ */
-static void site_D(const cplx* link_fwd[4], const cplx* link_bwd[4], const cplx* Fx, double kappa,
+/* Explicit site-diagonal matrices A(x), [V][12][12] with row/column index spin*3+colour, or NULL.
+ * When set (reduced-precision operand variant, reading R1) A(x) psi(x) is the plain
+ * matrix-vector product with the stored matrix and F, c_sw are not used. */
+static const cplx* g_Aexp = NULL;
+void wco_set_explicit_clover(const cplx* A) { g_Aexp = A; }
+#define AEXP(site) (g_Aexp ? g_Aexp + (site) * 144 : NULL)
+
+static void site_D(const cplx* link_fwd[4], const cplx* link_bwd[4], const cplx* Fx, const cplx* Ax, double kappa,
                    double csw, const cplx* psi_x, const cplx* psi_fwd[4], const cplx* psi_bwd[4],
                    cplx out[12]) {
     /* site-diagonal clover term A(x) psi(x) */
-    for (int al = 0; al < 4; al++)
-        for (int a = 0; a < 3; a++) out[3 * al + a] = psi_x[3 * al + a];
     double c = clover_coeff(kappa, csw);
+    if (Ax) {
+        for (int i = 0; i < 12; i++) {
+            cplx s = 0;
+            for (int j = 0; j < 12; j++) s += Ax[12 * i + j] * psi_x[j];
+            out[i] = s;
+        }
+        c = 0.0;
+    } else {
+        for (int al = 0; al < 4; al++)
+            for (int a = 0; a < 3; a++) out[3 * al + a] = psi_x[3 * al + a];
+    }
     if (c != 0.0) {
         for (int p = 0; p < 6; p++) {
             cplx sig[16], fpsi[12];
@@ -291,7 +316,7 @@ void wco_apply_D(const int L[4], const cplx* U, const cplx* F, double kappa, dou
             pb[mu] = in + j * 12;
             lb[mu] = LINK(U, j, mu);
         }
-        site_D(lf, lb, F + i * 54, kappa, csw, in + i * 12, pf, pb, out + i * 12);
+        site_D(lf, lb, F + i * 54, AEXP(i), kappa, csw, in + i * 12, pf, pb, out + i * 12);
     }
 }
 
@@ -321,7 +346,7 @@ void wco_apply_D_box(const int L[4], const cplx* U, const cplx* F, double kappa,
             pb[mu] = box_local_index(L, start, ext, y) >= 0 ? in + j * 12 : NULL;
             lb[mu] = LINK(U, j, mu);
         }
-        site_D(lf, lb, F + i * 54, kappa, csw, in + i * 12, pf, pb, out + i * 12);
+        site_D(lf, lb, F + i * 54, AEXP(i), kappa, csw, in + i * 12, pf, pb, out + i * 12);
     }
 }
 
@@ -420,7 +445,7 @@ static void box_apply_D_local(const int L[4], const cplx* U, const cplx* F, doub
             pb[mu] = kk >= 0 ? in + kk * 12 : NULL;
             lb[mu] = LINK(U, site_index(L, y), mu);
         }
-        site_D(lf, lb, F + i * 54, kappa, csw, in + k * 12, pf, pb, out + k * 12);
+        site_D(lf, lb, F + i * 54, AEXP(i), kappa, csw, in + k * 12, pf, pb, out + k * 12);
     }
 }
 
@@ -791,8 +816,58 @@ void wco_apply_D_sites(const int L[4], const cplx* U, const cplx* F, double kapp
             pb[mu] = in + j * 12;
             lb[mu] = LINK(U, j, mu);
         }
-        site_D(lf, lb, F + i * 54, kappa, csw, in + i * 12, pf, pb, out + n * 12);
+        site_D(lf, lb, F + i * 54, AEXP(i), kappa, csw, in + i * 12, pf, pb, out + n * 12);
     }
+}
+
+/* ------------------------------------------------------------------ */
+/* Reduced-precision operand variant (reading R1) */
+/* ------------------------------------------------------------------ */
+/* A(x) = 1 - (c_sw kappa/2) sum_{mu<nu} sigma_mu_nu (x) F_mu_nu(x) written out as a dense 12x12 matrix
+ * per site, index spin*3+colour (BASELINE.json:north_star formula, reading Q5): A[V][12][12]. */
+void wco_clover_matrix(const int L[4], const cplx* F, double kappa, double csw, cplx* A) {
+    long V = volume(L);
+    double c = clover_coeff(kappa, csw);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < V; i++) {
+        cplx* a = A + i * 144;
+        for (int k = 0; k < 144; k++) a[k] = 0;
+        for (int k = 0; k < 12; k++) a[13 * k] = 1;
+        for (int p = 0; p < 6; p++) {
+            cplx sig[16];
+            wco_sigma(PLANE[p][0], PLANE[p][1], sig);
+            const cplx* f = F + (i * 6 + p) * 9;
+            for (int al = 0; al < 4; al++)
+                for (int be = 0; be < 4; be++)
+                    for (int ca = 0; ca < 3; ca++)
+                        for (int cb = 0; cb < 3; cb++)
+                            a[12 * (3 * al + ca) + 3 * be + cb] -= c * sig[4 * al + be] * f[3 * ca + cb];
+        }
+    }
+}
+
+/* One real number rounded to IEEE binary16 (11-bit significand, exponents -14..15, gradual underflow),
+ * round to nearest, ties to even, after a first rounding to binary32 (the CUDA path's reduced-precision
+ * operands are roundings of its fp32 fields, reading Q16).  x = m 2^e with 0.5 <= m < 1 lies in the
+ * binade whose spacing is 2^(e-11), or 2^-24 below the smallest normal; rint() rounds to nearest even in
+ * the default rounding mode.  Values beyond the largest finite half (65504) do not occur (|U_ab| <= 1,
+ * A(x) = 1 + small) and are returned as +-infinity. */
+static double round_half_1(double x) {
+    x = (double)(float)x;
+    if (x == 0.0 || isnan(x) || isinf(x)) return x;
+    int e;
+    frexp(fabs(x), &e);
+    int eq = e - 11;
+    if (eq < -24) eq = -24;
+    double q = ldexp(1.0, eq);
+    double y = rint(x / q) * q;
+    if (fabs(y) > 65504.0) y = copysign(INFINITY, x);
+    return y;
+}
+/* out[k] = real and imaginary parts of in[k] rounded separately */
+void wco_round_half(long n, const cplx* in, cplx* out) {
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < n; k++) out[k] = round_half_1(creal(in[k])) + I * round_half_1(cimag(in[k]));
 }
 
 int wco_num_threads(void) {

@@ -66,6 +66,14 @@ def sigma(mu: int, nu: int) -> np.ndarray:
     return out
 
 
+def round_half(a) -> np.ndarray:
+    """Entrywise fp64 -> fp32 -> fp16 rounding (nearest even) of a complex array (wco_round_half)."""
+    a = _c(a)
+    out = np.empty_like(a)
+    _load().wco_round_half(C.c_long(a.size), _p(a), _p(out))
+    return out
+
+
 def field_strength(dims, U) -> np.ndarray:
     U = _c(U)
     F = np.empty((volume(dims), 6, 3, 3), np.complex128)
@@ -85,6 +93,20 @@ class Operator:
 
     def _args(self):
         return _i4(self.dims), _p(self.U), _p(self.F), C.c_double(self.kappa), C.c_double(self.csw)
+
+    def clover_matrix(self) -> np.ndarray:
+        """A(x) = 1 - (c_sw kappa/2) sum sigma (x) F as dense 12x12 matrices, [V][12][12] (wco_clover_matrix)."""
+        A = np.empty((self.V, 12, 12), np.complex128)
+        _load().wco_clover_matrix(_i4(self.dims), _p(self.F), C.c_double(self.kappa), C.c_double(self.csw), _p(A))
+        return A
+
+    def with_operands(self, U, A):
+        """The same lattice and kappa with explicit links U [V][4][3][3] and site-diagonal matrices A [V][12][12]."""
+        return ExplicitOperator(self, U, A)
+
+    def rounded(self):
+        """Reduced-precision operand variant (reading R1): links and A(x) rounded entrywise to fp16."""
+        return self.with_operands(round_half(self.U), round_half(self.clover_matrix()))
 
     def apply_D(self, v):
         v = _c(v)
@@ -176,3 +198,38 @@ class Operator:
     def true_residual(self, eta, phi) -> float:
         eta, phi = _c(eta), _c(phi)
         return float(_load().wco_true_residual(*self._args(), _p(eta), _p(phi)))
+
+
+class ExplicitOperator(Operator):
+    """Operator whose site-diagonal term is the stored matrix A(x) (wco_set_explicit_clover is set around every
+    call into the C library and cleared afterwards); F and c_sw are not used."""
+
+    def __init__(self, base, U, A):
+        self.dims, self.V, self.kappa, self.csw = base.dims, base.V, base.kappa, base.csw
+        self.U = _c(U).reshape(self.V, 4, 3, 3)
+        self.F = base.F
+        self.A = _c(A).reshape(self.V, 12, 12)
+
+    def clover_matrix(self):
+        return self.A.copy()
+
+
+def _wrap_explicit(name):
+    plain = getattr(Operator, name)
+
+    def call(self, *a, **k):
+        lib = _load()
+        lib.wco_set_explicit_clover(_p(self.A))
+        try:
+            return plain(self, *a, **k)
+        finally:
+            lib.wco_set_explicit_clover(C.c_void_p(0))
+
+    call.__name__ = name
+    call.__doc__ = plain.__doc__
+    return call
+
+
+for _n in ("apply_D", "apply_D_sites", "apply_D_box", "mr_block", "ras_apply", "sap_apply", "bicgstab",
+           "nested_bicgstab", "true_residual"):
+    setattr(ExplicitOperator, _n, _wrap_explicit(_n))
