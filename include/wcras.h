@@ -88,6 +88,16 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
  * Call before wcras_ras_precondition. */
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
 
+/* Operand storage of the RAS block solver (SURVEY.md 8(f) NEXT-4 "reduced-precision storage of links+clover"; DESIGN.md
+ * reading R1).  bits = 32 (default): the fp32 links and clover blocks.  bits = 16: the preconditioner is K_RAS of the
+ * operator D~ whose links and packed clover blocks are the fp16 roundings (round to nearest even) of the fp32 ones --
+ * Alg. 1 unchanged, block solves AND residual updates with D~, all arithmetic in fp32.  The Krylov
+ * operator D, the outer solver and the stopping criterion are not touched, so the solution still meets the fp64 true
+ * residual.  On the persistent one-CTA-per-domain tier (extended domains of <= 256 sites) the operands are then STORED as
+ * fp16 (288 instead of 576 bytes per site and cycle) and staged into shared memory by TMA bulk copies (ras_cta16.cu);
+ * the other tiers compute with fp32 copies of the rounded fields.  Takes effect at the next wcras_ras_precondition. */
+int wcras_set_operand_precision(wcras_ctx* ctx, int bits);
+
 /* Order in which the full-lattice Dslash visits the sites (a traversal order only; no layout changes, results are
  * identical): ztile = -1 automatic (default: plain order x,y,z,t; above ~60 MB of operands per t-slice the order
  * x, y, z within a tile, t, z tile, with the largest tile whose slab stays under 30 MB, so that the t-neighbours are

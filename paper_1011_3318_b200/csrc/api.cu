@@ -52,6 +52,7 @@ int wcras_destroy(wcras_ctx* ctx) {
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
     if (ctx->dm) cudaFree(ctx->dm);
+    if (ctx->dm16) { cudaFree(ctx->dm16); cudaFree(ctx->rf_dm); }
     if (ctx->hb) cudaFree(ctx->hb);
     if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
@@ -82,6 +83,13 @@ int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     NEED(tier >= 0 && tier <= 4, "set_ras_tier: tier must be 0..4");
     ctx->tier_request = tier == 4 ? 2 : tier;
     ctx->chain_cycles = tier != 4;
+    return WCRAS_OK;
+}
+
+int wcras_set_operand_precision(wcras_ctx* ctx, int bits) {
+    NEED(ctx, "null ctx");
+    NEED(bits == 32 || bits == 16, "set_operand_precision: bits must be 32 or 16");
+    ctx->op_prec = bits;
     return WCRAS_OK;
 }
 

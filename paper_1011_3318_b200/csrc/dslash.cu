@@ -281,16 +281,16 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
 #define WC_DSL(TH, BLOCK, INP, OUTP, BM, DV, POFF)                                                                                    \
     {                                                                                                                              \
         if (dot == 1)                                                                                                              \
-            dslash_kernel<T, false, TH, 1, 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, 1, 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
         else if (dot == 2)                                                                                                         \
-            dslash_kernel<T, false, TH, 1, 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, 1, 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
         else if (b_minus)                                                                                                          \
-            dslash_kernel<T, true, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP,  \
+            dslash_kernel<T, true, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP,  \
                                                                               BM, nullptr, nullptr, 0, 0, rstride, ztile);         \
         else                                                                                                                       \
-            dslash_kernel<T, false, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, nullptr, nullptr, 0, 0, rstride, ztile);   \
         ctx->launches++;                                                                                                           \
     }

@@ -208,6 +208,11 @@ int ras_cta_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_sap_pdir(const FusedGeom& fg);
+int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
+int ras_round_fields(wcras_ctx* ctx);
+int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_cta16_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
     RasConfig rc;
@@ -227,6 +232,8 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     if (ctx->tier_request >= 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
     rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
     if (int e = ensure_workspace(ctx)) return e;
+    // 16-bit operand mode (reading R1): every path of the preconditioner sees the fp16-rounded links and clover blocks
+    if (ctx->op_prec == 16) if (int e = ras_round_fields(ctx)) return e;
     // per-domain workspace of the generic tier (kept even when the fused tier is active: cheap to hold)
     if (ctx->mr_rho) {
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -245,10 +252,18 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         cudaFree(ctx->dm);
         ctx->dm = nullptr;
     }
+    if (ctx->dm16) {
+        WC_CUDA(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->dm16); cudaFree(ctx->rf_dm);
+        ctx->dm16 = nullptr; ctx->rf_dm = nullptr;
+    }
     if (rc.tier == 2) {
         fgeom.pdir = ras_cta_sap_pdir(fgeom);
         ctx->fused = fgeom;
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
+        // 16-bit operand mode: the staged fp16 kernel takes the single-right-hand-side work of this tier (its grid size
+        // and halo geometry are those of ras_cta_prepare: same CTA shape, one CTA per SM)
+        rc.cta16 = rc.cta && ctx->op_prec == 16 && ras_cta16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
         if (!rc.cta) ras_fused_pack(ctx, ctx->fused, rc.nd);
         if (!rc.cta) {  // halo geometry of the chained cycles on the cluster tier (buffers allocated on first use)
             int nface = 1;
@@ -269,7 +284,7 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
     const int TH = 128;
     const dim3 grid((rc.nloc + TH - 1) / TH, rc.nd);
     WC_CUDA(cudaMemsetAsync(ctx->mr_scal, 0, sizeof(double) * 4 * (size_t)rc.nd * rc.niter, ctx->stream));
-    const Fields<float> f = ctx->fields<float>();
+    const Fields<float> f = ras_fields(ctx);
     const float kappa = (float)ctx->kappa;
     for (int it = 0; it < rc.niter; it++) {
         double* scal = ctx->mr_scal + (size_t)it * rc.nd * 4;
@@ -291,6 +306,7 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
 static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     TimedRegion tr(ctx, TC_BLOCK);
     ctx->block_dv += ctx->ras.niter;
+    if (ctx->ras.tier == 2 && ctx->ras.cta16 && ctx->nrhs == 1) return ras_cta16_block_solve(ctx, r, vout, accum);
     if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
     const size_t rstride = (size_t)6 * ctx->geom.V;
     for (int k = 0; k < ctx->nrhs; k++) {  // cluster and generic tiers: one right-hand side of the stack at a time
@@ -314,15 +330,22 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
             snprintf(ctx->err, sizeof ctx->err, "multiplicative Schwarz needs overlap 0, domains of <= 256 sites and an even number of blocks in every cut direction");
             return WCRAS_UNSUPPORTED;
         }
-        return ras_cta_apply_sap(ctx, r, v);
+        return rc.cta16 && ctx->nrhs == 1 ? ras_cta16_apply_sap(ctx, r, v) : ras_cta_apply_sap(ctx, r, v);
     }
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
+    if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cta16_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
     if (rc.tier == 2 && !rc.cta && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];
     const float4* rcur = r;
+    // 16-bit operand mode: Alg.1 line 9 uses the same rounded operator as the block solves (reading R1)
+    struct RoundedScope {
+        wcras_ctx* c;
+        explicit RoundedScope(wcras_ctx* cc) : c(cc) { c->dslash_rounded = c->op_prec == 16; }
+        ~RoundedScope() { c->dslash_rounded = 0; }
+    } rounded_scope(ctx);
     for (int j = 0; j < rc.nras; j++) {
         // v_j is needed on its own for r -= D v_j, so only the last cycle accumulates straight into phi
         const bool lastc = j == rc.nras - 1;

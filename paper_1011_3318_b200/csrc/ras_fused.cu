@@ -535,7 +535,7 @@ void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
     if (fg.s != 0) return;
     const size_t bytes = sizeof(float4) * 36 * (size_t)fg.nsp * fg.C * nd;
     if (cudaMalloc((void**)&ctx->dm, bytes) != cudaSuccess) { cudaGetLastError(); ctx->dm = nullptr; return; }
-    pack_cluster_dm_kernel<<<nd * fg.C, fg.nsp, 0, ctx->stream>>>(fg, ctx->fields<float>(), ctx->dm);
+    pack_cluster_dm_kernel<<<nd * fg.C, fg.nsp, 0, ctx->stream>>>(fg, ras_fields(ctx), ctx->dm);
     ctx->launches++;
     if (cudaGetLastError() != cudaSuccess) { cudaFree(ctx->dm); ctx->dm = nullptr; }
 }
@@ -543,7 +543,7 @@ void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd) {
 // v = K_RAS r with NRAS chained cycles on the cluster tier (overlap 0, one right-hand side): as ras_cta_apply_chained
 int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
     const FusedGeom& fg = ctx->fused;
-    const Fields<float> f = ctx->fields<float>();
+    const Fields<float> f = ras_fields(ctx);
     const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;
     const int nclus = nd < fg.nclus ? nd : fg.nclus;
     if (int rc = ensure_halo(ctx, 1)) return rc;
@@ -567,7 +567,7 @@ int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
 
 int ras_fused_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
-    const Fields<float> f = ctx->fields<float>();
+    const Fields<float> f = ras_fields(ctx);
     const int nclus = ctx->ras.nd < fg.nclus ? ctx->ras.nd : fg.nclus;
     if (fg.C > 1) WC_CUDA(launch_fused<true>(fg, ctx->ras.nd, nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0, 0, nullptr, nullptr, nullptr, ctx->dm));
     else WC_CUDA(launch_fused<false>(fg, ctx->ras.nd, nclus, ctx->stream, f, (float)ctx->kappa, r, vout, accum ? 1 : 0, 0, nullptr, nullptr, nullptr, ctx->dm));

@@ -138,6 +138,7 @@ struct RasConfig {
     int nloc = 0;                 // sites per extended domain
     int tier = 1;                 // 1 generic, 2 fused
     bool cta = false;             // fused tier, single persistent CTA per domain (ras_cta.cu)
+    bool cta16 = false;           // the same with fp16 operand storage staged by TMA (ras_cta16.cu)
 };
 constexpr int FUSED_CTA_MAX_THREADS = 256;
 
@@ -161,6 +162,18 @@ struct wcras_ctx {
     int chain_cycles = 1;          // overlap 0, persistent-CTA tier: NRAS cycles chained through rho_fin (ras_cta.cu)
     FusedGeom fused;               // valid when ras.tier == 2
     float4* dm = nullptr;          // domain-major operand copy of the persistent-CTA tier: [nd][36][nsp]
+    int op_prec = 32;              // operand storage of the block solver: 32, or 16 (reading R1: K_RAS of the operator with
+                                   // fp16-rounded links and clover blocks), wcras_set_operand_precision
+    uint4* dm16 = nullptr;         // fp16 domain-major operand copy (ras_cta16.cu): [nd][18][nsp]
+    float4* rf_dm = nullptr;       // rho_fin of the chained cycles, domain-major: [nd][6][nsp]
+    int4* dom_org = nullptr;       // ras_cta16: first site of every extended domain (inside the rf_dm allocation)
+    unsigned* dom_bc = nullptr;    //            block coordinates of every domain, 8 bits each
+    int stage_halo = 0;            // ras_cta16: halo slots staged in shared memory
+    size_t cta16_smem = 0;         // its dynamic shared memory
+    float4* r16a = nullptr;        // fp32 copies of the fp16-rounded links and clover blocks (16-bit operand mode):
+    float2* r16b = nullptr;        //   operands of every K_RAS path that does not read dm16
+    float4* r16c = nullptr;
+    int dslash_rounded = 0;        // the next fp32 dslash applies the rounded operator (r -= D~ v inside K_RAS)
     int cta_grid = 0;              // its persistent grid size
     float4* hb = nullptr;          // halo buffers of the chained K_RAS cycles: [2][nd][8][3][nface]
     int nface = 0;
@@ -199,9 +212,18 @@ struct wcras_ctx {
     char err[512] = {0};
 
     template <typename T> wc::Fields<T> fields() const;
+    template <typename T> wc::Fields<T> dslash_fields() const;  // fields<T>(), or the rounded copies while dslash_rounded
 };
 template <> inline wc::Fields<float> wcras_ctx::fields<float>() const { return wc::Fields<float>{g32a, g32b, c32}; }
 template <> inline wc::Fields<double> wcras_ctx::fields<double>() const { return wc::Fields<double>{g64, c64}; }
+template <> inline wc::Fields<double> wcras_ctx::dslash_fields<double>() const { return fields<double>(); }
+template <> inline wc::Fields<float> wcras_ctx::dslash_fields<float>() const {
+    return dslash_rounded && r16a ? wc::Fields<float>{r16a, r16b, r16c} : fields<float>();
+}
+// operands of the preconditioner: the fp32 fields, or their fp16-rounded copies in 16-bit operand mode (reading R1)
+inline wc::Fields<float> ras_fields(const wcras_ctx* ctx) {
+    return ctx->op_prec == 16 && ctx->r16a ? wc::Fields<float>{ctx->r16a, ctx->r16b, ctx->r16c} : ctx->fields<float>();
+}
 
 #define WC_CUDA(call)                                                                                   \
     do {                                                                                                \

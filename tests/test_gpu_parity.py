@@ -244,6 +244,87 @@ def test_ras_apply(which, block, s, nit, nras, tier):
     cs.ctx.set_ras_tier(0)
 
 
+FP16_CASES = [
+    # (case, block, overlap, N_dominv, NRAS): persistent tier with fp16 operand storage + TMA staging (overlap 0: chained
+    # cycles through the domain-major rho_fin; overlap 1: unchained, residual update with the rounded operator), ragged
+    # shapes (nsp < 256, padding lanes), wrap-around directions, and shapes that fall to the cluster / generic tiers
+    (0, (2, 2, 2, 2), 0, 4, 3), (0, (2, 2, 2, 2), 1, 3, 2), (0, (4, 4, 4, 4), 0, 6, 1),
+    (1, (4, 4, 4, 4), 0, 2, 3), (1, (4, 4, 4, 4), 0, 5, 1), (1, (8, 4, 4, 2), 0, 3, 3), (1, (4, 4, 4, 4), 1, 2, 2),
+    ("ragged", (3, 4, 5, 2), 0, 2, 3), ("ragged", (2, 2, 5, 4), 1, 3, 2), ("ragged", (3, 2, 5, 2), 0, 1, 2),
+    (2, (4, 4, 4, 4), 0, 2, 3), (2, (8, 8, 4, 4), 0, 2, 2), (2, (8, 4, 4, 4), 2, 2, 2),
+]
+
+
+def rounded_op(cs):
+    if not hasattr(cs, "op16"):
+        cs.op16 = cs.op.rounded()
+    return cs.op16
+
+
+@pytest.mark.parametrize("tier", [0, 1, 4])
+@pytest.mark.parametrize("which,block,s,nit,nras", FP16_CASES)
+def test_ras_apply_fp16_operands(which, block, s, nit, nras, tier):
+    """wcras_set_operand_precision(16) (reading R1): K_RAS of the operator with fp16-rounded
+    links and clover blocks, against the oracle's Alg. 1 on its own rounding of the same operands (fp64 arithmetic)."""
+    cs = ragged_case() if which == "ragged" else case(which)
+    cs.ctx.set_ras_tier(tier)
+    cs.ctx.set_operand_precision(16)
+    try:
+        try:
+            cs.ctx.ras_precondition(block, s, nit, nras)
+        except binding.WcrasError as e:
+            if tier == 4 and e.code == binding.UNSUPPORTED:
+                pytest.skip("shape does not fit the fused tier")
+            raise
+        r32 = I.spinor(cs.dims, 57).astype(np.complex64).astype(np.complex128)
+        want = rounded_op(cs).ras_apply(block, s, nit, nras, r32)
+        got = cs.ras_apply(r32)
+        assert rel(got, want) <= TOL_RAS
+        # and it is not the unrounded preconditioner: the two differ at the fp16 rounding level
+        exact = cs.op.ras_apply(block, s, nit, nras, r32)
+        assert rel(want, exact) > 2e-5 and rel(got, exact) > 2e-5
+    finally:
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_ras_tier(0)
+
+
+def test_fp16_operands_sap_and_solve():
+    """16-bit operand mode through multiplicative Schwarz (red-black launches of the staged kernel) and through the whole
+    nested solve: the preconditioner changes, the solution still meets the fp64 true residual (oracle, exact operator)."""
+    cs = case(1)
+    cs.ctx.set_ras_tier(0)
+    cs.ctx.set_operand_precision(16)
+    try:
+        r32 = I.spinor(cs.dims, 58).astype(np.complex64).astype(np.complex128)
+        for block, nit, ncyc in (((4, 4, 4, 4), 3, 2), ((8, 4, 4, 2), 2, 3)):
+            cs.ctx.ras_precondition(block, 0, nit, ncyc)
+            cs.ctx.set_schwarz(True)
+            assert rel(cs.ras_apply(r32), rounded_op(cs).sap_apply(block, nit, ncyc, r32)) <= TOL_RAS
+            cs.ctx.set_schwarz(False)
+        eta = I.spinor(cs.dims, 2)
+        cs.ctx.set_solver(use_ras=False)
+        _, i0 = cs.solve(eta)
+        for block, s, nit, nras, sap in (((4, 4, 4, 4), 0, 2, 3, False), ((4, 4, 4, 4), 0, 3, 2, True), ((4, 4, 4, 4), 1, 4, 1, False)):
+            cs.ctx.ras_precondition(block, s, nit, nras)
+            cs.ctx.set_schwarz(sap)
+            cs.ctx.set_solver(use_ras=True)
+            phi, info = cs.solve(eta, 1e-12)
+            assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+            assert info["inner_iters"] < i0["inner_iters"]
+        etas = [I.spinor(cs.dims, 2, stream=k) for k in range(2)]      # stacked right-hand sides: fp32 kernel on the rounded operands
+        cs.ctx.set_schwarz(False)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+        x = dev(np.stack(etas), torch.float64)
+        y = torch.empty_like(x)
+        info, res = cs.ctx.solve_multi(2, x, y, 1e-12)
+        phis = host(y, (2, cs.V, 4, 3))
+        assert info["status"] == 0 and all(cs.op.true_residual(etas[k], phis[k]) <= 1e-12 for k in range(2))
+    finally:
+        cs.ctx.set_schwarz(False)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_solver(use_ras=False)
+
+
 SAP_CASES = [
     (0, (2, 2, 2, 2), 4, 1), (0, (2, 2, 2, 2), 4, 3), (1, (4, 4, 4, 4), 3, 1), (1, (4, 4, 4, 4), 2, 2),
     (1, (8, 4, 4, 2), 2, 3), ("ragged", (3, 2, 5, 2), 3, 2),
@@ -481,6 +562,17 @@ def test_full_size_32_ras_apply():
         assert rel(got, want) <= TOL_RAS
         assert np.abs(got - want).max() / np.abs(want).max() <= 10 * TOL_RAS
     cs.ctx.set_ras_tier(0)
+    # the same point with fp16 operand storage (the staged kernel bench.py times), against the oracle's own rounding
+    cs.ctx.set_operand_precision(16)
+    try:
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+        got = cs.ras_apply(r32)
+        want16 = rounded_op(cs).ras_apply((4, 4, 4, 4), 0, 2, 3, r32)
+        assert rel(got, want16) <= TOL_RAS
+        assert np.abs(got - want16).max() / np.abs(want16).max() <= 10 * TOL_RAS
+        assert rel(want16, want) > 2e-5
+    finally:
+        cs.ctx.set_operand_precision(32)
 
 
 def test_full_size_32_sap_and_multi():
