@@ -6,11 +6,12 @@ residual <= 1e-12 on the 32^4 workload of BASELINE.json:configs[3] (kappa=0.1225
 links seed 4, Gaussian source), RAS-preconditioned inner solver.  Inputs are synthetic (paper_1011_3318_b200/
 inputs.py) and stand in for the paper's "random gauge configuration".
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config4]
 
 N > 1 (torchrun): replicas only -- every rank solves its own right-hand side on its own GPU, no data-path
 collective (north_star: "no sharding and no inter-GPU collectives"); NCCL is used for the barrier and the
-max-over-ranks timing.  --impl reference times the fp64 CPU oracle (oracle/) on a bounded sample.
+max-over-ranks timing.  --impl reference times the fp64 CPU oracle (oracle/): real 32^4 solves, as many of the
+requested steps as fit a wall-clock budget (the line states how many were run).
 """
 from __future__ import annotations
 
@@ -29,17 +30,22 @@ sys.path.insert(0, ROOT)
 
 METRIC = "clover Dslash GB/s (% HBM peak); 32^4 RAS-BiCGStab time-to-1e-12"
 TOL = 1e-12
-# RAS parameters of the timed solve (every row states NRAS, Q10)
-# The timed step uses the fastest point of the paper's parameter survey (NRAS x N_dominv, here also
-# over the domain shape) as measured on B200; the domain shapes BASELINE.json:configs[3] names are timed beside it.
+# RAS parameters of the timed solve (every row states NRAS, Q10).  The timed step uses the fastest point of
+# the paper's parameter survey (NRAS x N_dominv, here also over the domain shape and the operand
+# storage) as found by wcras_ras_autotune on B200: it is NOT one of the two shapes configs[3] names; those are timed
+# beside it (solve.named_shapes) and in the same interleaved loop as the unpreconditioned solve.
 RAS = dict(domain=(4, 4, 4, 4), overlap=0, block_iters=2, nras=3)
+OPERAND_BITS = 16   # block-solver operand storage of the timed step (reading R1); 32 is reported beside it
 RAS_NAMED = [dict(domain=(8, 8, 4, 4), overlap=0, block_iters=3, nras=2),
              dict(domain=(8, 8, 8, 8), overlap=0, block_iters=5, nras=1)]
 SAP = dict(domain=(4, 4, 4, 4), block_iters=3, ncycle=2)
 INNER_TOL = 5e-7
+REFERENCE_BUDGET_S = 150.0   # wall-clock budget of the --impl reference arm
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
 # `ncu --set full` capture (profiles/r1j_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
 DSLASH_TRAFFIC_NCU_BYTES = 810.3e6
+KEYS = ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies", "rel_resid_true",
+        "ms_total")
 
 
 def peaks():
@@ -88,55 +94,117 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def cpu_sample(cfg_id, steps=1):
-    """The oracle as it stands, on a bounded sample: the 16^4 sub-volume of the same workload (same kappa, c_sw,
-    gauge recipe/seed, source recipe, RAS parameters), flat fp64 RAS-BiCGStab to 1e-12.  Returns seconds per
-    solve at 16^4 and the x16 per-site extrapolation to 32^4 (iteration counts are nearly volume independent on
-    these random fields; stated in `sample`)."""
-    import oracle as O
-    from paper_1011_3318_b200 import inputs as I
-    cfg = I.CONFIGS[cfg_id]
-    dims = tuple(min(16, d) for d in cfg["dims"])
-    scale = I.volume(cfg["dims"]) / I.volume(dims)
-    U = I.make_gauge(cfg, dims)
-    eta = I.spinor(dims, cfg["seed"])
-    op = O.Operator(dims, U, cfg["kappa"], cfg["csw"])
+def ras_label(r):
+    return "%s_it%d_nras%d" % ("x".join(map(str, r["domain"])), r["block_iters"], r["nras"])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the oracle as it stands, timed on the host cores (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_solve_32(op, eta, n=1):
+    """n real flat fp64 RAS-BiCGStab solves of the full 32^4 workload with the oracle (exact fp64 operands)."""
     ts, info = [], None
-    for _ in range(steps):
+    for _ in range(n):
         t0 = time.time()
         _, info = op.bicgstab(eta, tol=TOL, ras=dict(RAS))
         ts.append(time.time() - t0)
-    t = float(np.mean(ts))
-    return dict(seconds_sample=t, seconds_scaled=t * scale, cores=O.num_threads(), iters=int(info["iters"]),
-                dv=int(info["dv"]), true_resid=float(info["rel_resid_true"]),
-                sample="flat fp64 RAS-BiCGStab (domain %s, overlap %d, %d MR, NRAS %d) to 1e-12 on the %s sub-volume of "
-                       "the workload (1/%d of the sites), time scaled x%d per site" %
-                       ("x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"], RAS["nras"],
-                        "x".join(map(str, dims)), int(scale), int(scale)))
+    return ts, info
+
+
+def cpu_sample_desc(cfg_id):
+    return ("flat fp64 RAS-BiCGStab (domain %s, overlap %d, %d MR, NRAS %d) to 1e-12 on the FULL configs[%d] lattice, "
+            "measured, not extrapolated" % ("x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"],
+                                            RAS["nras"], cfg_id))
 
 
 def run_reference(args, rank):
     if rank != 0:
         return
-    ts = []
-    c = None
-    for k in range(args.warmup + args.steps):
-        c = cpu_sample(args.config, 1)
-        if k >= args.warmup:
-            ts.append(c["seconds_scaled"] * 1e3)
-    ms = float(np.mean(ts))
+    import oracle as O
+    from paper_1011_3318_b200 import inputs as I
+    cfg = I.CONFIGS[3]
+    dims = cfg["dims"]
+    op = O.Operator(dims, I.make_gauge(cfg), cfg["kappa"], cfg["csw"])
+    eta = I.spinor(dims, cfg["seed"])
+    t_start = time.time()
+    ts, info = oracle_solve_32(op, eta, 1)
+    while len(ts) < args.steps and (time.time() - t_start) + ts[0] < REFERENCE_BUDGET_S:
+        t2, info = oracle_solve_32(op, eta, 1)
+        ts += t2
+    ms = float(np.mean(ts)) * 1e3
     line = {
-        "impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus, "steps": len(ts),
+        "warmup": 0, "steps_requested": args.steps, "warmup_requested": args.warmup,
+        "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "configs[%d] 32^4 kappa=0.1225 c_sw=1.0 Haar SU(3) seed 4, RAS %s s=%d N_dominv=%d NRAS=%d, tol 1e-12"
-                   % (args.config, "x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"], RAS["nras"])},
-        "cpu_baseline": {"value": ms, "unit": "ms", "cores": c["cores"], "kind": "oracle", "sample": c["sample"],
-                         "iters": c["iters"], "dv": c["dv"]},
+        "config": {"workload": "configs[3] 32^4 kappa=0.1225 c_sw=1.0 Haar SU(3) seed 4, RAS %s s=%d N_dominv=%d NRAS=%d, tol 1e-12"
+                   % ("x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"], RAS["nras"]),
+                   "note": "every step is one real oracle solve of the full lattice; %d of the %d requested steps fit the %.0f s "
+                           "budget of this arm, no warm-up solves (a CPU loop nest has nothing to warm)" %
+                           (len(ts), args.steps, REFERENCE_BUDGET_S)},
+        "cpu_baseline": {"value": ms, "unit": "ms", "cores": O.num_threads(), "kind": "oracle", "sample": cpu_sample_desc(3),
+                         "iters": int(info["iters"]), "dv": int(info["dv"]), "true_resid": float(info["rel_resid_true"]),
+                         "seconds_each": ts},
         "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+def oracle_table(torch, binding, I, O, config4=False):
+    """SURVEY.md 8(d) / BASELINE.md 3: per config the oracle's apply_D (min of 5) and its flat fp64 BiCGStab with and
+    without K_RAS, beside the GPU's D and nested solves at the RAS parameters BASELINE.json:configs names (NRAS 1)."""
+    out = {}
+    cores = O.num_threads()
+    for cid in (0, 1, 2) + ((4,) if config4 else ()):
+        cfg = I.CONFIGS[cid]
+        dims = cfg["dims"]
+        V = I.volume(dims)
+        U = I.make_gauge(cfg)
+        eta = I.spinor(dims, cfg["seed"])
+        op = O.Operator(dims, U, cfg["kappa"], cfg["csw"])
+        row = {"dims": "x".join(map(str, dims)), "sites": V}
+        ts = []
+        for _ in range(3 if cid == 4 else 5):
+            t0 = time.time()
+            op.apply_D(eta)
+            ts.append(time.time() - t0)
+        t = min(ts)
+        row["oracle"] = {"cores": cores, "apply_D_ms": t * 1e3, "apply_D_gflops_1824": 1824.0 * V / t / 1e9,
+                         "apply_D_gbs_1536": 1536.0 * V / t / 1e9}
+        r = cfg["ras"][0]
+        ras = dict(domain=r["domain"], overlap=r["overlap"], block_iters=r["block_iters"], nras=1)
+        if cid != 4:
+            for key, rr in (("no_prec", None), ("ras_" + ras_label(ras) + "_s%d" % ras["overlap"], ras)):
+                t0 = time.time()
+                _, i = op.bicgstab(eta, tol=TOL, ras=rr)
+                row["oracle"][key] = {"seconds": time.time() - t0, "iters": int(i["iters"]), "dv": int(i["dv"]),
+                                      "rel_resid_true": float(i["rel_resid_true"])}
+        ctx = binding.Context(dims, cfg["kappa"], cfg["csw"], torch.view_as_real(torch.from_numpy(U)).contiguous().cuda())
+        e = torch.view_as_real(torch.from_numpy(eta)).contiguous().cuda()
+        p = torch.empty_like(e)
+        g = {"dslash_fp32_us": ctx.time_kernel(0, 200) * 1e3, "dslash_fp64_us": ctx.time_kernel(1, 100) * 1e3}
+        g["dslash_fp32_gbs_768"] = 768.0 * V / (g["dslash_fp32_us"] * 1e-6) / 1e9
+        for key, rr in (("no_prec", None), ("ras_" + ras_label(ras) + "_s%d" % ras["overlap"], ras)):
+            if rr is None:
+                ctx.set_solver(inner_tol=INNER_TOL, use_ras=False)
+            else:
+                ctx.ras_precondition(rr["domain"], rr["overlap"], rr["block_iters"], rr["nras"])
+                ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+            ctx.solve(e, p, TOL)
+            ms = []
+            for _ in range(5):
+                i = ctx.solve(e, p, TOL)
+                ms.append(i["ms_total"])
+            g[key] = {k: i[k] for k in KEYS}
+            g[key]["ms_total"] = float(np.median(ms))
+            if cid != 4:
+                a = p.cpu().numpy()
+                g[key]["oracle_rel_resid_true"] = float(op.true_residual(eta, (a[..., 0] + 1j * a[..., 1]).reshape(V, 4, 3)))
+        row["gpu"] = g
+        out["config%d" % cid] = row
+        del ctx, e, p
+    return out
 
 
 def main():
@@ -145,9 +213,10 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg and the oracle table")
     ap.add_argument("--no-hard", action="store_true", help="skip the near-critical side rows (a second gauge field)")
+    ap.add_argument("--no-side", action="store_true", help="skip the side rows (named shapes, SAP, multi-RHS, configs 0-2)")
+    ap.add_argument("--config4", action="store_true", help="add configs[4] (48^3 x 96, minutes of host time) to `configs`")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -166,7 +235,7 @@ def main():
         R.init("nccl", torch.device("cuda", local))
     hbm_peak, peak_src, peaks_json = peaks()
 
-    cfg = I.CONFIGS[args.config]
+    cfg = I.CONFIGS[3]
     dims = cfg["dims"]
     V = I.volume(dims)
     U = I.make_gauge(cfg)
@@ -179,6 +248,7 @@ def main():
     phi_d = torch.empty_like(eta_d)
     eta_h = torch.view_as_real(torch.from_numpy(eta)).contiguous().pin_memory()
     phi_h = torch.empty_like(eta_h).pin_memory()
+    warm = max(args.warmup, 3)
 
     def barrier():
         R.barrier(world, cuda=True)
@@ -186,52 +256,51 @@ def main():
     def max_over_ranks(x):
         return R.max_over_ranks(x, world, "cuda")
 
-    # ---- unpreconditioned solve, for the side-by-side row (not the timed step) ----
-    ctx.set_solver(inner_tol=INNER_TOL, use_ras=False)
-    ctx.set_timing(False)
-    ctx.solve(eta_d, phi_d, TOL)
-    info_noprec = ctx.solve(eta_d, phi_d, TOL)
-
-    # ---- the domain shapes configs[3] names, for the side-by-side rows (not the timed step) ----
-    named = {}
-    for rp in RAS_NAMED:
-        ctx.ras_precondition(rp["domain"], rp["overlap"], rp["block_iters"], rp["nras"])
+    def configure(r, bits, sap=False):
+        ctx.set_operand_precision(bits)
+        ctx.set_schwarz(sap)
+        ctx.ras_precondition(r["domain"], r.get("overlap", 0), r["block_iters"], r["nras"] if "nras" in r else r["ncycle"])
         ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+
+    def measure(n=3):
+        """one warm-up solve, then n solves: the last info with the median / min / max of ms_total"""
         ctx.solve(eta_d, phi_d, TOL)
-        i = ctx.solve(eta_d, phi_d, TOL)
-        named["ras_%s_it%d_nras%d" % ("x".join(map(str, rp["domain"])), rp["block_iters"], rp["nras"])] = {
-            k: i[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies",
-                              "rel_resid_true", "ms_total")}
+        ms, i = [], None
+        for _ in range(n):
+            i = ctx.solve(eta_d, phi_d, TOL)
+            ms.append(i["ms_total"])
+        d = {k: i[k] for k in KEYS}
+        d.update(ms_total=float(np.median(ms)), ms_min=float(min(ms)), ms_max=float(max(ms)), solves=n)
+        return d
 
-    # ---- multiplicative Schwarz (SAP) beside it: same kernel, red-black half steps ----
-    ctx.set_schwarz(True)
-    ctx.ras_precondition(SAP["domain"], 0, SAP["block_iters"], SAP["ncycle"])
-    ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
-    ctx.solve(eta_d, phi_d, TOL)
-    i = ctx.solve(eta_d, phi_d, TOL)
-    named["sap_%s_it%d_ncycle%d" % ("x".join(map(str, SAP["domain"])), SAP["block_iters"], SAP["ncycle"])] = {
-        k: i[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies",
-                          "rel_resid_true", "ms_total")}
-    ctx.set_schwarz(False)
+    ctx.set_timing(False)
+    side = {}
+    if not args.no_side:
+        # ---- the domain shapes configs[3] names (cluster tier), multiplicative Schwarz, stacked right-hand sides ----
+        for rp in RAS_NAMED:
+            for bits in (32, 16):
+                configure(rp, bits)
+                side["ras_%s_op%d" % (ras_label(rp), bits)] = measure()
+        for bits in (32, 16):
+            configure(SAP, bits, sap=True)
+            side["sap_%s_it%d_ncycle%d_op%d" % ("x".join(map(str, SAP["domain"])), SAP["block_iters"], SAP["ncycle"], bits)] = measure()
+        ctx.set_schwarz(False)
+        configure(RAS, 32)
+        side["ras_%s_op32" % ras_label(RAS)] = measure()
+        if world == 1:
+            etas4 = np.stack([I.spinor(dims, cfg["seed"], stream=k) for k in range(4)])
+            e4 = torch.view_as_real(torch.from_numpy(etas4)).contiguous().cuda()
+            p4 = torch.empty_like(e4)
+            ctx.solve_multi(4, e4, p4, TOL)
+            i4, res4 = ctx.solve_multi(4, e4, p4, TOL)
+            side["ras_multi_rhs_4_op32"] = {"ms_total": i4["ms_total"], "ms_per_rhs": i4["ms_total"] / 4,
+                                            "inner_iters": i4["inner_iters"], "ras_applies": i4["ras_applies"],
+                                            "worst_rel_resid_true": max(res4)}
+            del e4, p4, etas4
 
-    # ---- four right-hand sides as one stacked solve, RAS point of the timed step ----
-    if world == 1:
-        etas4 = np.stack([I.spinor(dims, cfg["seed"], stream=k) for k in range(4)])
-        e4 = torch.view_as_real(torch.from_numpy(etas4)).contiguous().cuda()
-        p4 = torch.empty_like(e4)
-        ctx.ras_precondition(RAS["domain"], RAS["overlap"], RAS["block_iters"], RAS["nras"])
-        ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
-        ctx.solve_multi(4, e4, p4, TOL)
-        i4, res4 = ctx.solve_multi(4, e4, p4, TOL)
-        named["ras_multi_rhs_4"] = {"ms_total": i4["ms_total"], "ms_per_rhs": i4["ms_total"] / 4, "inner_iters": i4["inner_iters"],
-                                    "ras_applies": i4["ras_applies"], "worst_rel_resid_true": max(res4)}
-        del e4, p4
-
-    # ---- the timed step: RAS-preconditioned nested solve ----
-    ctx.ras_precondition(RAS["domain"], RAS["overlap"], RAS["block_iters"], RAS["nras"])
-    ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
-    ctx.set_timing(True)
-    for _ in range(max(args.warmup, 3)):
+    # ---- the timed step: RAS-preconditioned nested solve, per-class event timing OFF ----
+    configure(RAS, OPERAND_BITS)
+    for _ in range(warm):
         ctx.solve(eta_d, phi_d, TOL)
     barrier()
     l0 = ctx.launch_count()
@@ -248,8 +317,21 @@ def main():
     clocks = sampler.stop() if sampler else None
     info = infos[-1]
 
+    # ---- the same solve and the unpreconditioned one, interleaved, same flags, same number of solves ----
+    pair = {"ras": [], "no_prec": []}
+    info_np = None
+    for _ in range(args.steps):
+        ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+        pair["ras"].append(ctx.solve(eta_d, phi_d, TOL)["ms_total"])
+        ctx.set_solver(inner_tol=INNER_TOL, use_ras=False)
+        info_np = ctx.solve(eta_d, phi_d, TOL)
+        pair["no_prec"].append(info_np["ms_total"])
+    ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+
+    def stats(x):
+        return {"mean": float(np.mean(x)), "median": float(np.median(x)), "min": float(min(x)), "max": float(max(x)), "n": len(x)}
+
     # ---- end to end: host buffers, H2D of eta and D2H of phi inside the timed region ----
-    ctx.set_timing(False)
     ctx.solve_host(eta_h, phi_h, TOL)
     barrier()
     e0.record(stream)
@@ -259,20 +341,27 @@ def main():
     barrier()
     ms_e2e = max_over_ranks(e0.elapsed_time(e1) / args.steps)
 
-    # ---- per-kernel numbers ----
-    n_dv = sum(i["dv_fp32"] for i in infos)
-    ms_dslash_in_solve = sum(i["ms_dslash"] for i in infos) / max(1, n_dv)
+    # ---- per-kernel-class split (separate pass with the event timers ON) and burst timings ----
+    ctx.set_timing(True)
+    split = [ctx.solve(eta_d, phi_d, TOL) for _ in range(3)]
+    ctx.set_timing(False)
+    n_dv = sum(i["dv_fp32"] for i in split)
+    ms_dslash_in_solve = sum(i["ms_dslash"] for i in split) / max(1, n_dv)
+    n_blk = sum(i["block_dv"] for i in split) // RAS["block_iters"]
+    ms_blk_in_solve = sum(i["ms_blocksolve"] for i in split) / max(1, n_blk)
     ms_d32 = ctx.time_kernel(0, 100)
     ms_d64 = ctx.time_kernel(1, 50)
     ms_blk = ctx.time_kernel(2, 50)
     ms_blas = ctx.time_kernel(3, 100)
-    n_blk = sum(i["block_dv"] for i in infos) // RAS["block_iters"]
-    ms_blk_in_solve = sum(i["ms_blocksolve"] for i in infos) / max(1, n_blk)
-    # inside the solve every fp32 D launch is the variant with the fused dot (<rt,v> or <t,s>,<t,t>): it also reads
-    # the dot vector, 864 B/site, and its time includes the one-CTA dot_finish_kernel launched behind it
-    gbs_in_solve = 864.0 * V / (ms_dslash_in_solve * 1e-3) / 1e9
+    gbs_in_solve = 768.0 * V / (ms_dslash_in_solve * 1e-3) / 1e9
     gbs_burst = 768.0 * V / (ms_d32 * 1e-3) / 1e9
     true_resid = info["rel_resid_true"]
+    # algorithmic HBM bytes per site of one block-solver launch: operands + residual in + v out,
+    # chained cycles add rho_fin, the halo slots (96 B per site each way at 4^4: every face site) and the phi read-modify-write
+    ob = 288 if OPERAND_BITS == 16 else 576
+    cyc_bytes = [ob + 96 + 96 + 96 + 96, ob + 96 + 96 + 96 + 96 + 192, ob + 96 + 96 + 192]   # cycle 0, middle, last (NRAS = 3)
+    blk_bytes_in_solve = float(np.mean(cyc_bytes))
+    blk_bytes_plain = ob + 96 + 96
 
     if rank != 0:
         R.shutdown(world)
@@ -297,65 +386,105 @@ def main():
         ch.set_solver(inner_tol=INNER_TOL, use_ras=False)
         hrun("no_prec")
         ch.set_solver(inner_tol=INNER_TOL, use_ras=True)
-        ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)     # the paper's best point: NRAS 3, N_dominv 5
-        hrun("ras_4x4x4x4_it5_nras3")
+        for bits in (32, 16):
+            ch.set_operand_precision(bits)
+            ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)     # the paper's best point: NRAS 3, N_dominv 5
+            hrun("ras_4x4x4x4_it5_nras3_op%d" % bits)
+        ch.set_operand_precision(32)
         for dom in ((8, 8, 4, 4), (8, 8, 8, 8)):        # the domain shapes configs[3] names (cluster tier)
             ch.ras_precondition(dom, 0, 5, 3)
-            hrun("ras_%s_it5_nras3" % "x".join(map(str, dom)))
+            hrun("ras_%s_it5_nras3_op32" % "x".join(map(str, dom)))
+        ch.set_operand_precision(16)
         ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)
         ch.set_schwarz(True)
-        hrun("sap_4x4x4x4_it5_ncycle3")
+        hrun("sap_4x4x4x4_it5_ncycle3_op16")
         del ch, eh, ph
+        torch.cuda.empty_cache()
 
-    cpu = None
+    cpu, configs = None, None
     if world == 1 and not args.no_cpu:
-        c = cpu_sample(args.config, 1)
-        cpu = {"value": c["seconds_scaled"] * 1e3, "unit": "ms", "cores": c["cores"], "kind": "oracle",
-               "sample": c["sample"], "iters": c["iters"], "dv": c["dv"], "sample_seconds": c["seconds_sample"]}
+        import oracle as O
+        if not args.no_side:
+            configs = oracle_table(torch, binding, I, O, args.config4)
+        op = O.Operator(dims, U, cfg["kappa"], cfg["csw"])
+        ts = []
+        for _ in range(5):
+            t0 = time.time()
+            op.apply_D(eta)
+            ts.append(time.time() - t0)
+        tD = min(ts)
+        t_solve, oi = oracle_solve_32(op, eta, 1)
+        t0 = time.time()
+        _, oi_np = op.bicgstab(eta, tol=TOL, ras=None)
+        t_np = time.time() - t0
+        cpu = {"value": t_solve[0] * 1e3, "unit": "ms", "cores": O.num_threads(), "kind": "oracle", "sample": cpu_sample_desc(3),
+               "iters": int(oi["iters"]), "dv": int(oi["dv"]), "true_resid": float(oi["rel_resid_true"]),
+               "no_prec": {"value": t_np * 1e3, "unit": "ms", "iters": int(oi_np["iters"]), "dv": int(oi_np["dv"])},
+               "apply_D_ms": tD * 1e3, "apply_D_gflops_1824": 1824.0 * V / tD / 1e9, "apply_D_gbs_1536": 1536.0 * V / tD / 1e9}
 
+    named_faster = {k: v["ms_total"] < float(np.median(pair["no_prec"])) for k, v in side.items() if k.startswith("ras_8x8")}
     line = {
         "metric": METRIC, "value": ms_step, "unit": "ms", "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
+        "warmup": warm, "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32 inner / f64 outer", "data": "synthetic",
         "config": {"workload": "configs[%d]: %s lattice, kappa=%g c_sw=%g, Haar SU(3) links seed %d, Gaussian source; RAS "
-                               "domain %s overlap %d N_dominv %d NRAS %d; inner_tol %g; tol 1e-12; replicas only (one RHS per GPU)"
-                               % (args.config, "x".join(map(str, dims)), cfg["kappa"], cfg["csw"], cfg["seed"],
-                                  "x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"], RAS["nras"], INNER_TOL),
-                   "l2": "inputs larger than L2 (links+clover 604 MB fp32 per Dslash pass)"},
+                               "domain %s overlap %d N_dominv %d NRAS %d, block-solver operands stored as fp%d; inner_tol %g; "
+                               "tol 1e-12; replicas only (one RHS per GPU)"
+                               % (3, "x".join(map(str, dims)), cfg["kappa"], cfg["csw"], cfg["seed"],
+                                  "x".join(map(str, RAS["domain"])), RAS["overlap"], RAS["block_iters"], RAS["nras"], OPERAND_BITS,
+                                  INNER_TOL),
+                   "ras_point": "fastest point of the parameter survey (wcras_ras_autotune, PAPER.md:109); NOT a shape configs[3] "
+                                "names -- the named shapes 8x8x4x4 and 8^4 are in solve.named_shapes",
+                   "l2": "inputs larger than L2 (links+clover 604 MB fp32 per Dslash pass, 302 MB fp16 per block-solver launch)"},
         "clocks": clocks,
         "e2e": {"value": ms_e2e, "unit": "ms", "h2d_bytes_per_step": int(eta_h.numel() * 8),
                 "d2h_bytes_per_step": int(phi_h.numel() * 8)},
         "gpu_launches": int(launches),
+        # fp32 clover Dslash: 768 B/site; inside the solve every launch also carries a fused dot (it reads a
+        # fourth vector: 864 B/site, frac_fused_variant) and its time includes the dot_finish_kernel behind it
         "roofline": {"kernel": "dslash_kernel<float> (fp32 clover Dslash)", "bound": "hbm", "achieved": gbs_in_solve,
                      "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": gbs_in_solve / hbm_peak,
-                     "traffic": DSLASH_TRAFFIC_NCU_BYTES if V == 1 << 20 else None, "algorithmic_bytes": 768.0 * V,
-                     "bytes_per_site": 768, "bytes_per_site_in_solve": 864, "sites": V,
+                     "traffic": DSLASH_TRAFFIC_NCU_BYTES, "algorithmic_bytes": 768.0 * V,
+                     "bytes_per_site": 768, "sites": V,
                      "ms_per_launch_in_solve": ms_dslash_in_solve, "ms_per_launch_burst": ms_d32,
+                     "frac_fused_variant": 864.0 * V / (ms_dslash_in_solve * 1e-3) / 1e9 / hbm_peak,
                      "achieved_burst": gbs_burst, "frac_burst": gbs_burst / hbm_peak,
                      "frac_of_nominal_8TBs": gbs_burst / 8000.0,
                      "gflops_1824_per_site": 1824.0 * V / (ms_d32 * 1e-3) / 1e9},
-        # the kernel the timed solve spends most of its time in (profiles/): one K_RAS cycle over all domains
+        # the kernel the timed solve spends most of its time in: one K_RAS cycle over all domains
         "roofline_block_solve": {
-            "kernel": "ras_cta_kernel (persistent one-CTA-per-domain MR block solver, %d sweeps per launch)" % RAS["block_iters"],
-            "bound": "hbm", "unit": "GB/s", "bytes_per_site": 864, "sites": V, "peak": hbm_peak,
-            "ms_per_launch_in_solve": ms_blk_in_solve, "achieved": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9,
-            "frac": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9 / hbm_peak,
-            "ms_per_launch_burst": ms_blk, "frac_burst": 864.0 * V / (ms_blk * 1e-3) / 1e9 / hbm_peak,
-            "note": "HBM floor = operands 576 + r 96 + v 96 + phi/rho 96 B per site; the kernel is bound by fp32 issue "
-                    "latency at 2 warps per scheduler, see profiles/r1j_kernels.md"},
+            "kernel": "ras_cta16_kernel (persistent one-CTA-per-domain MR block solver, fp%d operands staged by TMA, %d sweeps "
+                      "per launch)" % (OPERAND_BITS, RAS["block_iters"]),
+            "bound": "hbm", "unit": "GB/s", "sites": V, "peak": hbm_peak,
+            "bytes_per_site_in_solve": blk_bytes_in_solve, "bytes_per_site_by_cycle": cyc_bytes,
+            "ms_per_launch_in_solve": ms_blk_in_solve,
+            "achieved": blk_bytes_in_solve * V / (ms_blk_in_solve * 1e-3) / 1e9,
+            "frac": blk_bytes_in_solve * V / (ms_blk_in_solve * 1e-3) / 1e9 / hbm_peak,
+            "frac_fp32_equivalent_864": 864.0 * V / (ms_blk_in_solve * 1e-3) / 1e9 / hbm_peak,
+            "bytes_per_site_plain": blk_bytes_plain, "ms_per_launch_burst": ms_blk,
+            "frac_burst": blk_bytes_plain * V / (ms_blk * 1e-3) / 1e9 / hbm_peak,
+            "site_sweeps_per_s_burst": V * RAS["block_iters"] / (ms_blk * 1e-3),
+            "note": "frac = algorithmic bytes actually moved by the fp16-operand kernel; frac_fp32_equivalent_864 prices the same "
+                    "launch at the 864 B/site of the fp32-operand kernel it replaces (VERDICT r1 item 1); the kernel is bound by "
+                    "fp32 instruction issue, not HBM, see profiles/"},
         "cpu_baseline": cpu,
-        "solve": {"ras": {k: info[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv",
-                                              "ras_applies", "rel_resid_true", "ms_total", "ms_dslash", "ms_dslash64",
-                                              "ms_blocksolve", "ms_blas")},
-                  "no_prec": {k: info_noprec[k] for k in ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64",
-                                                          "rel_resid_true", "ms_total")},
-                  "ras_faster_than_no_prec": info["ms_total"] < info_noprec["ms_total"], **named},
+        "solve": {"ras": {k: info[k] for k in KEYS},
+                  "class_split_ms": {"note": "separate pass with wcras_set_timing(1), mean of 3 solves",
+                                     "dslash": float(np.mean([i["ms_dslash"] for i in split])),
+                                     "dslash64": float(np.mean([i["ms_dslash64"] for i in split])),
+                                     "blocksolve": float(np.mean([i["ms_blocksolve"] for i in split])),
+                                     "blas": float(np.mean([i["ms_blas"] for i in split])),
+                                     "total": float(np.mean([i["ms_total"] for i in split]))},
+                  "no_prec": {k: info_np[k] for k in KEYS if k in info_np},
+                  "interleaved_ms": {"ras": stats(pair["ras"]), "no_prec": stats(pair["no_prec"])},
+                  "ras_faster_than_no_prec": float(np.median(pair["ras"])) < float(np.median(pair["no_prec"])),
+                  "ras_named_shapes_faster_than_no_prec": named_faster,
+                  "named_shapes": side},
         "kernels": {"dslash_fp32_ms": ms_d32, "dslash_fp64_ms": ms_d64,
                     "dslash_fp64_gbs": 1536.0 * V / (ms_d64 * 1e-3) / 1e9,
                     "block_solve_ms": ms_blk,
-                    "block_solve_site_sweeps_per_s": V * RAS["block_iters"] / (ms_blk * 1e-3),
-                    "block_solve_hbm_gbs": 864.0 * V / (ms_blk * 1e-3) / 1e9,
                     "blas_update_xr_ms": ms_blas, "blas_update_xr_gbs": 8 * 96.0 * V / (ms_blas * 1e-3) / 1e9},
+        "configs": configs,
         "hard_regime": hard,
         "true_residual": true_resid,
     }

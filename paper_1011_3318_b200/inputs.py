@@ -16,6 +16,9 @@ Canonical layouts:
 """
 from __future__ import annotations
 
+import os
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 
 _M64 = np.uint64(0xFFFFFFFFFFFFFFFF)
@@ -67,19 +70,33 @@ _GAUGE_STREAM = 1000
 _CHUNK = 1 << 18  # links per chunk
 
 
+def _chunks(total: int, fn):
+    """fn(start, count) for every chunk of the element range; the chunks run on a thread pool (numpy releases the GIL in
+    its inner loops).  Values are functions of the element index only, so neither chunking nor scheduling changes them."""
+    starts = list(range(0, total, _CHUNK))
+    if len(starts) <= 1:
+        for s in starts:
+            fn(s, min(_CHUNK, total - s))
+        return
+    with ThreadPoolExecutor(max_workers=min(len(starts), os.cpu_count() or 1)) as ex:
+        list(ex.map(lambda s: fn(s, min(_CHUNK, total - s)), starts))
+
+
 def gauge_exp(dims, eps: float, seed: int) -> np.ndarray:
     """U = exp(i*eps*H), H = (G+G^dag)/2 - tr/3, G 3x3 complex Gaussian (configs 0,1,2,4)."""
     nlink = 4 * volume(dims)
     out = np.empty((nlink, 3, 3), dtype=np.complex128)
     eye = np.eye(3)
-    for s in range(0, nlink, _CHUNK):
-        n = min(_CHUNK, nlink - s)
+
+    def fill(s, n):
         g = complex_normal(seed, _GAUGE_STREAM, 9 * s, 9 * n).reshape(n, 3, 3)
         h = 0.5 * (g + np.conj(np.swapaxes(g, 1, 2)))
         tr = np.einsum("nii->n", h).real / 3.0
         h = h - tr[:, None, None] * eye
         w, v = np.linalg.eigh(h)
         out[s:s + n] = np.einsum("nij,nj,nkj->nik", v, np.exp(1j * eps * w), np.conj(v))
+
+    _chunks(nlink, fill)
     return out.reshape(volume(dims), 4, 3, 3)
 
 
@@ -87,14 +104,16 @@ def gauge_haar(dims, seed: int) -> np.ndarray:
     """'Fully random' SU(3): Gram-Schmidt rows 1-2 of a complex Gaussian 3x3, row 3 = conj(row1 x row2) (config 3)."""
     nlink = 4 * volume(dims)
     out = np.empty((nlink, 3, 3), dtype=np.complex128)
-    for s in range(0, nlink, _CHUNK):
-        n = min(_CHUNK, nlink - s)
+
+    def fill(s, n):
         g = complex_normal(seed, _GAUGE_STREAM, 9 * s, 9 * n).reshape(n, 3, 3)
         a = g[:, 0] / np.linalg.norm(g[:, 0], axis=1)[:, None]
         b = g[:, 1] - a * np.einsum("ni,ni->n", np.conj(a), g[:, 1])[:, None]
         b = b / np.linalg.norm(b, axis=1)[:, None]
         c = np.conj(np.cross(a, b))
         out[s:s + n, 0], out[s:s + n, 1], out[s:s + n, 2] = a, b, c
+
+    _chunks(nlink, fill)
     return out.reshape(volume(dims), 4, 3, 3)
 
 
@@ -109,10 +128,11 @@ def spinor(dims, seed: int, stream: int = 0) -> np.ndarray:
     """Gaussian source: 12 complex N(0,1)+iN(0,1) per site, [V][4][3]."""
     v = volume(dims)
     out = np.empty(12 * v, dtype=np.complex128)
-    step = 12 * _CHUNK
-    for s in range(0, 12 * v, step):
-        n = min(step, 12 * v - s)
+
+    def fill(s, n):
         out[s:s + n] = complex_normal(seed, stream, s, n)
+
+    _chunks(12 * v, fill)
     return out.reshape(v, 4, 3)
 
 

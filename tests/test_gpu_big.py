@@ -1,14 +1,16 @@
-"""BASELINE.json:configs[4] at full size (48^3 x 96, 10.6 M sites, ~60 GB of device memory, a few minutes of host
-time for the synthetic gauge field).  Opt-in: WCRAS_BIG=1 python -m pytest tests/test_gpu_big.py -m gpu -s
+"""BASELINE.json:configs[4] at full size (48^3 x 96, 10.6 M sites, ~60 GB of device memory; most of the run time is
+the host-side generation of the synthetic gauge field and the oracle's field strength).
 
-D is checked on sampled sites the oracle computes one by one; the solutions by the oracle's residual on the same sites
-(the full-lattice residual is the library's own fp64 recomputation, reported beside it)."""
+Always on (north_star: "true relative residual <= 1e-12 on every config"): D fp32/fp64 on sampled sites the oracle computes
+one by one, the unpreconditioned solve and the RAS solve at the point configs[4] names (8^4 domains, overlap 1, 4 MR
+iterations), each checked by the oracle's residual on the sampled sites beside the library's full-lattice fp64 residual.
+WCRAS_BIG=1 adds the other preconditioner variants."""
 import os
 
 import numpy as np
 import pytest
 
-pytestmark = [pytest.mark.gpu, pytest.mark.skipif(os.environ.get("WCRAS_BIG") != "1", reason="set WCRAS_BIG=1 (60 GB, minutes)")]
+pytestmark = [pytest.mark.gpu]
 
 torch = pytest.importorskip("torch")
 
@@ -32,7 +34,7 @@ def test_config4_full_size():
     want = op.apply_D_sites(psi, sites)
 
     def to_host(t):
-        a = t.cpu().double().numpy()
+        a = t.cpu().numpy()
         return (a[..., 0] + 1j * a[..., 1]).reshape(V, 4, 3)
 
     for prec, dt, tol in ((32, torch.float32, 2e-6), (64, torch.float64, 1e-13)):
@@ -40,7 +42,7 @@ def test_config4_full_size():
         y = torch.empty_like(x)
         ctx.apply_D(prec, x, y)
         torch.cuda.synchronize()
-        got = to_host(y)[sites]
+        got = to_host(y)[sites].astype(np.complex128)
         assert np.linalg.norm(got - want) / np.linalg.norm(want) <= tol
         del x, y
     t32, t64 = ctx.time_kernel(0, 20), ctx.time_kernel(1, 10)
@@ -49,25 +51,34 @@ def test_config4_full_size():
     eta_d = torch.view_as_real(torch.from_numpy(psi)).contiguous().cuda()
     phi_d = torch.empty_like(eta_d)
 
-    def solve(label):
-        ctx.solve(eta_d, phi_d, 1e-12)
+    def solve(label, warm=False):
+        if warm:
+            ctx.solve(eta_d, phi_d, 1e-12)
         i = ctx.solve(eta_d, phi_d, 1e-12)
         phi = to_host(phi_d)
         res = np.linalg.norm(psi[sites] - op.apply_D_sites(phi, sites)) / np.linalg.norm(psi[sites])
-        print("%-34s %8.1f ms  inner %3d  K %3d  residual %.1e (oracle, sampled sites %.1e)" % (
+        print("%-40s %8.1f ms  inner %3d  K %3d  residual %.1e (oracle, sampled sites %.1e)" % (
             label, i["ms_total"], i["inner_iters"], i["ras_applies"], i["rel_resid_true"], res))
         assert i["status"] == 0 and i["rel_resid_true"] <= 1e-12 and res <= 3e-12
         return i
 
+    big = os.environ.get("WCRAS_BIG") == "1"
     ctx.set_solver(use_ras=False)
-    solve("no preconditioner")
+    i0 = solve("no preconditioner", warm=big)
     ctx.set_solver(use_ras=True)
-    ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
-    solve("RAS 4^4 overlap 0 N_dominv 2 NRAS 3")
-    ctx.set_schwarz(True)
-    ctx.ras_precondition((4, 4, 4, 4), 0, 3, 2)
-    solve("SAP 4^4 N_dominv 3, 2 cycles")
-    ctx.set_schwarz(False)
     r = cfg["ras"][0]                                     # the configuration BASELINE.json names: 8^4, overlap 1, 4 MR
     ctx.ras_precondition(r["domain"], r["overlap"], r["block_iters"], 1)
-    solve("RAS 8^4 overlap 1 N_dominv 4 (generic tier)")
+    i1 = solve("RAS 8^4 overlap 1 N_dominv 4 NRAS 1", warm=big)
+    assert i1["inner_iters"] < i0["inner_iters"]          # the preconditioner cuts the Krylov iterations
+    if not big:
+        return
+    ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+    solve("RAS 4^4 overlap 0 N_dominv 2 NRAS 3", warm=True)
+    ctx.set_operand_precision(16)
+    ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+    solve("RAS 4^4 overlap 0 N_dominv 2 NRAS 3, fp16 operands", warm=True)
+    ctx.set_schwarz(True)
+    ctx.ras_precondition((4, 4, 4, 4), 0, 3, 2)
+    solve("SAP 4^4 N_dominv 3, 2 cycles, fp16 operands", warm=True)
+    ctx.set_schwarz(False)
+    ctx.set_operand_precision(32)
