@@ -209,6 +209,9 @@ int ras_fused_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 void ras_fused_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd);
 int ras_cta_sap_pdir(const FusedGeom& fg);
 int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
+int ras_stream_prepare(wcras_ctx* ctx, const int b[4], const int ext[4], int s, int niter, FusedGeom* out);
+int ras_stream_pack(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
+int ras_stream_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_round_fields(wcras_ctx* ctx);
 int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
@@ -228,7 +231,13 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     }
     rc.s = s; rc.niter = niter; rc.nras = nras; rc.set = true;
     FusedGeom fgeom;
-    const bool fused_ok = ctx->tier_request != 1 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
+    // tier request 5: force the streamed-operand cluster kernel (tier 2c); automatic: 2a/2b when Omega' fits on chip with
+    // its operands, else 2c when the spinors fit a cluster, else the generic tier
+    bool fused_ok = ctx->tier_request != 1 && ctx->tier_request != 5 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
+    if (!fused_ok && (ctx->tier_request == 0 || ctx->tier_request == 5) && ras_stream_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0) {
+        fused_ok = true;
+        rc.stream = true;
+    }
     if (ctx->tier_request >= 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
     rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
     if (int e = ensure_workspace(ctx)) return e;
@@ -257,7 +266,13 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         cudaFree(ctx->dm16); cudaFree(ctx->rf_dm);
         ctx->dm16 = nullptr; ctx->rf_dm = nullptr;
     }
-    if (rc.tier == 2) {
+    if (rc.tier == 2 && rc.stream) {
+        ctx->fused = fgeom;
+        if (!ras_stream_pack(ctx, fgeom, rc.nd, ras_fields(ctx))) {
+            snprintf(ctx->err, sizeof ctx->err, "ras_precondition: out of device memory for the streamed operand records");
+            return WCRAS_CUDA_ERROR;
+        }
+    } else if (rc.tier == 2) {
         fgeom.pdir = ras_cta_sap_pdir(fgeom);
         ctx->fused = fgeom;
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
@@ -310,7 +325,8 @@ static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum
     if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
     const size_t rstride = (size_t)6 * ctx->geom.V;
     for (int k = 0; k < ctx->nrhs; k++) {  // cluster and generic tiers: one right-hand side of the stack at a time
-        const int e = ctx->ras.tier == 2 ? ras_fused_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
+        const int e = ctx->ras.tier == 2 ? (ctx->ras.stream ? ras_stream_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
+                                                            : ras_fused_block_solve(ctx, r + k * rstride, vout + k * rstride, accum))
                                          : generic_block_solve(ctx, r + k * rstride, vout + k * rstride, accum);
         if (e) return e;
     }
@@ -336,7 +352,7 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
     if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cta16_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
-    if (rc.tier == 2 && !rc.cta && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
+    if (rc.tier == 2 && !rc.cta && !rc.stream && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];
     const float4* rcur = r;

@@ -139,6 +139,7 @@ struct RasConfig {
     int tier = 1;                 // 1 generic, 2 fused
     bool cta = false;             // fused tier, single persistent CTA per domain (ras_cta.cu)
     bool cta16 = false;           // the same with fp16 operand storage staged by TMA (ras_cta16.cu)
+    bool stream = false;          // fused tier 2c: rho, v in (distributed) shared memory, operands streamed (ras_stream.cu)
 };
 constexpr int FUSED_CTA_MAX_THREADS = 256;
 
@@ -169,6 +170,7 @@ struct wcras_ctx {
     int4* dom_org = nullptr;       // ras_cta16: first site of every extended domain (inside the rf_dm allocation)
     unsigned* dom_bc = nullptr;    //            block coordinates of every domain, 8 bits each
     int stage_halo = 0;            // ras_cta16: halo slots staged in shared memory
+    int stream_half = 0;           // ras_stream: operand records packed as fp16
     size_t cta16_smem = 0;         // its dynamic shared memory
     float4* r16a = nullptr;        // fp32 copies of the fp16-rounded links and clover blocks (16-bit operand mode):
     float2* r16b = nullptr;        //   operands of every K_RAS path that does not read dm16

@@ -221,19 +221,21 @@ RAS_CASES = [
 ]
 
 
-@pytest.mark.parametrize("tier", [1, 0, 3, 4])
+@pytest.mark.parametrize("tier", [1, 0, 3, 4, 5])
 @pytest.mark.parametrize("which,block,s,nit,nras", RAS_CASES)
 def test_ras_apply(which, block, s, nit, nras, tier):
-    """tier 1 = generic, 0 = automatic (persistent CTA kernel for |Omega'| <= 256, cluster kernel above, generic
-    if neither fits), 3 = cluster kernel forced (skipped where the shape does not fit it), 4 = fused tier with the
-    NRAS cycles not chained (tier 0 chains them when the overlap is 0)."""
+    """tier 1 = generic, 0 = automatic (persistent CTA kernel for |Omega'| <= 256, cluster kernel above, then the
+    streamed-operand cluster kernel, generic if nothing fits), 3 = cluster kernel forced (skipped where the shape does
+    not fit it), 4 = fused tier with the NRAS cycles not chained (tier 0 chains them when the overlap is 0), 5 = the
+    streamed-operand kernel forced (tier 2c: rho and v in distributed shared memory, links and clover re-read every
+    sweep; its automatic use is for extended domains above 4096 sites, e.g. 12x8x8x8 of configs[2])."""
     cs = ragged_case() if which == "ragged" else case(which)
     cs.ctx.set_ras_tier(tier)
     try:
         cs.ctx.ras_precondition(block, s, nit, nras)
     except binding.WcrasError as e:
         cs.ctx.set_ras_tier(0)
-        if tier in (3, 4) and e.code == binding.UNSUPPORTED:
+        if tier in (3, 4, 5) and e.code == binding.UNSUPPORTED:
             pytest.skip("shape does not fit the cluster kernel")
         raise
     r = I.spinor(cs.dims, 55)
@@ -261,7 +263,7 @@ def rounded_op(cs):
     return cs.op16
 
 
-@pytest.mark.parametrize("tier", [0, 1, 4])
+@pytest.mark.parametrize("tier", [0, 1, 4, 5])
 @pytest.mark.parametrize("which,block,s,nit,nras", FP16_CASES)
 def test_ras_apply_fp16_operands(which, block, s, nit, nras, tier):
     """wcras_set_operand_precision(16) (reading R1): K_RAS of the operator with fp16-rounded
@@ -273,7 +275,7 @@ def test_ras_apply_fp16_operands(which, block, s, nit, nras, tier):
         try:
             cs.ctx.ras_precondition(block, s, nit, nras)
         except binding.WcrasError as e:
-            if tier == 4 and e.code == binding.UNSUPPORTED:
+            if tier in (4, 5) and e.code == binding.UNSUPPORTED:
                 pytest.skip("shape does not fit the fused tier")
             raise
         r32 = I.spinor(cs.dims, 57).astype(np.complex64).astype(np.complex128)
