@@ -128,6 +128,14 @@ int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev);
  * (default 1000 / 50).  use_ras = 0 runs the inner solver without preconditioner ("No prec." column of Table 1). */
 int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int outer_maxit, int use_ras);
 
+/* Convergence of the inner fp32 BiCGStab is decided on the device (a flag set by the last block of the update kernels;
+ * every kernel of an iteration returns at once when it is set), so the host need not wait for an iteration before it
+ * enqueues the next one (the inner solver runs on the GPU; only scalars cross to the host).  iterations =
+ * how many inner iterations are enqueued ahead of the host's look at the scalars (default 1): 0 = every iteration is
+ * checked before the next one is enqueued; n <= 3 = the host looks at iteration j - n while iteration j is enqueued, at
+ * the price of up to n no-op iterations after convergence.  Results are identical for every value. */
+int wcras_set_lookahead(wcras_ctx* ctx, int iterations);
+
 /* Per-kernel-class CUDA-event timing inside wcras_solve (fills ms_dslash / ms_blocksolve / ms_blas). */
 int wcras_set_timing(wcras_ctx* ctx, int enable);
 

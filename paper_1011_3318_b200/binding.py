@@ -17,7 +17,7 @@ OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, 
 
 EXPORTS = [
     "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_ras_precondition", "wcras_set_ras_tier", "wcras_set_operand_precision", "wcras_set_schwarz", "wcras_set_traversal",
-    "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_timing", "wcras_solve",
+    "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_lookahead", "wcras_set_timing", "wcras_solve",
     "wcras_solve_host", "wcras_solve_multi", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
 ]
 
@@ -145,6 +145,9 @@ class Context:
     def set_solver(self, inner_tol=5e-7, inner_maxit=1000, outer_maxit=50, use_ras=True):
         self._chk(self._lib.wcras_set_solver(self._h, C.c_double(inner_tol), C.c_int(inner_maxit),
                                              C.c_int(outer_maxit), C.c_int(1 if use_ras else 0)))
+
+    def set_lookahead(self, iterations):
+        self._chk(self._lib.wcras_set_lookahead(self._h, C.c_int(iterations)))
 
     def set_timing(self, enable):
         self._chk(self._lib.wcras_set_timing(self._h, C.c_int(1 if enable else 0)))

@@ -55,6 +55,8 @@ int wcras_destroy(wcras_ctx* ctx) {
     if (ctx->dm16) { cudaFree(ctx->dm16); cudaFree(ctx->rf_dm); }
     if (ctx->hb) cudaFree(ctx->hb);
     if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
+    if (ctx->sc_ring) cudaFreeHost(ctx->sc_ring);
+    for (cudaEvent_t e : ctx->ev_ring) if (e) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
     return WCRAS_OK;
@@ -149,6 +151,13 @@ int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int oute
     ctx->inner_maxit = inner_maxit;
     ctx->outer_maxit = outer_maxit;
     ctx->use_ras = use_ras ? 1 : 0;
+    return WCRAS_OK;
+}
+
+int wcras_set_lookahead(wcras_ctx* ctx, int iterations) {
+    NEED(ctx, "null ctx");
+    NEED(iterations >= 0 && iterations <= 3, "set_lookahead: 0..3 iterations");
+    ctx->lookahead = iterations;
     return WCRAS_OK;
 }
 

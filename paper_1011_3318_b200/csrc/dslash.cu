@@ -54,7 +54,8 @@ __device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __r
 constexpr int FIN_CTAS = 16;
 template <int DOT>
 __global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restrict__ part, unsigned nblk, double* __restrict__ slice,
-                                                         unsigned* ticket, Scalars* sc) {
+                                                         unsigned* ticket, Scalars* sc, const int* stop) {
+    if (stop && __ldg(stop)) return;
     __shared__ double sm[3][16];
     __shared__ bool last;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -110,6 +111,9 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
     // blockDim = (sites, right-hand sides): the threads threadIdx.y = 0..nrhs-1 of a site work on the vectors of a
     // stack rstride apart and load the same links and clover term, which L1 serves after the first warp has
     // fetched them (576/nrhs + 192 bytes of DRAM traffic per site and right-hand side)
+    // the inner solver has converged: this launch was enqueued ahead of the host's check.  Read-only path (L1 per SM):
+    // a plain load by every warp of the grid would serialise on one L2 sector
+    if (g.stop && __ldg(g.stop)) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (ztile > 0 && i < g.V) {
         // Large lattices: visit the sites in the order (x, y, z within a tile of ztile planes, t, z tile) instead of
@@ -246,7 +250,8 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
     TimedRegion tr(ctx, sizeof(T) == 4 ? TC_DSLASH : TC_DSLASH64);
     const int V = ctx->geom.V, nr = ctx->nrhs;
     const size_t rstride = (size_t)VecOf<T>::CHUNKS * V;
-    // 64-thread CTAs with the full register budget (165 registers fp32, 252 fp64): the compiler then keeps all
+    // 64-thread CTAs with the full register budget (fp32: __launch_bounds__(64, 6) = at most 168 registers so that six CTAs
+    // stay resident per SM, 252 fp64): the compiler then keeps all
     // loads of a site in flight at once, which is what an HBM latency-bound stencil needs -- measured on B200 at
     // 32^4: 130 us (fp32) / 292 us (fp64) against 147 / 330 us at 96 / 186 registers with 128-thread CTAs.
     // fp32, nrhs 2..4: one launch covers the whole stack with CTAs of 32 sites x nrhs right-hand sides; otherwise
@@ -281,16 +286,16 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
 #define WC_DSL(TH, BLOCK, INP, OUTP, BM, DV, POFF)                                                                                    \
     {                                                                                                                              \
         if (dot == 1)                                                                                                              \
-            dslash_kernel<T, false, TH, 1, 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, (sizeof(T) == 4 ? 384 / TH : 1), 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
         else if (dot == 2)                                                                                                         \
-            dslash_kernel<T, false, TH, 1, 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, (sizeof(T) == 4 ? 384 / TH : 1), 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
         else if (b_minus)                                                                                                          \
-            dslash_kernel<T, true, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP,  \
+            dslash_kernel<T, true, TH, (sizeof(T) == 4 ? 384 / TH : 1), 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP,  \
                                                                               BM, nullptr, nullptr, 0, 0, rstride, ztile);         \
         else                                                                                                                       \
-            dslash_kernel<T, false, TH, 1, 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+            dslash_kernel<T, false, TH, (sizeof(T) == 4 ? 384 / TH : 1), 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, nullptr, nullptr, 0, 0, rstride, ztile);   \
         ctx->launches++;                                                                                                           \
     }
@@ -303,8 +308,8 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
             WC_DSL(64, dim3(64, 1), in + r * rstride, out + r * rstride, b_minus + r * rstride, dotv + r * rstride, r * grid)
     }
 #undef WC_DSL
-    if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc);
-    if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc);
+    if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
+    if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
     if (dot) ctx->launches++;
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;
     WC_CHECK_LAUNCH();

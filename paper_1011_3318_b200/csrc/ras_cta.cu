@@ -66,6 +66,7 @@ ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __res
                float4* rho_out, int nrhs, size_t rstride, size_t hstride) {
     // nrhs > 1 (wcras_solve_multi): every vector argument is a stack of nrhs vectors rstride apart (halo buffers:
     // hstride); the right-hand sides of a domain are solved one after the other with the operands loaded once
+    if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     float4* hbuf = smem;            // [8][3][nsp]

@@ -140,6 +140,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                  const float4* __restrict__ r_lat, const float4* __restrict__ r_dm, const float4* __restrict__ hb_in,
                  float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out, float4* __restrict__ rho_dm,
                  const int4* __restrict__ dom_org, const unsigned* __restrict__ dom_bc) {
+    if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     const Cta16Smem lay = cta16_smem(nsp, nface, stage_halo);

@@ -86,6 +86,7 @@ ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float
     // Chained cycles (overlap 0; same scheme as ras_cta.cu, reading A3): hb_in != nullptr: r is rho_fin of the
     // previous cycle and the hops of the previous v that cross the domain boundary are subtracted from it (halo slots
     // filled by the neighbouring domains); hb_out: halo scatter of this cycle's v; rho_out: rho_fin of this cycle.
+    if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;                 // threads per CTA = slots per chunk
     float4* hbuf = smem;                    // [8][3][nsp]
@@ -457,7 +458,7 @@ static FusedGeom make_fused_geom(const wcras_ctx* ctx, const int b[4], const int
         fg.wrap[mu] = ext[mu] == ctx->geom.L[mu];
         if (*ok) { fg.ns *= fg.sb[mu]; fg.C *= fg.c[mu]; }
     }
-    fg.V = ctx->geom.V; fg.s = s; fg.niter = niter;
+    fg.V = ctx->geom.V; fg.s = s; fg.niter = niter; fg.stop = nullptr;
     fg.nsp = (fg.ns + 31) / 32 * 32;
     return fg;
 }

@@ -10,14 +10,15 @@
 //     site, the C CTAs of a domain form a cluster; the grid is persistent (as many clusters as the chip holds).
 //   * On chip, for the whole block solve: the MR vectors rho and v of the sub-block in shared memory (192 B per site,
 //     120 KB at 625 sites), q in registers.  q = D_Omega' rho is a GATHER: every site reads the full spinors of its (up to) 8
-//     neighbours from shared memory -- ld.shared::cluster through a precomputed cluster-space address, so a neighbour in
-//     another CTA of the cluster (DSMEM) costs the same instruction as a local one; a neighbour outside Omega' is
-//     skipped (Dirichlet), wrap-around inside Omega' (ext = L) is kept.
+//     neighbours from shared memory through a precomputed address: plain ld.shared for a neighbour in the same CTA,
+//     ld.shared::cluster (DSMEM) for one in another CTA of the cluster; a neighbour outside Omega' is skipped
+//     (Dirichlet), wrap-around inside Omega' (ext = L) is kept.
 //   * Links and clover are NOT resident: every sweep streams a domain-major operand record per site from global memory
 //     -- 4 forward links, the 4 backward links U_mu(x-mu) already gathered to the site, the clover blocks; fp32 (58
 //     16-byte chunks) or, in 16-bit operand mode (reading R1), fp16 (33 chunks = 528 B).  The N_dominv sweeps of a
-//     domain re-read the same record, which L2 serves (a cluster's record is 5.3 MB in fp16 at 10^4 sites); the record
-//     of the cluster's NEXT domain is pulled from HBM into L2 meanwhile (cp.async.bulk.prefetch.L2).
+//     domain re-read the same record, which L2 serves (a cluster's record is 5.3 MB in fp16 at 10^4 sites).  Pulling
+//     the NEXT domain's record into L2 meanwhile (cp.async.bulk.prefetch.L2) was measured 5 % slower: it halves the L2
+//     room of the records in use (ncu: L2 hit rate 51 %), so it is not done.
 //   * Domain-local dots: warp shuffle -> one float4 per warp pushed to every CTA of the cluster -> fixed-order sum.
 //     Two cluster barriers per MR iteration (dots; rho updated before the neighbours read it again).
 // Roofline: L2 operand stream, 528 (fp16) or 928 (fp32) B per site and sweep, against ~1.7 k fp32 instructions per site
@@ -190,6 +191,7 @@ __global__ void __launch_bounds__(STREAM_MAX_SITES, 1)
 ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ rec, const float4* __restrict__ r,
                   float4* __restrict__ vout, int accum) {
     typedef Rec<OP> R;
+    if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp;
     float4* rho = smem;             // [6][nsp] MR residual: read by the neighbours, also across the cluster
@@ -209,7 +211,7 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
     for (int mu = 0; mu < 4; mu++)
         if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
     // cluster-space address of chunk 0 of rho at the neighbour in direction (mu, +) [index 2mu] and (mu, -) [2mu+1]
-    unsigned nbr[8];
+    unsigned nbr[8], remote = 0;
     {
         const unsigned base = st_smem_u32(rho);
         int lstride = 1, cstride = 1;
@@ -236,8 +238,10 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
                         else ok = false;
                     }
                 }
+                // a neighbour in this CTA is read through the plain shared window (ld.shared at full shared-memory
+                // bandwidth); only a neighbour in another CTA goes through the cluster window (DSMEM, ~20 B/clk per SM)
                 unsigned a = base + (unsigned)kd * 16u;
-                if (CL) a = st_mapa(a, (unsigned)rk);
+                if (CL && rk != (int)rank) { a = st_mapa(a, (unsigned)rk); remote |= 1u << (2 * mu + sg); }
                 nbr[2 * mu + sg] = ok ? a : ST_NONE;
             }
             lstride *= fg.sb[mu];
@@ -256,10 +260,6 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
             rho[c * nsp + k] = active ? r[(size_t)c * V + gi] : make_float4(0.f, 0.f, 0.f, 0.f);
             vv[c * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
-        if (dom + nclus < nd && k < R::ALL)
-            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rec + (((size_t)(dom + nclus) * fg.C + rank) * R::ALL + k) * stride),
-                         "r"(chunk_bytes)
-                         : "memory");
         st_barrier<CL>();  // every CTA of the cluster has its rho in place
 
         for (int it = 0; it < fg.niter; it++) {
@@ -272,7 +272,8 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
         float u[18], sn[24];                                                                                  \
         load_rec<R::LINK, 18>(myrec + (size_t)(MU * R::LINK) * stride, stride, (const OP*)nullptr, u);        \
         _Pragma("unroll") for (int c = 0; c < 6; c++) {                                                       \
-            const float4 t = CL ? ld_cluster_f4(nbr[2 * MU] + c * chunk_bytes) : ld_shared_f4(nbr[2 * MU] + c * chunk_bytes); \
+            const float4 t = CL && (remote >> (2 * MU) & 1u) ? ld_cluster_f4(nbr[2 * MU] + c * chunk_bytes)       \
+                                                         : ld_shared_f4(nbr[2 * MU] + c * chunk_bytes);      \
             sn[4 * c] = t.x; sn[4 * c + 1] = t.y; sn[4 * c + 2] = t.z; sn[4 * c + 3] = t.w;                   \
         }                                                                                                     \
         hop_fwd<float, MU>(u, sn, hop);                                                                       \
@@ -281,7 +282,8 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
         float u[18], sn[24];                                                                                  \
         load_rec<R::LINK, 18>(myrec + (size_t)((4 + MU) * R::LINK) * stride, stride, (const OP*)nullptr, u);  \
         _Pragma("unroll") for (int c = 0; c < 6; c++) {                                                       \
-            const float4 t = CL ? ld_cluster_f4(nbr[2 * MU + 1] + c * chunk_bytes) : ld_shared_f4(nbr[2 * MU + 1] + c * chunk_bytes); \
+            const float4 t = CL && (remote >> (2 * MU + 1) & 1u) ? ld_cluster_f4(nbr[2 * MU + 1] + c * chunk_bytes)       \
+                                                         : ld_shared_f4(nbr[2 * MU + 1] + c * chunk_bytes);      \
             sn[4 * c] = t.x; sn[4 * c + 1] = t.y; sn[4 * c + 2] = t.z; sn[4 * c + 3] = t.w;                   \
         }                                                                                                     \
         hop_bwd<float, MU>(u, sn, hop);                                                                       \
@@ -452,7 +454,7 @@ int ras_stream_prepare(wcras_ctx* ctx, const int b[4], const int ext[4], int s, 
         fg.wrap[mu] = ext[mu] == ctx->geom.L[mu];
         fg.ns *= fg.sb[mu]; fg.C *= fg.c[mu];
     }
-    fg.V = ctx->geom.V; fg.s = s; fg.niter = niter; fg.pdir = -1;
+    fg.V = ctx->geom.V; fg.s = s; fg.niter = niter; fg.pdir = -1; fg.stop = nullptr;
     fg.nsp = (fg.ns + 31) / 32 * 32;
     int dev = 0, smem_max = 0;
     cudaGetDevice(&dev);

@@ -36,7 +36,7 @@ template <typename T> __device__ __forceinline__ cpx<T> ld_scalar(const double* 
 // writes x instead of updating it, and the shadow residual rt is b itself ("first iteration").
 template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __restrict__ b, Scalars* sc, double* partials,
-                                                      unsigned* ticket) {
+                                                      unsigned* ticket, double tol, double tiny, int half) {
     constexpr int N = Cx<Vec>::N;
     double acc[1] = {0};
     GRID_STRIDE(k, n) {
@@ -50,6 +50,9 @@ __global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __res
         sc->bb = tot[0]; sc->rr = tot[0]; sc->ss = tot[0];
         sc->rho[0] = tot[0]; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
         sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+        sc->thresh = tol * tol; sc->tiny = tiny; sc->half = half;
+        sc->flag = tot[0] > 0 ? 0 : 1;  // zero right-hand side: x = 0 is the solution
+        sc->it_done = 0; sc->half_exit = 0;
     }
 }
 
@@ -74,6 +77,7 @@ __global__ void __launch_bounds__(RED_THREADS) k_restart(size_t n, const Vec* __
         sc->rr = tot[0];
         sc->rho[0] = tot[0]; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
         sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+        sc->flag = 0;
     }
 }
 
@@ -82,6 +86,7 @@ template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* __restrict__ r, Vec* __restrict__ p,
                                                           const Vec* __restrict__ v, const Scalars* __restrict__ sc, int first) {
     constexpr int N = Cx<Vec>::N;
+    if (sc->flag) return;
     if (first) {  // p = v = 0 before the first iteration: p = r (= b), nothing else is read
         GRID_STRIDE(k, n) p[k] = r[k];
         return;
@@ -105,6 +110,7 @@ template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_update_s(size_t n, const Vec* __restrict__ r, const Vec* __restrict__ v,
                                                           Vec* __restrict__ s, Scalars* sc, double* partials, unsigned* ticket) {
     constexpr int N = Cx<Vec>::N;
+    if (sc->flag) return;
     const cpx<T> alpha = ld_scalar<T>(sc->alpha);
     double acc[1] = {0};
     GRID_STRIDE(k, n) {
@@ -118,7 +124,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_s(size_t n, const Vec* _
         s[k] = pack(rc, (Vec*)nullptr);
     }
     double tot[1];
-    if (grid_reduce<1>(acc, partials, ticket, tot)) sc->ss = tot[0];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) {
+        sc->ss = tot[0];
+        // half-step exit (van der Vorst): |s| already below the tolerance -> x += alpha ph finishes the solve; every kernel
+        // up to k_update_xr of this iteration sees flag = 2 and returns, k_update_xr applies the half step
+        if (sc->half && tot[0] < sc->thresh * sc->bb) sc->flag = 2;
+    }
 }
 
 // x += alpha ph + omega sh; r = s - omega t; rho_old = rho; rho = <rt,r>; rr = |r|^2
@@ -128,8 +139,30 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_xr(size_t n, Vec* __rest
                                                            const Vec* __restrict__ t, const Vec* __restrict__ rt, Vec* __restrict__ r,
                                                            Scalars* sc, double* partials, unsigned* ticket, int first) {
     constexpr int N = Cx<Vec>::N;
+    const int fl = sc->flag;  // every block reads it before the last block (the only writer) can change it
+    if (fl == 1 || fl == 3) return;
     const cpx<T> alpha = ld_scalar<T>(sc->alpha), omega = ld_scalar<T>(sc->omega);
     double acc[3] = {0, 0, 0};
+    if (fl == 2) {  // half-step exit: x += alpha ph, the residual is s
+        GRID_STRIDE(k, n) {
+            cpx<T> xc[N], pc[N];
+            if (first) {
+#pragma unroll
+                for (int j = 0; j < N; j++) xc[j] = {0, 0};
+            } else {
+                unpack<T>(x[k], xc);
+            }
+            unpack<T>(ph[k], pc);
+#pragma unroll
+            for (int j = 0; j < N; j++) xc[j] = xc[j] + alpha * pc[j];
+            x[k] = pack(xc, (Vec*)nullptr);
+        }
+        double tot[3];
+        if (grid_reduce<3>(acc, partials, ticket, tot)) {
+            sc->rr = sc->ss; sc->it_done += 1; sc->half_exit = 1; sc->flag = 1;
+        }
+        return;
+    }
     GRID_STRIDE(k, n) {
         cpx<T> xc[N], pc[N], hc[N], sc_[N], tc[N], rc[N];
         if (first) {  // x = 0 before the first iteration
@@ -155,27 +188,12 @@ __global__ void __launch_bounds__(RED_THREADS) k_update_xr(size_t n, Vec* __rest
         sc->rho_old[0] = sc->rho[0]; sc->rho_old[1] = sc->rho[1];
         sc->rho[0] = tot[0]; sc->rho[1] = tot[1];
         sc->rr = tot[2];
-    }
-}
-
-// x += alpha ph (half-step exit)
-template <typename T, typename Vec>
-__global__ void __launch_bounds__(RED_THREADS) k_axpy_alpha(size_t n, Vec* __restrict__ x, const Vec* __restrict__ ph,
-                                                            const Scalars* __restrict__ sc, int first) {
-    constexpr int N = Cx<Vec>::N;
-    const cpx<T> alpha = ld_scalar<T>(sc->alpha);
-    GRID_STRIDE(k, n) {
-        cpx<T> xc[N], pc[N];
-        if (first) {
-#pragma unroll
-            for (int j = 0; j < N; j++) xc[j] = {0, 0};
-        } else {
-            unpack<T>(x[k], xc);
-        }
-        unpack<T>(ph[k], pc);
-#pragma unroll
-        for (int j = 0; j < N; j++) xc[j] = xc[j] + alpha * pc[j];
-        x[k] = pack(xc, (Vec*)nullptr);
+        sc->it_done += 1;
+        // convergence and breakdown are decided here, on the device: NaN or |rho|, |omega| underflow (reading Q13) stop the
+        // iteration with flag 3 (the host restarts once), |r| below the tolerance with flag 1
+        if (!(tot[2] == tot[2])) sc->flag = 3;
+        else if (tot[2] < sc->thresh * sc->bb) sc->flag = 1;
+        else if (hypot(tot[0], tot[1]) < sc->tiny * sc->bb || hypot(sc->omega[0], sc->omega[1]) < sc->tiny) sc->flag = 3;
     }
 }
 
@@ -257,89 +275,120 @@ template <typename T> struct Work {
 
 // BiCGStab driver.  K(in,out) applies the preconditioner (ignored when k_identity).  status: 0 converged,
 // WCRAS_NOT_CONVERGED, WCRAS_BREAKDOWN, or a CUDA error.
+//
+// Convergence, the half-step exit and breakdown are decided on the device (Scalars::flag, set by the last block of
+// k_update_s / k_update_xr); every kernel of an iteration returns at once when the flag is set.  The host therefore
+// does not wait for an iteration before it enqueues the next one: after every iteration it enqueues a copy of the scalars
+// into a pinned ring slot and looks at the slot of `lookahead` iterations ago.  With lookahead 0 (the outer fp64 solver,
+// whose preconditioner is a whole inner solve) every iteration is checked before the next one is enqueued, and the
+// half-step flag is read before K(s).
 template <typename T, typename KFunc>
 static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b, typename VecOf<T>::type* x, double tol, int maxit,
                     bool half_exit, bool k_identity, KFunc K, int* iters, double* relres) {
     typedef typename VecOf<T>::type Vec;
+    constexpr int RING = 4;
     const size_t n = w.n;
     double* part = ctx->partials;
     unsigned* tk = ctx->ticket;
+    const int la = sizeof(T) == 4 ? (ctx->lookahead < RING - 1 ? ctx->lookahead : RING - 1) : 0;
+    const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH((k_init<T, Vec>), n, b, w.sc, part, tk);
+        LAUNCH((k_init<T, Vec>), n, b, w.sc, part, tk, tol, tiny, half_exit ? 1 : 0);
     }
-    if (int rc = read_scalars(ctx, w.sc)) return rc;
-    const double bb = ctx->sc_host->bb;
     *iters = 0;
     *relres = 0;
-    if (bb == 0.0) {
-        WC_CUDA(cudaMemsetAsync(x, 0, sizeof(Vec) * n, ctx->stream));
-        return WCRAS_OK;
-    }
     Vec* ph = k_identity ? w.p : w.ph;
     Vec* sh = k_identity ? w.s : w.sh;
-    const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
     const Vec* rt = b;    // shadow residual = initial residual = b (x0 = 0); a restart switches to the copy in w.rt
     const Vec* rcur = b;  // residual read by the first iteration; w.r from the first r = s - omega t on
-    bool x_written = false;
-    int it = 0, restarts = 0, status = WCRAS_NOT_CONVERGED;
-    double rr = bb, best = bb;
+    // the fp32 launches of this solver carry the device flag so that those enqueued past convergence are no-ops
+    struct StopScope {
+        wcras_ctx* c;
+        bool on;
+        StopScope(wcras_ctx* cc, const int* f, bool o) : c(cc), on(o) { if (on) { c->geom.stop = f; c->fused.stop = f; } }
+        ~StopScope() { if (on) { c->geom.stop = nullptr; c->fused.stop = nullptr; } }
+    } stop_scope(ctx, &w.sc->flag, sizeof(T) == 4);
+    const int c0[4] = {ctx->dv32, ctx->dv64, ctx->block_dv, ctx->ras_applies};
+    bool x_written = false, first = true;
+    int enq = 0, restarts = 0, status = WCRAS_NOT_CONVERGED;
+    double best = -1;
     int it_best = 0;
-    while (it < maxit) {
+    for (;;) {
+        bool stop = false;
+        while (!stop && enq < maxit) {
+            if (la > 0 && enq > la) {  // look at the iteration enqueued `la` iterations ago
+                const int j = enq - la - 1;
+                WC_CUDA(cudaEventSynchronize(ctx->ev_ring[j % RING]));
+                const Scalars& h = ctx->sc_ring[j % RING];
+                if (h.flag) break;
+                // stagnation guard (fp32 inner solver at the end of its accuracy): no new minimum of |r| for 10 iterations
+                if (best < 0 || h.rr < best) { best = h.rr; it_best = j; }
+                else if (j - it_best >= 10) break;
+            }
+            {
+                TimedRegion tr(ctx, TC_BLAS);
+                LAUNCH((k_update_p<T, Vec>), n, rcur, w.p, w.v, w.sc, first ? 1 : 0);
+            }
+            if (!k_identity) if (int rc = K(w.p, ph)) return rc;
+            if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
+            {
+                TimedRegion tr(ctx, TC_BLAS);
+                LAUNCH((k_update_s<T, Vec>), n, rcur, w.v, w.s, w.sc, part, tk);
+            }
+            bool half_now = false;
+            if (la == 0 && half_exit) {  // the second half costs a whole inner solve: read the flag first
+                if (int rc = read_scalars(ctx, w.sc)) return rc;
+                half_now = ctx->sc_host->flag == 2;
+            }
+            if (!half_now) {
+                if (!k_identity) if (int rc = K(w.s, sh)) return rc;
+                if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
+            }
+            {
+                TimedRegion tr(ctx, TC_BLAS);
+                LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, rt, w.r, w.sc, part, tk, x_written ? 0 : 1);
+            }
+            x_written = true;
+            first = false;
+            rcur = w.r;
+            WC_CUDA(cudaMemcpyAsync(&ctx->sc_ring[enq % RING], w.sc, sizeof(Scalars), cudaMemcpyDeviceToHost, ctx->stream));
+            WC_CUDA(cudaEventRecord(ctx->ev_ring[enq % RING], ctx->stream));
+            enq++;
+            if (la == 0) {
+                WC_CUDA(cudaEventSynchronize(ctx->ev_ring[(enq - 1) % RING]));
+                const Scalars& h = ctx->sc_ring[(enq - 1) % RING];
+                if (h.flag) stop = true;
+            }
+        }
+        if (int rc = read_scalars(ctx, w.sc)) return rc;  // drains the stream: the state is that of the last effective iteration
         const Scalars& h = *ctx->sc_host;
-        if (hypot(h.rho[0], h.rho[1]) < tiny * bb || (it > 0 && hypot(h.omega[0], h.omega[1]) < tiny)) {
-            if (restarts++) { status = WCRAS_BREAKDOWN; break; }
+        if (h.flag == 1) { status = WCRAS_OK; break; }
+        if (h.flag == 3 && restarts == 0 && h.rr == h.rr && enq < maxit) {  // breakdown: one restart with rt = r (reading Q13)
+            restarts++;
             TimedRegion tr(ctx, TC_BLAS);
             LAUNCH((k_restart<T, Vec>), n, rcur, w.rt, w.p, w.v, w.sc, part, tk);
             rt = w.rt;
+            first = false;  // p = v = 0 are stored now: the general p update applies
+            enq = h.it_done;
+            best = -1;
+            continue;
         }
-        {
-            TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_p<T, Vec>), n, rcur, w.p, w.v, w.sc, (it == 0 && restarts == 0) ? 1 : 0);
-        }
-        if (!k_identity) if (int rc = K(w.p, ph)) return rc;
-        if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
-        {
-            TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_s<T, Vec>), n, rcur, w.v, w.s, w.sc, part, tk);
-        }
-        // The half-step test costs a host round trip.  In the inner fp32 solver it is only made once the residual is
-        // within a factor 1e3 of the target (half an iteration does not gain three digits there; skipping the test can
-        // only waste half an iteration, never accept an unconverged x).  The outer solver always tests: its half step is
-        // a whole inner solve.
-        if (half_exit && (sizeof(T) == 8 || std::sqrt(rr / bb) < 1e3 * tol)) {
-            if (int rc = read_scalars(ctx, w.sc)) return rc;
-            if (std::sqrt(ctx->sc_host->ss / bb) < tol) {
-                TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_axpy_alpha<T, Vec>), n, x, ph, w.sc, x_written ? 0 : 1);
-                x_written = true;
-                rr = ctx->sc_host->ss;
-                it++;
-                status = WCRAS_OK;
-                break;
-            }
-        }
-        if (!k_identity) if (int rc = K(w.s, sh)) return rc;
-        if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
-        {
-            TimedRegion tr(ctx, TC_BLAS);
-            LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, rt, w.r, w.sc, part, tk, x_written ? 0 : 1);
-            x_written = true;
-            rcur = w.r;
-        }
-        it++;
-        if (int rc = read_scalars(ctx, w.sc)) return rc;
-        rr = ctx->sc_host->rr;
-        if (!(rr == rr)) { status = WCRAS_BREAKDOWN; break; }  // NaN
-        if (std::sqrt(rr / bb) < tol) { status = WCRAS_OK; break; }
-        // stagnation guard (fp32 inner solver at the end of its accuracy): no new minimum of |r| for 10 iterations
-        if (rr < best) { best = rr; it_best = it; }
-        else if (it - it_best >= 10) break;
+        status = h.flag == 3 ? WCRAS_BREAKDOWN : WCRAS_NOT_CONVERGED;
+        break;
     }
-    if (!x_written) WC_CUDA(cudaMemsetAsync(x, 0, sizeof(Vec) * n, ctx->stream));  // left before the first update of x
+    const Scalars& h = *ctx->sc_host;
+    if (!x_written || h.it_done == 0) WC_CUDA(cudaMemsetAsync(x, 0, sizeof(Vec) * n, ctx->stream));  // no update of x happened
+    if (la > 0 && enq > 0) {
+        // iterations enqueued past convergence were no-ops: count the effective ones (every inner iteration adds the same
+        // number of D and K applications, a half-step exit half of them)
+        const long eff = 2L * h.it_done - (h.half_exit ? 1 : 0), all = 2L * enq;
+        int* cnt[4] = {&ctx->dv32, &ctx->dv64, &ctx->block_dv, &ctx->ras_applies};
+        for (int k = 0; k < 4; k++) *cnt[k] = c0[k] + (int)((long)(*cnt[k] - c0[k]) * eff / all);
+    }
     WC_CHECK_LAUNCH();
-    *iters = it;
-    *relres = std::sqrt(rr / bb);
+    *iters = h.it_done;
+    *relres = h.bb > 0 ? std::sqrt(h.rr / h.bb) : 0.0;
     return status;
 }
 
@@ -360,6 +409,8 @@ int ensure_workspace(wcras_ctx* ctx) {
         if (alloc_dev(ctx, (void**)&ctx->ticket, sizeof(unsigned))) return WCRAS_CUDA_ERROR;
         WC_CUDA(cudaMemsetAsync(ctx->ticket, 0, sizeof(unsigned), ctx->stream));
         WC_CUDA(cudaMallocHost((void**)&ctx->sc_host, sizeof(Scalars)));
+        WC_CUDA(cudaMallocHost((void**)&ctx->sc_ring, sizeof(Scalars) * 4));
+        for (int k = 0; k < 4; k++) WC_CUDA(cudaEventCreateWithFlags(&ctx->ev_ring[k], cudaEventDisableTiming));
     }
     if (ctx->ws_nrhs < ctx->nrhs) {
         WC_CUDA(cudaStreamSynchronize(ctx->stream));

@@ -22,6 +22,7 @@ namespace wc {
 struct Geom {
     int L[4];
     int V;  // number of sites (<= 2^31 / 36)
+    const int* stop = nullptr;  // device flag of the running inner solver: non-zero = converged, the launch is a no-op
 };
 
 template <typename T> struct VecOf;
@@ -113,6 +114,14 @@ struct Scalars {
     double bb;          // |b|^2
     double nrm;         // scratch norm^2 (conversion / true residual)
     double scale;       // scratch
+    // device-side convergence control (no host round trip per iteration: the inner solver does "most of
+    // arithmetics" on the GPU): every kernel of an iteration returns at once when flag != 0
+    double thresh;      // tol^2: converged when |r|^2 < thresh * |b|^2
+    double tiny;        // breakdown threshold on |rho| / |b|^2 and |omega|
+    int flag;           // 0 running, 1 converged, 2 converged at the half step (x += alpha ph pending), 3 breakdown / NaN
+    int it_done;        // completed iterations (a half-step exit counts as one)
+    int half;           // test |s| after the first half step
+    int half_exit;      // the solve ended at a half step
 };
 
 }  // namespace wc
@@ -126,6 +135,7 @@ struct FusedGeom {
     int V, s, ns, nsp, C, niter;
     int nclus;       // tier 2b: clusters (or CTAs) resident at once = persistent grid size in clusters
     int pdir;        // multiplicative Schwarz: pairing direction of the red-black domain enumeration, -1 = not colourable
+    const int* stop; // device flag of the running inner solver (see wc::Geom::stop), or nullptr
 };
 
 struct RasConfig {
@@ -196,6 +206,9 @@ struct wcras_ctx {
     wc::Scalars* sc32 = nullptr;   // device scalars of the inner solver
     wc::Scalars* sc64 = nullptr;   // device scalars of the outer solver
     wc::Scalars* sc_host = nullptr;  // pinned
+    wc::Scalars* sc_ring = nullptr;  // pinned [SC_RING]: per-iteration snapshots the host polls a few iterations late
+    cudaEvent_t ev_ring[4] = {nullptr, nullptr, nullptr, nullptr};
+    int lookahead = 1;             // inner iterations enqueued ahead of the host's convergence check (0 = check every one)
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;
     double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][blocks], slice sums, ticket
