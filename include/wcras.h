@@ -82,7 +82,11 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
  * 1 = generic global-memory tier, 2 = fused tier (WCRAS_UNSUPPORTED at the next wcras_ras_precondition if
  * the shape does not fit; extended domains of <= 256 sites use the persistent one-CTA-per-domain kernel,
  * larger ones a thread-block cluster per domain), 3 = fused tier, cluster kernel forced (for checking),
- * 4 = fused tier with the NRAS cycles NOT chained (for checking).  On the persistent-CTA kernel with overlap 0
+ * 4 = fused tier with the NRAS cycles NOT chained (for checking), 5 = the streamed-operand cluster kernel forced
+ * (tier 2c of SURVEY.md 8(a): rho and v of an extended domain in the distributed shared memory of a <= 16-CTA cluster,
+ * links and clover re-read from L2 every sweep; chosen automatically when the extended domain exceeds 4096 sites,
+ * e.g. configs[4]: 8^4 blocks with overlap 1), 6 = as 0 but, in 16-bit operand mode, the two-threads-per-site variant
+ * of the persistent kernel (ras_pair.cu; measured slower, kept for comparison).  On the persistent-CTA kernel with overlap 0
  * the cycles of Alg.1 are chained: the MR recurrence leaves rho = r - D_Omega v on every domain, so line 9,
  * r -= D v, only adds the hops of v that cross a domain boundary and no full-lattice D runs between cycles.
  * Call before wcras_ras_precondition. */

@@ -82,7 +82,7 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     NEED(ctx, "null ctx");
-    NEED(tier >= 0 && tier <= 5, "set_ras_tier: tier must be 0..5");
+    NEED(tier >= 0 && tier <= 6, "set_ras_tier: tier must be 0..6");
     ctx->tier_request = tier == 4 ? 2 : tier;
     ctx->chain_cycles = tier != 4;
     return WCRAS_OK;

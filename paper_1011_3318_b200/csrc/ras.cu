@@ -216,6 +216,10 @@ int ras_round_fields(wcras_ctx* ctx);
 int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_cta16_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_pair_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
+int ras_pair_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+int ras_pair_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_pair_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
 
 int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nras) {
     RasConfig rc;
@@ -234,11 +238,12 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     // tier request 5: force the streamed-operand cluster kernel (tier 2c); automatic: 2a/2b when Omega' fits on chip with
     // its operands, else 2c when the spinors fit a cluster, else the generic tier
     bool fused_ok = ctx->tier_request != 1 && ctx->tier_request != 5 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
-    if (!fused_ok && (ctx->tier_request == 0 || ctx->tier_request == 5) && ras_stream_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0) {
+    if (!fused_ok && (ctx->tier_request == 0 || ctx->tier_request == 5 || ctx->tier_request == 6) &&
+        ras_stream_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0) {
         fused_ok = true;
         rc.stream = true;
     }
-    if (ctx->tier_request >= 2 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
+    if (ctx->tier_request >= 2 && ctx->tier_request != 6 && !fused_ok) { snprintf(ctx->err, sizeof ctx->err, "ras_precondition: domain does not fit the fused tier"); return WCRAS_UNSUPPORTED; }
     rc.tier = (ctx->tier_request == 1 || !fused_ok) ? 1 : 2;
     if (int e = ensure_workspace(ctx)) return e;
     // 16-bit operand mode (reading R1): every path of the preconditioner sees the fp16-rounded links and clover blocks
@@ -278,7 +283,9 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         rc.cta = ctx->tier_request != 3 && ras_cta_prepare(ctx, fgeom, rc.nd) != 0;  // tier request 3: force the cluster kernel
         // 16-bit operand mode: the staged fp16 kernel takes the single-right-hand-side work of this tier (its grid size
         // and halo geometry are those of ras_cta_prepare: same CTA shape, one CTA per SM)
-        rc.cta16 = rc.cta && ctx->op_prec == 16 && ras_cta16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
+        // (tier request 6: the two-threads-per-site variant ras_pair.cu instead -- measured slower, kept for comparison)
+        rc.pair = rc.cta && ctx->op_prec == 16 && ctx->tier_request == 6 && ras_pair_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
+        rc.cta16 = rc.cta && ctx->op_prec == 16 && !rc.pair && ras_cta16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
         if (!rc.cta) ras_fused_pack(ctx, ctx->fused, rc.nd);
         if (!rc.cta) {  // halo geometry of the chained cycles on the cluster tier (buffers allocated on first use)
             int nface = 1;
@@ -321,6 +328,7 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
 static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     TimedRegion tr(ctx, TC_BLOCK);
     ctx->block_dv += ctx->ras.niter;
+    if (ctx->ras.tier == 2 && ctx->ras.pair && ctx->nrhs == 1) return ras_pair_block_solve(ctx, r, vout, accum);
     if (ctx->ras.tier == 2 && ctx->ras.cta16 && ctx->nrhs == 1) return ras_cta16_block_solve(ctx, r, vout, accum);
     if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
     const size_t rstride = (size_t)6 * ctx->geom.V;
@@ -346,10 +354,12 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
             snprintf(ctx->err, sizeof ctx->err, "multiplicative Schwarz needs overlap 0, domains of <= 256 sites and an even number of blocks in every cut direction");
             return WCRAS_UNSUPPORTED;
         }
+        if (rc.pair && ctx->nrhs == 1) return ras_pair_apply_sap(ctx, r, v);
         return rc.cta16 && ctx->nrhs == 1 ? ras_cta16_apply_sap(ctx, r, v) : ras_cta_apply_sap(ctx, r, v);
     }
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
+    if (rc.tier == 2 && rc.pair && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_pair_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cta16_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
     if (rc.tier == 2 && !rc.cta && !rc.stream && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);

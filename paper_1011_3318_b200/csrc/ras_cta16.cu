@@ -28,35 +28,6 @@
 
 namespace wc {
 
-// ---- mbarrier + bulk-copy (TMA) helpers ----
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tWC_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra WC_DONE;\n\tbra WC_WAIT;\n\tWC_DONE:\n\t}" ::"r"(bar),
-        "r"(parity)
-        : "memory");
-}
-// global -> shared bulk copy (TMA unit, SASS UBLKCP), bytes a multiple of 16, completion counted on the mbarrier
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
-                 "r"(bytes), "r"(bar)
-                 : "memory");
-}
-
-__device__ __forceinline__ void half8_to_float(const uint4& t, float* f) {
-    const __half2* h = reinterpret_cast<const __half2*>(&t);
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-        const float2 p = __half22float2(h[j]);
-        f[2 * j] = p.x; f[2 * j + 1] = p.y;
-    }
-}
-
 // pack the fp16 domain-major operand copy: one thread per (domain, local site); zero for the padding lanes
 // also fills the per-domain tables dom_org (first site of Omega', coordinates mod L) and dom_bc (block coordinates packed
 // 8 bits each), so that the block solver needs no integer division per domain

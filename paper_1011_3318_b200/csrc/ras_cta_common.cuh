@@ -2,6 +2,8 @@
 // ras_cta16.cu: fp16 operand storage staged by TMA): shared-memory half-spinor slots, asynchronous copies, the
 // domain -> site geometry of PAPER.md:45 (Omega_i, Omega'_i) and the red-black domain enumeration.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "wcras_internal.cuh"
 
 namespace wc {
@@ -74,6 +76,35 @@ __device__ __forceinline__ int launch_dom(const FusedGeom& fg, int h, int colour
         stride *= nb;
     }
     return dom + (2 * cp + ((colour + par) & 1)) * sp;
+}
+
+// ---- mbarrier + bulk-copy (TMA) helpers ----
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tWC_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra WC_DONE;\n\tbra WC_WAIT;\n\tWC_DONE:\n\t}" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy (TMA unit, SASS UBLKCP), bytes a multiple of 16, completion counted on the mbarrier
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+__device__ __forceinline__ void half8_to_float(const uint4& t, float* f) {
+    const __half2* h = reinterpret_cast<const __half2*>(&t);
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const float2 p = __half22float2(h[j]);
+        f[2 * j] = p.x; f[2 * j + 1] = p.y;
+    }
 }
 
 }  // namespace wc

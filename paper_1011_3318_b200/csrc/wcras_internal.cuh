@@ -149,6 +149,7 @@ struct RasConfig {
     int tier = 1;                 // 1 generic, 2 fused
     bool cta = false;             // fused tier, single persistent CTA per domain (ras_cta.cu)
     bool cta16 = false;           // the same with fp16 operand storage staged by TMA (ras_cta16.cu)
+    bool pair = false;            // the same with two threads per site, 16 warps per SM (ras_pair.cu)
     bool stream = false;          // fused tier 2c: rho, v in (distributed) shared memory, operands streamed (ras_stream.cu)
 };
 constexpr int FUSED_CTA_MAX_THREADS = 256;

@@ -263,7 +263,7 @@ def rounded_op(cs):
     return cs.op16
 
 
-@pytest.mark.parametrize("tier", [0, 1, 4, 5])
+@pytest.mark.parametrize("tier", [0, 1, 4, 5, 6])
 @pytest.mark.parametrize("which,block,s,nit,nras", FP16_CASES)
 def test_ras_apply_fp16_operands(which, block, s, nit, nras, tier):
     """wcras_set_operand_precision(16) (reading R1): K_RAS of the operator with fp16-rounded
@@ -275,7 +275,7 @@ def test_ras_apply_fp16_operands(which, block, s, nit, nras, tier):
         try:
             cs.ctx.ras_precondition(block, s, nit, nras)
         except binding.WcrasError as e:
-            if tier in (4, 5) and e.code == binding.UNSUPPORTED:
+            if tier in (4, 5, 6) and e.code == binding.UNSUPPORTED:
                 pytest.skip("shape does not fit the fused tier")
             raise
         r32 = I.spinor(cs.dims, 57).astype(np.complex64).astype(np.complex128)
