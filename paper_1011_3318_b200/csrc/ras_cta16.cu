@@ -344,6 +344,9 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #undef WC_GATHER
             }
             float d0 = 0.f, d1 = 0.f, d2 = 0.f;
+#ifdef WC_X2
+            x2::mr_dots(q, rho, d0, d1, d2);
+#else
 #pragma unroll
             for (int n = 0; n < 12; n++) {
                 const float qr = q[2 * n], qi = q[2 * n + 1], rr = rho[2 * n], ri = rho[2 * n + 1];
@@ -351,6 +354,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                 d1 = fmaf(qr, ri, d1); d1 = fmaf(-qi, rr, d1);
                 d2 = fmaf(qr, qr, d2); d2 = fmaf(qi, qi, d2);
             }
+#endif
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 d0 += __shfl_xor_sync(0xffffffffu, d0, o);
@@ -370,6 +374,10 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             const float inv = s2 > 0.f ? 1.f / s2 : 0.f;
             const float ar = s0 * inv, ai = s1 * inv;
             const bool upd_rho = it + 1 < fg.niter || rho_dm != nullptr;
+#ifdef WC_X2
+            if (upd_rho) x2::mr_update<true>(ar, ai, q, rho, v);
+            else x2::mr_update<false>(ar, ai, q, rho, v);
+#else
 #pragma unroll
             for (int n = 0; n < 12; n++) {
                 const float rr = rho[2 * n], ri = rho[2 * n + 1];
@@ -380,6 +388,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                     rho[2 * n + 1] = fmaf(-ar, q[2 * n + 1], ri); rho[2 * n + 1] = fmaf(-ai, q[2 * n], rho[2 * n + 1]);
                 }
             }
+#endif
         }
         WC_T(11)
         // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
