@@ -216,6 +216,9 @@ int ras_round_fields(wcras_ctx* ctx);
 int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_cta16_apply_sap(wcras_ctx* ctx, const float4* r, float4* v);
+int ras_cl16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
+int ras_cl16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
+int ras_cl16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
 int ras_pair_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f);
 int ras_pair_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum);
 int ras_pair_apply_chained(wcras_ctx* ctx, const float4* r, float4* v);
@@ -286,7 +289,9 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         // (tier request 6: the two-threads-per-site variant ras_pair.cu instead -- measured slower, kept for comparison)
         rc.pair = rc.cta && ctx->op_prec == 16 && ctx->tier_request == 6 && ras_pair_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
         rc.cta16 = rc.cta && ctx->op_prec == 16 && !rc.pair && ras_cta16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
-        if (!rc.cta) ras_fused_pack(ctx, ctx->fused, rc.nd);
+        // 16-bit operand mode on the cluster tier: fp16 operands staged by TMA (ras_cl16.cu); otherwise ras_fused.cu
+        rc.cl16 = !rc.cta && ctx->op_prec == 16 && fgeom.C > 1 && ras_cl16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
+        if (!rc.cta && !rc.cl16) ras_fused_pack(ctx, ctx->fused, rc.nd);
         if (!rc.cta) {  // halo geometry of the chained cycles on the cluster tier (buffers allocated on first use)
             int nface = 1;
             for (int mu = 0; mu < 4; mu++) nface = rc.nloc / rc.ext[mu] > nface ? rc.nloc / rc.ext[mu] : nface;
@@ -334,6 +339,7 @@ static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum
     const size_t rstride = (size_t)6 * ctx->geom.V;
     for (int k = 0; k < ctx->nrhs; k++) {  // cluster and generic tiers: one right-hand side of the stack at a time
         const int e = ctx->ras.tier == 2 ? (ctx->ras.stream ? ras_stream_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
+                                            : ctx->ras.cl16 ? ras_cl16_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
                                                             : ras_fused_block_solve(ctx, r + k * rstride, vout + k * rstride, accum))
                                          : generic_block_solve(ctx, r + k * rstride, vout + k * rstride, accum);
         if (e) return e;
@@ -362,6 +368,7 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     if (rc.tier == 2 && rc.pair && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_pair_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cta16_apply_chained(ctx, r, v);
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
+    if (rc.tier == 2 && rc.cl16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cl16_apply_chained(ctx, r, v);
     if (rc.tier == 2 && !rc.cta && !rc.stream && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];

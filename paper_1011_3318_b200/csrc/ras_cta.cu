@@ -18,6 +18,10 @@
 // Shared memory: 8 x 3 float4 x nsp half-spinor slots (96 KB at nsp = 256) + nwarps float4.
 // Roofline: HBM, (96 + 576) B per extended site in + 96 B per bulk site out (768 B/site at s = 0); the sweeps
 // cost ~1.4 k fp32 instructions per site each and must hide behind that stream.
+// This kernel sits at the 255-register limit with fp32 operands (links in registers, 36-real clover blocks unpacked from
+// shared memory): the aligned register pairs of the packed-fp32 arithmetic (site_math.cuh, WC_X2) make it spill
+// (~500 B per thread, measured 12.3 -> 17.2 ms per solve), so this translation unit keeps the scalar FFMA forms.
+#define WC_NO_F32X2
 #include "ras_cta_common.cuh"
 
 namespace wc {

@@ -23,6 +23,7 @@
 //   * Shared memory at nsp = 256: 96 KB half-spinor slots + 72 KB operands + 24 KB residual + 24 KB halo = 216 KB.
 // Roofline: HBM; algorithmic bytes per site and launch 288 operands + 96 residual in + 96 out (+ 96 rho_fin, + halo).
 #include <cuda_fp16.h>
+#include <stdlib.h>
 
 #include "ras_cta_common.cuh"
 
@@ -231,6 +232,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         const int dom = launch_dom(fg, h, colour);
         const int nxt = launch_dom(fg, has_next ? h + gridDim.x : h, colour);
         const int4 org_nxt = __ldg(dom_org + nxt);  // consumed at the earliest when the next residual is requested
+        const unsigned dom_bc_here = hb_out ? __ldg(dom_bc + dom) : 0u;  // consumed by the halo scatter after the sweeps
         const size_t gi = site_of(org);
 
         // ---- operands: links from the staged fp16 block into registers, scaled by -kappa ----
@@ -393,7 +395,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         WC_T(11)
         // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
         if (hb_out) {
-            unsigned dd = __ldg(dom_bc + dom);
+            unsigned dd = dom_bc_here;
             int dstride = 1;
             float hs[12], g[12];
 #define WC_HALO(MU)                                                                                              \
@@ -467,19 +469,39 @@ int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    int stage_halo = 1;
-    if (cta16_smem(fg.nsp, nface, 1).bytes > (size_t)smem_max) stage_halo = 0;
-    const size_t smem = cta16_smem(fg.nsp, nface, stage_halo).bytes;
-    if (smem > (size_t)smem_max) return 0;
-    if (cudaFuncSetAttribute(ras_cta16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-        cudaFuncSetAttribute(ras_cta16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
-    }
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ras_cta16_kernel<true>, fg.nsp, smem) != cudaSuccess || per_sm < 1) {
-        cudaGetLastError();
-        return 0;
+    // Halo slots staged in shared memory by a bulk copy, unless leaving them in global memory lets one more CTA live on
+    // an SM (128-site domains: 98 KB instead of 123 KB per CTA, two independent domains per SM hide each other's
+    // barriers and memory phases)
+    int stage_halo = 1, per_sm = 0;
+    size_t smem = 0;
+    {
+        int best = 0;
+        for (int sh = 1; sh >= 0; sh--) {
+            const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
+            if (b > (size_t)smem_max) continue;
+            if (cudaFuncSetAttribute(ras_cta16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess ||
+                cudaFuncSetAttribute(ras_cta16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) {
+                cudaGetLastError();
+                continue;
+            }
+            int n = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, ras_cta16_kernel<true>, fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
+            if (n > best) { best = n; stage_halo = sh; smem = b; }
+        }
+        if (const char* e = getenv("WCRAS_CTA16_STAGE_HALO")) {  // experiment switch
+            const int sh = atoi(e);
+            const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
+            if (b <= (size_t)smem_max) {
+                int n = 0;
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, ras_cta16_kernel<true>, fg.nsp, b);
+                if (n >= 1) { best = n; stage_halo = sh; smem = b; }
+            }
+        }
+        per_sm = best;
+        if (getenv("WCRAS_DEBUG")) fprintf(stderr, "cta16: nsp %d nface %d stage_halo %d smem %zu per_sm %d\n", fg.nsp, nface, stage_halo, smem, per_sm);
+        if (per_sm < 1) return 0;
+        cudaFuncSetAttribute(ras_cta16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(ras_cta16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }
     if (ctx->dm16) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm16); ctx->dm16 = nullptr; }
     if (ctx->rf_dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->rf_dm); ctx->rf_dm = nullptr; }

@@ -181,8 +181,11 @@ __device__ __forceinline__ void mr_update(float ar, float ai, const float* __res
 template <typename T, int MU, int SIGN>
 WC_HD void project(const T* __restrict__ s, T* __restrict__ h) {
 #ifdef WC_X2
-    if constexpr (sizeof(T) == 4) { x2::project<MU, SIGN>(reinterpret_cast<const float*>(s), reinterpret_cast<float*>(h)); return; }
+    if constexpr (sizeof(T) == 4) {
+        x2::project<MU, SIGN>(reinterpret_cast<const float*>(s), reinterpret_cast<float*>(h));
+    } else
 #endif
+    {
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         const T s0r = s[2 * c], s0i = s[2 * c + 1];
@@ -206,6 +209,7 @@ WC_HD void project(const T* __restrict__ s, T* __restrict__ h) {
         h[2 * c] = h0r; h[2 * c + 1] = h0i;
         h[6 + 2 * c] = h1r; h[6 + 2 * c + 1] = h1i;
     }
+    }
 }
 
 // acc += sg * (full spinor whose upper rows are g and whose rows 2,3 follow from (1 + SIGN*gamma_MU)), sg = +1 or,
@@ -213,8 +217,11 @@ WC_HD void project(const T* __restrict__ s, T* __restrict__ h) {
 template <typename T, int MU, int SIGN, int NEG>
 WC_HD void reconstruct_acc(const T* __restrict__ g, T* __restrict__ acc) {
 #ifdef WC_X2
-    if constexpr (sizeof(T) == 4) { x2::reconstruct_acc<MU, SIGN, NEG>(reinterpret_cast<const float*>(g), reinterpret_cast<float*>(acc)); return; }
+    if constexpr (sizeof(T) == 4) {
+        x2::reconstruct_acc<MU, SIGN, NEG>(reinterpret_cast<const float*>(g), reinterpret_cast<float*>(acc));
+    } else
 #endif
+    {
     const T sg = NEG ? T(-1) : T(1);
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -238,6 +245,7 @@ WC_HD void reconstruct_acc(const T* __restrict__ g, T* __restrict__ acc) {
             else          { a2[0] += sg * g0r; a2[1] += sg * g0i; a3[0] += sg * g1r; a3[1] += sg * g1i; }
         }
     }
+    }
 }
 
 template <typename T, int MU, int SIGN>
@@ -254,8 +262,11 @@ WC_HD double wc_fma(double a, double b, double c) { return fma(a, b, c); }
 template <typename T>
 WC_HD void su3_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restrict__ g) {
 #ifdef WC_X2
-    if constexpr (sizeof(T) == 4) { x2::su3_mul(reinterpret_cast<const float*>(u), reinterpret_cast<const float*>(h), reinterpret_cast<float*>(g)); return; }
+    if constexpr (sizeof(T) == 4) {
+        x2::su3_mul(reinterpret_cast<const float*>(u), reinterpret_cast<const float*>(h), reinterpret_cast<float*>(g));
+    } else
 #endif
+    {
 #pragma unroll
     for (int hs = 0; hs < 2; hs++)
 #pragma unroll
@@ -276,14 +287,18 @@ WC_HD void su3_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restri
             g[(hs * 3 + a) * 2] = re;
             g[(hs * 3 + a) * 2 + 1] = im;
         }
+    }
 }
 
 // g = U^dagger h
 template <typename T>
 WC_HD void su3_adj_mul(const T* __restrict__ u, const T* __restrict__ h, T* __restrict__ g) {
 #ifdef WC_X2
-    if constexpr (sizeof(T) == 4) { x2::su3_adj_mul(reinterpret_cast<const float*>(u), reinterpret_cast<const float*>(h), reinterpret_cast<float*>(g)); return; }
+    if constexpr (sizeof(T) == 4) {
+        x2::su3_adj_mul(reinterpret_cast<const float*>(u), reinterpret_cast<const float*>(h), reinterpret_cast<float*>(g));
+    } else
 #endif
+    {
 #pragma unroll
     for (int hs = 0; hs < 2; hs++)
 #pragma unroll
@@ -305,6 +320,7 @@ WC_HD void su3_adj_mul(const T* __restrict__ u, const T* __restrict__ h, T* __re
             g[(hs * 3 + a) * 2] = re;
             g[(hs * 3 + a) * 2 + 1] = im;
         }
+    }
 }
 
 // hop += (1 - gamma_MU) U psi_fwd      (forward hop; u = U_MU(x), sf = psi(x+MU))
@@ -329,8 +345,11 @@ WC_HD void hop_bwd(const T* __restrict__ u, const T* __restrict__ sb, T* __restr
 template <typename T>
 WC_HD void herm6_mul(const T* __restrict__ b, const T* __restrict__ x, T* __restrict__ out) {
 #ifdef WC_X2
-    if constexpr (sizeof(T) == 4) { x2::herm6_mul(reinterpret_cast<const float*>(b), reinterpret_cast<const float*>(x), reinterpret_cast<float*>(out)); return; }
+    if constexpr (sizeof(T) == 4) {
+        x2::herm6_mul(reinterpret_cast<const float*>(b), reinterpret_cast<const float*>(x), reinterpret_cast<float*>(out));
+    } else
 #endif
+    {
 #pragma unroll
     for (int i = 0; i < 6; i++) {
         T re = b[i] * x[2 * i], im = b[i] * x[2 * i + 1];
@@ -352,6 +371,7 @@ WC_HD void herm6_mul(const T* __restrict__ b, const T* __restrict__ x, T* __rest
         }
         out[2 * i] = re;
         out[2 * i + 1] = im;
+    }
     }
 }
 

@@ -150,6 +150,7 @@ struct RasConfig {
     bool cta = false;             // fused tier, single persistent CTA per domain (ras_cta.cu)
     bool cta16 = false;           // the same with fp16 operand storage staged by TMA (ras_cta16.cu)
     bool pair = false;            // the same with two threads per site, 16 warps per SM (ras_pair.cu)
+    bool cl16 = false;            // cluster tier with fp16 operand storage staged by TMA (ras_cl16.cu)
     bool stream = false;          // fused tier 2c: rho, v in (distributed) shared memory, operands streamed (ras_stream.cu)
 };
 constexpr int FUSED_CTA_MAX_THREADS = 256;
@@ -188,6 +189,7 @@ struct wcras_ctx {
     float4* r16c = nullptr;
     int dslash_rounded = 0;        // the next fp32 dslash applies the rounded operator (r -= D~ v inside K_RAS)
     int cta_grid = 0;              // its persistent grid size
+    int cl16_nclus = 0;            // ras_cl16: clusters resident at once
     float4* hb = nullptr;          // halo buffers of the chained K_RAS cycles: [2][nd][8][3][nface]
     int nface = 0;
     int hb_nrhs = 0;               // stack depth the halo buffers are allocated for
