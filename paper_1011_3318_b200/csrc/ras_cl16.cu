@@ -110,7 +110,7 @@ __global__ void pack_cl16_kernel(FusedGeom fg, int nd, Fields<float> f, uint4* _
 }
 
 struct Cl16Smem {  // offsets in float4 units
-    int hbuf, opbuf, rstage, red, bars;
+    int hbuf, opbuf, rstage, red, bars, org;
     size_t bytes;
 };
 __host__ __device__ inline Cl16Smem cl16_smem(int nsp, int C) {
@@ -120,7 +120,8 @@ __host__ __device__ inline Cl16Smem cl16_smem(int nsp, int C) {
     s.rstage = s.opbuf + 18 * nsp;
     s.red = s.rstage + 6 * nsp;
     s.bars = s.red + C * (nsp / 32);
-    s.bytes = (size_t)(s.bars + 2) * 16;
+    s.org = s.bars + 2;
+    s.bytes = (size_t)(s.org + 2) * 16;
     return s;
 }
 
@@ -138,6 +139,7 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
     const uint4* opbuf = reinterpret_cast<const uint4*>(smem + lay.opbuf);  // [18][nsp] fp16 operands of the current domain
     float4* rstage = smem + lay.rstage;                                    // [6][nsp] residual of the current / next domain
     float4* red = smem + lay.red;                                          // [C][nwarps] dot partials of the whole cluster
+    int4* org_s = reinterpret_cast<int4*>(smem + lay.org);                 // [2] first site of the current / next domain (table dom_org)
     const unsigned bar_links = cta_smem_u32(smem + lay.bars), bar_clov = bar_links + 8, bar_vec = bar_links + 16;
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const unsigned rank = cl16_rank();
@@ -202,6 +204,10 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             cstride *= fg.c[mu];
         }
     }
+    // coordinates in Omega' and face indices travel through the block solve as one / two registers
+    const unsigned ec_pk = (unsigned)ec[0] | (unsigned)ec[1] << 8 | (unsigned)ec[2] << 16 | (unsigned)ec[3] << 24;
+    const unsigned fidx_lo = (unsigned)fidx[0] | (unsigned)fidx[1] << 16, fidx_hi = (unsigned)fidx[2] | (unsigned)fidx[3] << 16;
+#define WC_FIDX(MU) ((int)((((MU) < 2 ? fidx_lo : fidx_hi) >> (16 * ((MU) & 1))) & 0xffffu))
 #pragma unroll
     for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (k == 0) {
@@ -236,7 +242,8 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         }
     };
     auto site_of = [&](const int4& org) -> size_t {
-        int x0 = org.x + ec[0], x1 = org.y + ec[1], x2 = org.z + ec[2], x3 = org.w + ec[3];
+        int x0 = org.x + (int)(ec_pk & 255u), x1 = org.y + (int)((ec_pk >> 8) & 255u), x2 = org.z + (int)((ec_pk >> 16) & 255u),
+            x3 = org.w + (int)(ec_pk >> 24);
         if (x0 >= fg.L[0]) x0 -= fg.L[0];
         if (x1 >= fg.L[1]) x1 -= fg.L[1];
         if (x2 >= fg.L[2]) x2 -= fg.L[2];
@@ -252,12 +259,12 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         cp_async_commit();
     };
 
-    int4 org = make_int4(0, 0, 0, 0);
     if (cl < nd) {
-        org = dom_org[cl];
         request_links_vec(cl);
         request_clover(cl);
-        if (!src_dm) request_r_lat(org);
+        if (k == 0) cp_async16(org_s, dom_org + cl);  // committed with (or as) the first group below, waited for at the loop top
+        if (!src_dm) request_r_lat(dom_org[cl]);
+        else cp_async_commit();
     }
 
     float U[72];
@@ -267,9 +274,9 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         const unsigned par = (unsigned)j & 1u;
         const bool has_next = dom + ncl < nd;
         const int nxt = has_next ? dom + ncl : dom;
-        const int4 org_nxt = __ldg(dom_org + nxt);
         const unsigned dom_bc_here = hb_out ? __ldg(dom_bc + dom) : 0u;
-        const size_t gi = site_of(org);
+        int4 org_nxt = make_int4(0, 0, 0, 0);
+        if (!src_dm) org_nxt = __ldg(dom_org + nxt);  // lattice-layout source: the next residual column is requested below
 
         // ---- operands: links from the staged fp16 block into registers, scaled by -kappa ----
         mbar_wait(bar_links, par);
@@ -282,8 +289,8 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         }
         // ---- projection P_Omega' r: the staged residual column of this thread ----
         float rho[24], v[24];
+        cp_async_wait();  // own residual column (lattice-layout source); thread 0: the origin of this domain in org_s
         if (src_dm) mbar_wait(bar_vec, par);
-        else cp_async_wait();
 #pragma unroll
         for (int c = 0; c < 6; c++) {
             float4 t = rstage[c * nsp + k];
@@ -299,7 +306,7 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
 #define WC_CROSS_LOAD(SL)                                                                         \
     {                                                                                             \
         const bool rcv = active && dst[(SL) ^ 1] == 0xffffffffu;                                  \
-        const float4* q4 = hin + (size_t)(SL) * 3 * nface + fidx[(SL) >> 1];                      \
+        const float4* q4 = hin + (size_t)(SL) * 3 * nface + WC_FIDX((SL) >> 1);                      \
         _Pragma("unroll") for (int jj = 0; jj < 3; jj++) {                                        \
             float4 t = make_float4(0.f, 0.f, 0.f, 0.f);                                           \
             if (rcv) t = __ldcs(q4 + (size_t)jj * nface);                                         \
@@ -351,10 +358,11 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             cl_wait();
             // Every thread of the cluster is past its staging reads of this domain (links, residual: before the first
             // barrier; clover: before this barrier of the last sweep): thread 0 requests the next domain's data.
-            if (has_next) {
+            if (has_next && warp == 0) {
                 if (it == 0) {
                     request_links_vec(nxt);
-                    if (k == 32) prefetch_l2_bulk(dm16 + (((size_t)nxt * C + rank) * 18 + 9) * nsp, half_bytes);
+                    if (k == 1) prefetch_l2_bulk(dm16 + (((size_t)nxt * C + rank) * 18 + 9) * nsp, half_bytes);
+                    if (k == 0) { cp_async16(org_s + ((j + 1) & 1), dom_org + nxt); cp_async_commit(); }
                 }
                 if (it + 1 == fg.niter) request_clover(nxt);
             }
@@ -436,13 +444,13 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         dd >>= 8;                                                                                                \
         if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the domain at -mu */            \
             const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                              \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + WC_FIDX(MU);                             \
             project<float, MU, -1>(v, hs);                                                                       \
             for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(hs[4 * jj], hs[4 * jj + 1], hs[4 * jj + 2], hs[4 * jj + 3]); \
         }                                                                                                        \
         if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the domain at +mu */      \
             const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                          \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + WC_FIDX(MU);                         \
             project<float, MU, +1>(v, hs);                                                                       \
             su3_adj_mul<float>(U + 18 * MU, hs, g);                                                              \
             for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(g[4 * jj], g[4 * jj + 1], g[4 * jj + 2], g[4 * jj + 3]); \
@@ -459,6 +467,7 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             for (int c = 0; c < 6; c++) o[(size_t)c * nsp] = make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]);
         }
         if (bulk) {
+            const size_t gi = site_of(org_s[j & 1]);  // visible since the first barrier of this domain
             if (phi_in) {
                 // phi += v as a fire-and-forget vector reduction (phi_in == phi_out; one writer per site)
 #pragma unroll
@@ -472,7 +481,6 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
-        org = org_nxt;
     }
 }
 

@@ -87,7 +87,7 @@ __global__ void round_half_kernel(size_t n, const float* __restrict__ in, float*
 #endif
 
 struct Cta16Smem {  // offsets in float4 units
-    int hbuf, opbuf, rstage, hstage, red, bars;
+    int hbuf, opbuf, rstage, hstage, red, bars, org;
     size_t bytes;
 };
 __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_halo) {
@@ -98,7 +98,8 @@ __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_ha
     s.hstage = s.rstage + 6 * nsp;
     s.red = s.hstage + (stage_halo ? 24 * nface : 0);
     s.bars = s.red + 8;
-    s.bytes = (size_t)(s.bars + 2) * 16;
+    s.org = s.bars + 2;
+    s.bytes = (size_t)(s.org + 2) * 16;
     return s;
 }
 
@@ -106,7 +107,9 @@ __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_ha
 //   r_lat   residual source in the lattice layout (cycle 0 / first visit), or nullptr
 //   r_dm    residual source domain-major [nd][6][nsp] (rho_fin of the previous cycle), or nullptr
 //   rho_dm  rho_fin of this cycle, domain-major, or nullptr (then the last MR residual update is skipped, Q12)
-template <bool CHAIN>
+//   NSP     threads per CTA = padded sites per domain as a compile-time constant (256: every slot, operand and staging
+//           offset becomes an immediate), or 0 = taken from fg.nsp at run time
+template <bool CHAIN, int NSP>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
 ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, float mkappa, const uint4* __restrict__ dm16,
                  const float4* __restrict__ r_lat, const float4* __restrict__ r_dm, const float4* __restrict__ hb_in,
@@ -114,13 +117,14 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                  const int4* __restrict__ dom_org, const unsigned* __restrict__ dom_bc) {
     if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
-    const int nsp = fg.nsp;
+    const int nsp = NSP ? NSP : fg.nsp;
     const Cta16Smem lay = cta16_smem(nsp, nface, stage_halo);
     float4* hbuf = smem + lay.hbuf;                                       // [8][3][nsp] half-spinor slots
     const uint4* opbuf = reinterpret_cast<const uint4*>(smem + lay.opbuf);  // [18][nsp] fp16 operands of the current domain
     float4* rstage = smem + lay.rstage;                                   // [6][nsp] residual of the current / next domain
     const float4* hstage = smem + lay.hstage;                             // [8][3][nface] halo slots (stage_halo)
     float4* red = smem + lay.red;                                         // [nwarps]
+    int4* org_s = reinterpret_cast<int4*>(smem + lay.org);                // [2] first site of the current / next domain (table dom_org)
     const unsigned bar_links = cta_smem_u32(smem + lay.bars), bar_clov = bar_links + 8, bar_vec = bar_links + 16;
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const bool active = k < fg.ns;
@@ -158,8 +162,13 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             lstride *= e;
         }
     }
+    // local coordinates and face indices (all < 256) travel through the block solve as one register each
+    const unsigned lc_pk = (unsigned)lc[0] | (unsigned)lc[1] << 8 | (unsigned)lc[2] << 16 | (unsigned)lc[3] << 24;
+    const unsigned fidx_pk = (unsigned)fidx[0] | (unsigned)fidx[1] << 8 | (unsigned)fidx[2] << 16 | (unsigned)fidx[3] << 24;
+#define WC_FIDX(MU) ((int)((fidx_pk >> (8 * (MU))) & 255u))
 #pragma unroll
     for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (k < FUSED_CTA_MAX_THREADS / 32) red[k] = make_float4(0.f, 0.f, 0.f, 0.f);  // warps that do not exist contribute zero
     if (k == 0) {
         mbar_init(bar_links, 1);
         mbar_init(bar_clov, 1);
@@ -194,7 +203,8 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
     };
     // global site index of this thread's site in the domain whose Omega' starts at org (no division: table dom_org)
     auto site_of = [&](const int4& org) -> size_t {
-        int x0 = org.x + lc[0], x1 = org.y + lc[1], x2 = org.z + lc[2], x3 = org.w + lc[3];
+        int x0 = org.x + (int)(lc_pk & 255u), x1 = org.y + (int)((lc_pk >> 8) & 255u), x2 = org.z + (int)((lc_pk >> 16) & 255u),
+            x3 = org.w + (int)(lc_pk >> 24);
         if (x0 >= fg.L[0]) x0 -= fg.L[0];
         if (x1 >= fg.L[1]) x1 -= fg.L[1];
         if (x2 >= fg.L[2]) x2 -= fg.L[2];
@@ -210,13 +220,13 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         cp_async_commit();
     };
 
-    int4 org = make_int4(0, 0, 0, 0);
     if ((int)blockIdx.x < ndl) {
         const int dom0 = launch_dom(fg, blockIdx.x, colour);
-        org = dom_org[dom0];
         request_links_vec(dom0);
         request_clover(dom0);
-        if (!src_dm) request_r_lat(org);
+        if (k == 0) cp_async16(org_s, dom_org + dom0);  // committed with (or as) the first group below, waited for at the loop top
+        if (!src_dm) request_r_lat(dom_org[dom0]);
+        else cp_async_commit();
     }
 
 #ifdef WC_CTA16_PROFILE
@@ -231,10 +241,9 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         const bool has_next = h + (int)gridDim.x < ndl;
         const int dom = launch_dom(fg, h, colour);
         const int nxt = launch_dom(fg, has_next ? h + gridDim.x : h, colour);
-        const int4 org_nxt = __ldg(dom_org + nxt);  // consumed at the earliest when the next residual is requested
         const unsigned dom_bc_here = hb_out ? __ldg(dom_bc + dom) : 0u;  // consumed by the halo scatter after the sweeps
-        const size_t gi = site_of(org);
-
+        int4 org_nxt = make_int4(0, 0, 0, 0);
+        if (!src_dm) org_nxt = __ldg(dom_org + nxt);  // lattice-layout source: the next residual column is requested below
         // ---- operands: links from the staged fp16 block into registers, scaled by -kappa ----
         mbar_wait(bar_links, par);
         WC_T(1)
@@ -248,12 +257,8 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         // ---- projection P_Omega' r: the staged residual column of this thread ----
         float rho[24], v[24];
         WC_T(2)
-        if (src_dm) {
-            if (vec_bytes) mbar_wait(bar_vec, par);
-        } else {
-            cp_async_wait();
-            if (CHAIN && vec_bytes) mbar_wait(bar_vec, par);
-        }
+        cp_async_wait();  // own residual column (lattice-layout source); thread 0: the origin of this domain in org_s
+        if (vec_bytes) mbar_wait(bar_vec, par);
         WC_T(3)
 #pragma unroll
         for (int c = 0; c < 6; c++) {
@@ -272,7 +277,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #define WC_CROSS_LOAD(SL)                                                                         \
     {                                                                                             \
         const bool rcv = active && dst[(SL) ^ 1] == 0xffffffffu;                                  \
-        const float4* q4 = hin + (size_t)(SL) * 3 * nface + fidx[(SL) >> 1];                      \
+        const float4* q4 = hin + (size_t)(SL) * 3 * nface + WC_FIDX((SL) >> 1);                      \
         _Pragma("unroll") for (int jj = 0; jj < 3; jj++) {                                        \
             float4 t = make_float4(0.f, 0.f, 0.f, 0.f);                                           \
             if (rcv) t = q4[(size_t)jj * nface];                                                  \
@@ -327,10 +332,11 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             WC_T(9)
             // Every thread is past its staging reads of this domain (links, residual, halo: before the first barrier;
             // clover: before this barrier of the last sweep): thread 0 requests the next domain's data.
-            if (has_next) {
+            if (has_next && warp == 0) {
                 if (it == 0) {
                     request_links_vec(nxt);
-                    if (k == 32) prefetch_l2_bulk(dm16 + ((size_t)nxt * 18 + 9) * nsp, half_bytes);
+                    if (k == 1) prefetch_l2_bulk(dm16 + ((size_t)nxt * 18 + 9) * nsp, half_bytes);
+                    if (k == 0) { cp_async16(org_s + ((j + 1) & 1), dom_org + nxt); cp_async_commit(); }
                 }
                 if (it + 1 == fg.niter) request_clover(nxt);
             }
@@ -367,8 +373,10 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             WC_T(10)
             __syncthreads();
             WC_T(9)
+            // fixed-order sum over the zero-padded table of FUSED_CTA_MAX_THREADS / 32 warp partials, independent loads
             float s0 = 0.f, s1 = 0.f, s2 = 0.f;
-            for (int n = 0; n < nwarps; n++) {
+#pragma unroll
+            for (int n = 0; n < FUSED_CTA_MAX_THREADS / 32; n++) {
                 const float4 p = red[n];
                 s0 += p.x; s1 += p.y; s2 += p.z;
             }
@@ -404,13 +412,13 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         dd >>= 8;                                                                                                \
         if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the domain at -mu */            \
             const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + fidx[MU];                              \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + WC_FIDX(MU);                             \
             project<float, MU, -1>(v, hs);                                                                       \
             for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(hs[4 * jj], hs[4 * jj + 1], hs[4 * jj + 2], hs[4 * jj + 3]); \
         }                                                                                                        \
         if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the domain at +mu */      \
             const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + fidx[MU];                          \
+            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + WC_FIDX(MU);                         \
             project<float, MU, +1>(v, hs);                                                                       \
             su3_adj_mul<float>(U + 18 * MU, hs, g);                                                              \
             for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(g[4 * jj], g[4 * jj + 1], g[4 * jj + 2], g[4 * jj + 3]); \
@@ -427,6 +435,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             for (int c = 0; c < 6; c++) o[(size_t)c * nsp] = make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]);
         }
         if (bulk) {
+            const size_t gi = site_of(org_s[j & 1]);  // visible since the first barrier of this domain
             if (phi_in) {
                 // phi += v as a fire-and-forget vector reduction (phi_in == phi_out; one writer per site)
 #pragma unroll
@@ -440,7 +449,6 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
-        org = org_nxt;
     }
 #ifdef WC_CTA16_PROFILE
     if (k == 0 && blockIdx.x == 0)
@@ -453,7 +461,10 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 // ---- host side ----
 typedef void (*cta16_kernel_t)(FusedGeom, int, int, int, int, float, const uint4*, const float4*, const float4*, const float4*, float4*,
                                const float4*, float4*, float4*, const int4*, const unsigned*);
-static cta16_kernel_t cta16_kernel(bool chain) { return chain ? ras_cta16_kernel<true> : ras_cta16_kernel<false>; }
+static cta16_kernel_t cta16_kernel(bool chain, int nsp) {
+    if (nsp == 256) return chain ? ras_cta16_kernel<true, 256> : ras_cta16_kernel<false, 256>;
+    return chain ? ras_cta16_kernel<true, 0> : ras_cta16_kernel<false, 0>;
+}
 
 int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu
 
@@ -479,13 +490,13 @@ int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<
         for (int sh = 1; sh >= 0; sh--) {
             const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
             if (b > (size_t)smem_max) continue;
-            if (cudaFuncSetAttribute(ras_cta16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess ||
-                cudaFuncSetAttribute(ras_cta16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) {
+            if (cudaFuncSetAttribute(cta16_kernel(false, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess ||
+                cudaFuncSetAttribute(cta16_kernel(true, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) {
                 cudaGetLastError();
                 continue;
             }
             int n = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, ras_cta16_kernel<true>, fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg.nsp), fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
             if (n > best) { best = n; stage_halo = sh; smem = b; }
         }
         if (const char* e = getenv("WCRAS_CTA16_STAGE_HALO")) {  // experiment switch
@@ -493,15 +504,15 @@ int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<
             const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
             if (b <= (size_t)smem_max) {
                 int n = 0;
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, ras_cta16_kernel<true>, fg.nsp, b);
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg.nsp), fg.nsp, b);
                 if (n >= 1) { best = n; stage_halo = sh; smem = b; }
             }
         }
         per_sm = best;
         if (getenv("WCRAS_DEBUG")) fprintf(stderr, "cta16: nsp %d nface %d stage_halo %d smem %zu per_sm %d\n", fg.nsp, nface, stage_halo, smem, per_sm);
         if (per_sm < 1) return 0;
-        cudaFuncSetAttribute(ras_cta16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(ras_cta16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(cta16_kernel(false, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(cta16_kernel(true, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }
     if (ctx->dm16) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm16); ctx->dm16 = nullptr; }
     if (ctx->rf_dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->rf_dm); ctx->rf_dm = nullptr; }
@@ -547,7 +558,7 @@ int ras_round_fields(wcras_ctx* ctx) {
 
 int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
-    cta16_kernel(false)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ctx->ras.nd, -1, ctx->nface, ctx->stage_halo,
+    cta16_kernel(false, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ctx->ras.nd, -1, ctx->nface, ctx->stage_halo,
                                                                                 -(float)ctx->kappa, ctx->dm16, r, nullptr, nullptr, nullptr,
                                                                                 accum ? vout : nullptr, vout, nullptr, ctx->dom_org, ctx->dom_bc);
     ctx->launches++;
@@ -571,11 +582,11 @@ int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
         TimedRegion tr(ctx, TC_BLOCK);
         ctx->block_dv += ctx->ras.niter;
         if (j == 0)
-            cta16_kernel(false)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
+            cta16_kernel(false, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
                 fg, nd, -1, nface, ctx->stage_halo, mk, ctx->dm16, r, nullptr, nullptr, last ? nullptr : hb[0], nullptr, v, last ? nullptr : rf,
                 ctx->dom_org, ctx->dom_bc);
         else
-            cta16_kernel(true)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
+            cta16_kernel(true, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
                 fg, nd, -1, nface, ctx->stage_halo, mk, ctx->dm16, nullptr, rf, hb[(j - 1) & 1], last ? nullptr : hb[j & 1], v, v,
                 last ? nullptr : rf, ctx->dom_org, ctx->dom_bc);
         ctx->launches++;
@@ -603,10 +614,10 @@ int ras_cta16_apply_sap(wcras_ctx* ctx, const float4* r, float4* v) {
         float4* rho_out = last_visit ? nullptr : rf;
         float4* halo_out = last_step ? nullptr : hb;
         if (step == 0)
-            cta16_kernel(false)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm,
+            cta16_kernel(false, fg.nsp)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm,
                                                                                nullptr, halo_out, nullptr, v, rho_out, ctx->dom_org, ctx->dom_bc);
         else
-            cta16_kernel(true)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm, hb,
+            cta16_kernel(true, fg.nsp)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm, hb,
                                                                               halo_out, first_visit ? nullptr : v, v, rho_out, ctx->dom_org,
                                                                               ctx->dom_bc);
         ctx->launches++;
