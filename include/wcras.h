@@ -167,20 +167,27 @@ int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, d
 typedef struct {
     int domain[4];      /* block shape; all zero = no preconditioner */
     int overlap_s, block_iters, nras;
+    int schwarz;        /* 0 = additive (RAS, the paper's method), 1 = multiplicative (SAP; nras = red-black cycles) */
+    int operand_bits;   /* block-solver operand storage, 32 or 16 (wcras_set_operand_precision); 0 in the no-preconditioner row */
     int status;         /* status of the timed solve (WCRAS_OK, NOT_CONVERGED, BREAKDOWN) or WCRAS_UNSUPPORTED */
     int inner_iters, ras_applies;
     double ms;          /* device time of the timed solve */
     double rel_resid_true;
 } wcras_tune_row;
 
-/* The paper's parameter survey ("we survey the best parameters for NRAS and N_dominv ... we find the
- * best parameter", and :83-85 on the trade-off), run on this lattice and GPU: solves D phi = eta to `tol` once
- * untimed and once timed for every candidate (overlap 0; block shapes of <= 256 sites with extents 2/4/8 that
- * divide the lattice, plus 8x4x4x4 and 8x8x4x4; (N_dominv, NRAS) in {(2,2),(2,3),(2,4),(3,2),(3,3),(4,1),(4,2),(4,3),(5,3)} -- (5,3) is the paper's best point;
- * and the unpreconditioned solver), at most max_rows candidates.  The fastest converged candidate is left
- * configured (wcras_ras_precondition + use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.
- * table_host (may be NULL) receives the rows tried, *nrows their number.  eta_dev: device, canonical fp64.
- * Uses the workspace of wcras_solve plus one scratch solution vector. */
+/* The paper's parameter survey ("we survey the best parameters for NRAS and N_dominv ... NRAS = 1-10 and
+ * N_dominv = 1-20 ... for d = 0, 2, 4", and :83-85 on the trade-off), run on this lattice and GPU: solves D phi = eta to
+ * `tol` once untimed and once timed for every candidate, at most max_rows candidates, in this order:
+ *   row 0      the unpreconditioned solver;
+ *   stage 1    additive Schwarz at overlap 0: block shapes of 64..256 sites with extents 2/4/8 that divide the lattice, plus
+ *              8x4x4x4, 8x8x4x4 and 8^4, each at (N_dominv, NRAS) in {(2,3),(2,2),(2,4),(3,2),(3,3),(4,1),(4,2),(4,3),(5,3)}
+ *              ((5,3) is the paper's best point), with the operand precision the context is set to;
+ *   stage 2    around the fastest row so far: the rectangle N_dominv 1..8 x NRAS 1..5 on its shape; overlap s = 1, 2
+ *              (the paper's d = 2, 4) and multiplicative Schwarz on the three fastest shapes; the other operand precision.
+ * The fastest converged candidate is left configured (wcras_ras_precondition, wcras_set_schwarz, wcras_set_operand_precision,
+ * use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.  table_host (may be NULL, room for max_rows rows)
+ * receives the rows tried, *nrows their number.  On a CUDA error the previous configuration is put back.
+ * eta_dev: device, canonical fp64.  Uses the workspace of wcras_solve plus one scratch solution vector. */
 int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int max_rows, wcras_tune_row* best,
                        wcras_tune_row* table_host, int* nrows);
 

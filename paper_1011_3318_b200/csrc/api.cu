@@ -1,6 +1,7 @@
 // api.cu -- the extern "C" boundary declared in include/wcras.h: argument checks and marshalling only.
 #include <new>
 
+#include <algorithm>
 #include "wcras_internal.cuh"
 
 using namespace wc;
@@ -139,6 +140,7 @@ int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev) {
     NEED(r_dev && v_dev && r_dev != v_dev, "ras_apply: null or aliased buffers");
     NEED(ctx->ras.set, "ras_apply: call wcras_ras_precondition first");
     if (int rc = ensure_io(ctx)) return rc;
+    if (int rc = ensure_workspace(ctx)) return rc;  // the unchained cycles use work vectors (re-made after a failed growth)
     if (int rc = to_internal(ctx, 32, r_dev, ctx->io_a)) return rc;
     if (int rc = ras_apply(ctx, (const float4*)ctx->io_a, (float4*)ctx->io_b)) return rc;
     return from_internal(ctx, 32, ctx->io_b, v_dev);
@@ -209,14 +211,53 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
     NEED(eta_dev && best && tol > 0 && max_rows >= 1, "ras_autotune: bad arguments");
     if (int rc = ensure_io(ctx)) return rc;
     const int* L = ctx->geom.L;
-    std::vector<wcras_tune_row> rows;
-    auto add = [&](int b0, int b1, int b2, int b3, int it, int nras) {
-        wcras_tune_row r = {};
-        r.domain[0] = b0; r.domain[1] = b1; r.domain[2] = b2; r.domain[3] = b3;
-        r.block_iters = it; r.nras = nras;
-        rows.push_back(r);
+    // what the caller had configured, put back if the survey dies on a CUDA error
+    const RasConfig prev = ctx->ras;
+    const int prev_use = ctx->use_ras, prev_schwarz = ctx->schwarz, prev_bits = ctx->op_prec;
+    auto restore = [&]() {
+        ctx->use_ras = prev_use; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits;
+        if (prev.set) ras_configure(ctx, prev.b, prev.s, prev.niter, prev.nras);
     };
-    add(0, 0, 0, 0, 0, 0);  // no preconditioner
+    std::vector<wcras_tune_row> rows;
+    double* phi = (double*)ctx->io_b;
+    int ibest = -1;
+    // run one candidate (untimed, then timed solve) and append its row; returns WCRAS_CUDA_ERROR or WCRAS_OK
+    auto run = [&](const int b[4], int s, int it, int nras, int sap, int bits) -> int {
+        if ((int)rows.size() >= max_rows) return WCRAS_OK;
+        for (const wcras_tune_row& o : rows)  // already tried
+            if (o.domain[0] == b[0] && o.domain[1] == b[1] && o.domain[2] == b[2] && o.domain[3] == b[3] && o.overlap_s == s &&
+                o.block_iters == it && o.nras == nras && o.schwarz == sap && (it == 0 || o.operand_bits == bits)) return WCRAS_OK;
+        wcras_tune_row r = {};
+        for (int mu = 0; mu < 4; mu++) r.domain[mu] = b[mu];
+        r.overlap_s = s; r.block_iters = it; r.nras = nras; r.schwarz = sap; r.operand_bits = it ? bits : 0;
+        if (it == 0) {
+            ctx->use_ras = 0;
+        } else {
+            ctx->op_prec = bits;
+            ctx->schwarz = sap;
+            const int rc = ras_configure(ctx, b, s, it, nras);
+            if (rc == WCRAS_CUDA_ERROR) return rc;
+            if (rc) { r.status = WCRAS_UNSUPPORTED; rows.push_back(r); return WCRAS_OK; }
+            ctx->use_ras = 1;
+        }
+        wcras_info info = {};
+        int rc = WCRAS_OK;
+        for (int pass = 0; pass < 2; pass++) {  // pass 0 = warm-up
+            rc = solve(ctx, eta_dev, phi, tol, &info);
+            if (rc == WCRAS_CUDA_ERROR) return rc;
+            if (rc == WCRAS_UNSUPPORTED) break;  // e.g. multiplicative Schwarz on a shape it cannot colour
+        }
+        r.status = rc; r.ms = info.ms_total; r.inner_iters = info.inner_iters; r.ras_applies = info.ras_applies;
+        r.rel_resid_true = info.rel_resid_true;
+        rows.push_back(r);
+        if (rc == WCRAS_OK && (ibest < 0 || r.ms < rows[ibest].ms)) ibest = (int)rows.size() - 1;
+        return WCRAS_OK;
+    };
+#define WC_RUN(...) do { if (run(__VA_ARGS__) == WCRAS_CUDA_ERROR) { restore(); return WCRAS_CUDA_ERROR; } } while (0)
+    const int none[4] = {0, 0, 0, 0};
+    const int bits0 = prev_bits;
+    // ---- stage 0: no preconditioner; stage 1: block shapes x (N_dominv, NRAS) at overlap 0, additive ----
+    WC_RUN(none, 0, 0, 0, 0, 0);
     static const int par[9][2] = {{2, 3}, {2, 2}, {2, 4}, {3, 2}, {3, 3}, {4, 1}, {4, 2}, {4, 3}, {5, 3}};
     std::vector<std::vector<int>> shapes;
     for (int b3 : {8, 4, 2}) for (int b2 : {8, 4, 2}) for (int b1 : {8, 4, 2}) for (int b0 : {8, 4, 2}) {
@@ -225,46 +266,58 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
         bool ok = true;
         for (int mu = 0; mu < 4; mu++) { ns *= b[mu]; ok = ok && L[mu] % b[mu] == 0; }
         // persistent tier (<= 256 sites, not tiny) with x >= y >= z >= t to skip permutations of the same cut,
-        // and the two cluster-tier shapes BASELINE.json:configs name
+        // and the cluster-tier shapes BASELINE.json:configs name
         const bool sorted = b0 >= b1 && b1 >= b2 && b2 >= b3;
-        const bool named = (b0 == 8 && b1 == 4 && b2 == 4 && b3 == 4) || (b0 == 8 && b1 == 8 && b2 == 4 && b3 == 4);
+        const bool named = (b0 == 8 && b1 == 4 && b2 == 4 && b3 == 4) || (b0 == 8 && b1 == 8 && b2 == 4 && b3 == 4) ||
+                           (b0 == 8 && b1 == 8 && b2 == 8 && b3 == 8);
         if (ok && ((sorted && ns <= 256 && ns >= 64) || named)) shapes.push_back({b0, b1, b2, b3});
     }
     for (int p = 0; p < 9; p++)
-        for (const auto& sh : shapes) add(sh[0], sh[1], sh[2], sh[3], par[p][0], par[p][1]);
-    if ((int)rows.size() > max_rows) rows.resize(max_rows);
-    double* phi = (double*)ctx->io_b;
-    int ibest = -1;
-    for (size_t k = 0; k < rows.size(); k++) {
-        wcras_tune_row& r = rows[k];
-        if (r.block_iters == 0) {
-            ctx->use_ras = 0;
-        } else {
-            const int rc = ras_configure(ctx, r.domain, 0, r.block_iters, r.nras);
-            if (rc == WCRAS_CUDA_ERROR) return rc;
-            if (rc) { r.status = WCRAS_UNSUPPORTED; r.ms = 0; continue; }
-            ctx->use_ras = 1;
+        for (const auto& sh : shapes) WC_RUN(sh.data(), 0, par[p][0], par[p][1], 0, bits0);
+    // ---- stage 2: around the best additive point: the paper's other axes (N_RAS = 1-10, N_dominv = 1-20,
+    // d = 0, 2, 4).  The (N_dominv, NRAS) rectangle 1..8 x 1..5 on the best shape, overlap s = 1, 2 (d = 2s) on the best
+    // three shapes, multiplicative Schwarz, and the other operand precision ----
+    if (ibest > 0) {
+        std::vector<int> order;  // converged additive rows, fastest first
+        for (size_t k = 1; k < rows.size(); k++) if (rows[k].status == WCRAS_OK) order.push_back((int)k);
+        std::sort(order.begin(), order.end(), [&](int a, int c) { return rows[a].ms < rows[c].ms; });
+        const wcras_tune_row top = rows[order[0]];
+        for (int it = 1; it <= 8; it++)
+            for (int nras = 1; nras <= 5; nras++) WC_RUN(top.domain, 0, it, nras, 0, bits0);
+        std::vector<std::vector<int>> seen;
+        for (size_t k = 0; k < order.size() && seen.size() < 3; k++) {
+            const wcras_tune_row& r = rows[order[k]];
+            std::vector<int> sh(r.domain, r.domain + 4);
+            if (std::find(seen.begin(), seen.end(), sh) != seen.end()) continue;
+            seen.push_back(sh);
+            const int it = r.block_iters, nras = r.nras;
+            for (int s = 1; s <= 2; s++) {
+                bool fits = true;
+                for (int mu = 0; mu < 4; mu++) fits = fits && (sh[mu] == L[mu] || sh[mu] + 2 * s <= L[mu]);
+                if (!fits) continue;
+                WC_RUN(sh.data(), s, it, nras, 0, bits0);
+                if (nras > 1) WC_RUN(sh.data(), s, it + 1, nras - 1, 0, bits0);
+            }
+            WC_RUN(sh.data(), 0, it, nras, 1, bits0);                      // SAP: nras = number of red-black cycles
+            WC_RUN(sh.data(), 0, it + 1, nras > 1 ? nras - 1 : 1, 1, bits0);
         }
-        wcras_info info;
-        int rc = WCRAS_OK;
-        for (int pass = 0; pass < 2; pass++) {  // pass 0 = warm-up
-            rc = solve(ctx, eta_dev, phi, tol, &info);
-            if (rc == WCRAS_CUDA_ERROR) return rc;
-        }
-        r.status = rc; r.ms = info.ms_total; r.inner_iters = info.inner_iters; r.ras_applies = info.ras_applies;
-        r.rel_resid_true = info.rel_resid_true;
-        if (rc == WCRAS_OK && (ibest < 0 || r.ms < rows[ibest].ms)) ibest = (int)k;
+        const wcras_tune_row now = rows[ibest];
+        if (now.block_iters) WC_RUN(now.domain, now.overlap_s, now.block_iters, now.nras, now.schwarz, bits0 == 16 ? 32 : 16);
     }
+#undef WC_RUN
     if (table_host) for (size_t k = 0; k < rows.size(); k++) table_host[k] = rows[k];
     if (nrows) *nrows = (int)rows.size();
     if (ibest < 0) {
+        restore();
         snprintf(ctx->err, sizeof ctx->err, "ras_autotune: no candidate converged");
         return WCRAS_NOT_CONVERGED;
     }
     *best = rows[ibest];
-    if (best->block_iters == 0) { ctx->use_ras = 0; return WCRAS_OK; }
+    if (best->block_iters == 0) { ctx->use_ras = 0; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits; return WCRAS_OK; }
     ctx->use_ras = 1;
-    return ras_configure(ctx, best->domain, 0, best->block_iters, best->nras);
+    ctx->schwarz = best->schwarz;
+    ctx->op_prec = best->operand_bits;
+    return ras_configure(ctx, best->domain, best->overlap_s, best->block_iters, best->nras);
 }
 
 int wcras_export_clover(wcras_ctx* ctx, double* out_dev) {
@@ -283,9 +336,9 @@ int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch
     // deterministic non-trivial scratch input: reuse the fp32 link array bytes as a spinor-sized pattern
     WC_CUDA(cudaMemcpyAsync(ctx->w32[0], ctx->g32a, sizeof(float4) * 6 * V, cudaMemcpyDeviceToDevice, ctx->stream));
     WC_CUDA(cudaMemcpyAsync(ctx->w64[0], ctx->g64, sizeof(double2) * 12 * V, cudaMemcpyDeviceToDevice, ctx->stream));
-    cudaEvent_t e0, e1;
-    WC_CUDA(cudaEventCreate(&e0));
-    WC_CUDA(cudaEventCreate(&e1));
+    EventPair ev;
+    WC_CUDA(ev.create());
+    const cudaEvent_t e0 = ev.a, e1 = ev.b;
     int rc = WCRAS_OK;
     for (int pass = 0; pass < 2 && !rc; pass++) {  // pass 0 = warm-up
         const int n = pass == 0 ? 3 : reps;
@@ -300,8 +353,6 @@ int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch
     }
     float t = 0;
     WC_CUDA(cudaEventElapsedTime(&t, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     *ms_per_launch = t / reps;
     return rc;
 }

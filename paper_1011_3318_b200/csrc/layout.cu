@@ -1,11 +1,21 @@
 // layout.cu -- setup step A0: canonical -> internal SoA reordering of links and spinors, and the fp64
 // construction of the clover term (clover_build.cuh).  One-time cost in wcras_create, not on the timed path.
+#include <stdlib.h>
 #include "clover_build.cuh"
 #include "wcras_internal.cuh"
 
 namespace wc {
 
 int alloc_dev(wcras_ctx* ctx, void** p, size_t bytes) {
+    *p = nullptr;
+    // fault injection for the out-of-memory paths (tests/test_gpu_parity.py::test_workspace_growth_failure): allocations of
+    // at least WCRAS_FAIL_ALLOC_ABOVE bytes fail as cudaMalloc would
+    if (const char* e = getenv("WCRAS_FAIL_ALLOC_ABOVE")) {
+        if (*e && bytes >= (size_t)strtoull(e, nullptr, 10)) {
+            snprintf(ctx->err, sizeof ctx->err, "alloc_dev: out of memory (%zu bytes; injected)", bytes);
+            return WCRAS_CUDA_ERROR;
+        }
+    }
     WC_CUDA(cudaMalloc(p, bytes));
     ctx->owned.push_back(*p);
     return WCRAS_OK;

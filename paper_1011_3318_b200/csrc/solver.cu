@@ -413,16 +413,26 @@ int ensure_workspace(wcras_ctx* ctx) {
         for (int k = 0; k < 4; k++) WC_CUDA(cudaEventCreateWithFlags(&ctx->ev_ring[k], cudaEventDisableTiming));
     }
     if (ctx->ws_nrhs < ctx->nrhs) {
+        // Grow for a deeper stack: the old vectors go first (two sets would not fit at the sizes this is for).  ws_nrhs is 0
+        // while the set is incomplete, so that a failed growth (out of memory) leaves a context whose next solve allocates
+        // afresh instead of running on missing vectors.
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
-        for (int k = 0; k < 12; k++) { free_owned(ctx, ctx->w32[k]); free_owned(ctx, ctx->w64[k]); ctx->w32[k] = nullptr; ctx->w64[k] = nullptr; }
-        for (int k = 0; k < 3; k++) { free_owned(ctx, ctx->ras32[k]); ctx->ras32[k] = nullptr; }
+        auto release = [&]() {
+            for (int k = 0; k < 12; k++) { free_owned(ctx, ctx->w32[k]); free_owned(ctx, ctx->w64[k]); ctx->w32[k] = nullptr; ctx->w64[k] = nullptr; }
+            for (int k = 0; k < 3; k++) { free_owned(ctx, ctx->ras32[k]); ctx->ras32[k] = nullptr; }
+        };
+        ctx->ws_nrhs = 0;
+        release();
         const size_t nr = ctx->nrhs;
-        for (int k = 0; k < 12; k++)
-            if (alloc_dev(ctx, (void**)&ctx->w32[k], sizeof(float4) * 6 * V * nr)) return WCRAS_CUDA_ERROR;
-        for (int k = 0; k < 12; k++)
-            if (alloc_dev(ctx, (void**)&ctx->w64[k], sizeof(double2) * 12 * V * nr)) return WCRAS_CUDA_ERROR;
-        for (int k = 0; k < 3; k++)
-            if (alloc_dev(ctx, (void**)&ctx->ras32[k], sizeof(float4) * 6 * V * nr)) return WCRAS_CUDA_ERROR;
+        bool ok = true;
+        for (int k = 0; k < 12 && ok; k++) ok = alloc_dev(ctx, (void**)&ctx->w32[k], sizeof(float4) * 6 * V * nr) == WCRAS_OK;
+        for (int k = 0; k < 12 && ok; k++) ok = alloc_dev(ctx, (void**)&ctx->w64[k], sizeof(double2) * 12 * V * nr) == WCRAS_OK;
+        for (int k = 0; k < 3 && ok; k++) ok = alloc_dev(ctx, (void**)&ctx->ras32[k], sizeof(float4) * 6 * V * nr) == WCRAS_OK;
+        if (!ok) {
+            release();          // ctx->err holds the cudaMalloc message
+            cudaGetLastError();
+            return WCRAS_CUDA_ERROR;
+        }
         ctx->ws_nrhs = ctx->nrhs;
     }
     return WCRAS_OK;
@@ -497,9 +507,9 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
     if (int rc = ensure_workspace(ctx)) return rc;
     const int nr = ctx->nrhs;
     const size_t V = ctx->geom.V, n1 = 12 * V, n64 = n1 * nr;
-    cudaEvent_t e0, e1;
-    WC_CUDA(cudaEventCreate(&e0));
-    WC_CUDA(cudaEventCreate(&e1));
+    EventPair ev;
+    WC_CUDA(ev.create());
+    const cudaEvent_t e0 = ev.a, e1 = ev.b;
     WC_CUDA(cudaEventRecord(e0, ctx->stream));
     ctx->dv32 = ctx->dv64 = ctx->block_dv = ctx->ras_applies = 0;
     ctx->ev_used = 0;
@@ -572,8 +582,6 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
     float ms = 0;
     WC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     if (ctx->timing) {
         for (size_t k = 0; k + 1 < ctx->ev_used; k += 2) {
             float t = 0;
@@ -598,9 +606,9 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
 int time_blas(wcras_ctx* ctx, int reps, double* ms) {
     if (int rc = ensure_workspace(ctx)) return rc;
     Work<float> w = work32(ctx);
-    cudaEvent_t e0, e1;
-    WC_CUDA(cudaEventCreate(&e0));
-    WC_CUDA(cudaEventCreate(&e1));
+    EventPair ev;
+    WC_CUDA(ev.create());
+    const cudaEvent_t e0 = ev.a, e1 = ev.b;
     WC_CUDA(cudaMemsetAsync(ctx->sc32, 0, sizeof(Scalars), ctx->stream));
     for (int k = 0; k < 8; k++) WC_CUDA(cudaMemsetAsync(ctx->w32[k], 0, sizeof(float4) * w.n, ctx->stream));
     WC_CUDA(cudaEventRecord(e0, ctx->stream));
@@ -610,8 +618,6 @@ int time_blas(wcras_ctx* ctx, int reps, double* ms) {
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
     float t = 0;
     WC_CUDA(cudaEventElapsedTime(&t, e0, e1));
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
     *ms = t / reps;
     return WCRAS_OK;
 }

@@ -243,6 +243,19 @@ inline wc::Fields<float> ras_fields(const wcras_ctx* ctx) {
     return ctx->op_prec == 16 && ctx->r16a ? wc::Fields<float>{ctx->r16a, ctx->r16b, ctx->r16c} : ctx->fields<float>();
 }
 
+// two timing events, destroyed on every exit path of the function that owns them
+struct EventPair {
+    cudaEvent_t a = nullptr, b = nullptr;
+    cudaError_t create() {
+        cudaError_t e = cudaEventCreate(&a);
+        return e != cudaSuccess ? e : cudaEventCreate(&b);
+    }
+    ~EventPair() {
+        if (a) cudaEventDestroy(a);
+        if (b) cudaEventDestroy(b);
+    }
+};
+
 #define WC_CUDA(call)                                                                                   \
     do {                                                                                                \
         cudaError_t e_ = (call);                                                                        \

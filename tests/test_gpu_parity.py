@@ -514,7 +514,8 @@ def test_hard_regime_smooth_field():
 
 
 def test_ras_autotune():
-    """Parameter survey: the fastest converged row is returned and left configured."""
+    """Parameter survey: the fastest converged row is returned and left configured; truncated to 12 rows it
+    is the additive overlap-0 stage only."""
     cs = case(1)
     eta = I.spinor(cs.dims, 2)
     x = dev(eta, torch.float64)
@@ -524,11 +525,76 @@ def test_ras_autotune():
     assert ok and best["ms"] == min(r["ms"] for r in ok)
     assert all(r["rel_resid_true"] <= 1e-12 for r in ok)
     for r in rows[1:]:
-        assert all(d in (2, 4, 8) for d in r["domain"]) and r["overlap_s"] == 0
+        assert all(d in (2, 4, 8) for d in r["domain"]) and r["overlap_s"] == 0 and r["schwarz"] == 0
     phi, info = cs.solve(eta, 1e-12)                                  # solves with the configuration left behind
     assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
     assert (info["ras_applies"] > 0) == (best["block_iters"] > 0)
     cs.ctx.set_solver(use_ras=False)
+
+
+def test_ras_autotune_full_grid():
+    """The whole survey of PAPER.md:109 (N_dominv x NRAS rectangle, overlap s = 1, 2 = the paper's d = 2, 4, multiplicative
+    Schwarz, operand precision): rows with a non-zero overlap, SAP rows and both operand precisions are present, every
+    converged row meets the tolerance, and the configuration left behind (whatever its kind) solves to the oracle's
+    residual."""
+    cs = case(1)
+    eta = I.spinor(cs.dims, 2)
+    x = dev(eta, torch.float64)
+    try:
+        best, rows = cs.ctx.ras_autotune(x, 1e-12, max_rows=256)
+        assert rows[0]["block_iters"] == 0 and len(rows) > 60
+        ok = [r for r in rows if r["status"] == 0]
+        assert best["ms"] == min(r["ms"] for r in ok)
+        assert all(r["rel_resid_true"] <= 1e-12 for r in ok)
+        assert any(r["overlap_s"] == 1 for r in ok) and any(r["overlap_s"] == 2 for r in rows)
+        assert any(r["schwarz"] == 1 for r in ok)
+        assert {r["operand_bits"] for r in rows[1:]} == {16, 32}
+        rect = {(r["block_iters"], r["nras"]) for r in rows if r["overlap_s"] == 0 and r["schwarz"] == 0 and r["block_iters"]}
+        assert {(a, b) for a in range(1, 9) for b in range(1, 6)} <= rect          # the 1..8 x 1..5 rectangle was walked
+        phi, info = cs.solve(eta, 1e-12)
+        assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+        assert (info["ras_applies"] > 0) == (best["block_iters"] > 0)
+    finally:
+        cs.ctx.set_schwarz(False)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_solver(use_ras=False)
+
+
+def test_workspace_growth_failure():
+    """A stacked solve whose workspace growth runs out of memory (injected: WCRAS_FAIL_ALLOC_ABOVE) returns an error and
+    leaves a context that solves a single right-hand side again (ws_nrhs must not survive a failed growth)."""
+    import os
+    cfg = I.CONFIGS[1]
+    U = I.make_gauge(cfg)
+    ctx = binding.Context(cfg["dims"], cfg["kappa"], cfg["csw"], dev(U, torch.float64))
+    op = O.Operator(cfg["dims"], U, cfg["kappa"], cfg["csw"])
+    V = I.volume(cfg["dims"])
+    eta = I.spinor(cfg["dims"], 3)
+    x = dev(eta, torch.float64)
+    phi = torch.empty_like(x)
+    ctx.ras_precondition((4, 4, 4, 4), 0, 4, 2)
+    assert ctx.solve(x, phi, 1e-12)["status"] == 0
+    x2 = torch.cat([x, x]).contiguous()
+    p2 = torch.empty_like(x2)
+    os.environ["WCRAS_FAIL_ALLOC_ABOVE"] = str(16 * 12 * V + 1)        # above every nrhs = 1 vector, below the fp64 ones at nrhs = 2
+    try:
+        with pytest.raises(binding.WcrasError) as e:
+            ctx.solve_multi(2, x2, p2, 1e-12)
+        assert e.value.code == binding.CUDA_ERROR and "out of memory" in str(e.value)
+    finally:
+        del os.environ["WCRAS_FAIL_ALLOC_ABOVE"]
+    info = ctx.solve(x, phi, 1e-12)                                    # allocates afresh and solves
+    torch.cuda.synchronize()
+    a = phi.cpu().numpy()
+    got = (a[..., 0] + 1j * a[..., 1]).reshape(V, 4, 3)
+    assert info["status"] == 0 and op.true_residual(eta, got) <= 1e-12
+    r32 = I.spinor(cfg["dims"], 5).astype(np.complex64).astype(np.complex128)
+    y = dev(r32, torch.float32)
+    out = torch.empty_like(y)
+    ctx.ras_apply(y, out)                                             # the unchained K_RAS path uses the work vectors too
+    info2, res = ctx.solve_multi(2, x2, p2, 1e-12)                    # and the growth itself works once memory is there
+    assert info2["status"] == 0 and max(res) <= 1e-12
+    ctx.destroy()
 
 
 @pytest.mark.parametrize("prec", [32, 64])
