@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restric
 // DOT = 2: also ts = <out, dotv>, tt = <out, out>, omega = ts/tt (BiCGStab: t = D sh, dotv = s)
 template <typename T, bool XPAY, int TH, int MINB, int DOT>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
-                                                     typename VecOf<T>::type* __restrict__ out,
+                                                     typename VecOf<T>::type* out,  // may be bsrc (r = r - D v in place)
                                                      const typename VecOf<T>::type* bsrc,
                                                      const typename VecOf<T>::type* __restrict__ dotv, double* part,
                                                      unsigned pstride, unsigned poff, size_t rstride, int ztile) {

@@ -36,8 +36,8 @@ __device__ __forceinline__ void domain_start(const Geom& g, const DomGeom& dg, i
 template <bool FIRST>
 __global__ void __launch_bounds__(128) mr_dslash_kernel(Geom g, DomGeom dg, Fields<float> f, float kappa, const float4* __restrict__ rglob,
                                                         const float4* __restrict__ rho, float4* __restrict__ q, double* __restrict__ scal) {
-    const int d = blockIdx.y;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.x;  // domain in gridDim.x (no 65535 limit), chunk of the domain in gridDim.y
+    const int k = blockIdx.y * blockDim.x + threadIdx.x;
     double acc[3] = {0, 0, 0};
     if (k < dg.nloc) {
         int start[4], c[4], x[4];
@@ -112,10 +112,10 @@ __global__ void __launch_bounds__(128) mr_dslash_kernel(Geom g, DomGeom dg, Fiel
         if (lane == 0) sm[n][w] = s;
     }
     __syncthreads();
-    if (threadIdx.x < 3) {
+    if (threadIdx.x < 3) {  // one partial per CTA, summed in a fixed order by mr_update_kernel (deterministic)
         double s = 0;
         for (int ww = 0; ww < (int)(blockDim.x >> 5); ww++) s += sm[threadIdx.x][ww];
-        atomicAdd(&scal[(size_t)d * 4 + threadIdx.x], s);
+        scal[((size_t)d * gridDim.y + blockIdx.y) * 4 + threadIdx.x] = s;
     }
 }
 
@@ -125,10 +125,14 @@ template <bool FIRST, bool LAST, bool ACCUM>
 __global__ void __launch_bounds__(128) mr_update_kernel(Geom g, DomGeom dg, const float4* __restrict__ rglob, float4* __restrict__ rho,
                                                         const float4* __restrict__ q, float4* __restrict__ v, float4* __restrict__ vout,
                                                         const double* __restrict__ scal) {
-    const int d = blockIdx.y;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.x;
+    const int k = blockIdx.y * blockDim.x + threadIdx.x;
     if (k >= dg.nloc) return;
-    const double qr = scal[(size_t)d * 4], qi = scal[(size_t)d * 4 + 1], qq = scal[(size_t)d * 4 + 2];
+    double qr = 0, qi = 0, qq = 0;
+    for (unsigned c = 0; c < gridDim.y; c++) {  // the per-CTA partials of this domain, in order
+        const double* p = scal + ((size_t)d * gridDim.y + c) * 4;
+        qr += p[0]; qi += p[1]; qq += p[2];
+    }
     // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9)
     const float ar = qq > 0 ? (float)(qr / qq) : 0.f, ai = qq > 0 ? (float)(qi / qq) : 0.f;
     int start[4], c[4], x[4];
@@ -265,7 +269,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         WC_CUDA(cudaMalloc((void**)&ctx->mr_rho, nb));
         WC_CUDA(cudaMalloc((void**)&ctx->mr_q, nb));
         WC_CUDA(cudaMalloc((void**)&ctx->mr_v, nb));
-        WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * niter));
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * ((rc.nloc + 127) / 128) * niter));
     }
     if (ctx->dm) {
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -312,12 +316,12 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
     const RasConfig& rc = ctx->ras;
     const DomGeom dg = make_domgeom(ctx);
     const int TH = 128;
-    const dim3 grid((rc.nloc + TH - 1) / TH, rc.nd);
-    WC_CUDA(cudaMemsetAsync(ctx->mr_scal, 0, sizeof(double) * 4 * (size_t)rc.nd * rc.niter, ctx->stream));
+    const int nchunk = (rc.nloc + TH - 1) / TH;
+    const dim3 grid(rc.nd, nchunk);
     const Fields<float> f = ras_fields(ctx);
     const float kappa = (float)ctx->kappa;
     for (int it = 0; it < rc.niter; it++) {
-        double* scal = ctx->mr_scal + (size_t)it * rc.nd * 4;
+        double* scal = ctx->mr_scal + (size_t)it * rc.nd * nchunk * 4;  // [niter][nd][nchunk][4] per-CTA partial dots
         const bool first = it == 0, last = it == rc.niter - 1;
         if (first) mr_dslash_kernel<true><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);
         else mr_dslash_kernel<false><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);

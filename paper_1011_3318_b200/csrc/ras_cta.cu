@@ -65,9 +65,10 @@ __global__ void pack_domain_major_kernel(FusedGeom fg, int nd, Fields<float> f, 
 //   rho_out rho_fin of this cycle, or nullptr (then the last MR residual update is skipped, Q12)
 template <bool CHAIN, bool MULTI>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
-ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __restrict__ dm, const float4* __restrict__ r_src,
+ras_cta_kernel(FusedGeom fg, int ndl, int colour, int nface, const float4* __restrict__ dm, const float4* r_src,
                const float4* __restrict__ hb_in, float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out,
                float4* rho_out, int nrhs, size_t rstride, size_t hstride) {
+    // r_src and rho_out are the same buffer in the chained cycles (a thread reads its site before it writes it): no __restrict__
     // nrhs > 1 (wcras_solve_multi): every vector argument is a stack of nrhs vectors rstride apart (halo buffers:
     // hstride); the right-hand sides of a domain are solved one after the other with the operands loaded once
     if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)

@@ -78,9 +78,10 @@ __device__ __forceinline__ void ld_half(const float4* __restrict__ slot, int nsp
 
 template <bool CL>
 __global__ void __launch_bounds__(FUSED_MAX_THREADS, 1)
-ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* __restrict__ r, float4* __restrict__ vout, int accum,
+ras_fused_kernel(FusedGeom fg, int nd, Fields<float> f, float kappa, const float4* r, float4* __restrict__ vout, int accum,
                  int nface, const float4* __restrict__ hb_in, float4* __restrict__ hb_out, float4* rho_out,
                  const float4* __restrict__ dmc) {
+    // r and rho_out are the same buffer in the chained cycles (a thread reads its site before it writes it): no __restrict__
     // dmc (overlap 0 only): domain-major operand copy float4 [nd][C][36][nsp] -- the 72 link reals, then the 72 clover
     // reals of the sites of one CTA contiguous (147 KB), as in ras_cta.cu but with the links unscaled
     // Chained cycles (overlap 0; same scheme as ras_cta.cu, reading A3): hb_in != nullptr: r is rho_fin of the

@@ -194,7 +194,7 @@ struct wcras_ctx {
     int nface = 0;
     int hb_nrhs = 0;               // stack depth the halo buffers are allocated for
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
-    double* mr_scal = nullptr;                                     // [niter][nd][4]
+    double* mr_scal = nullptr;                                     // [niter][nd][nchunk][4] per-CTA partial dots
     // solver parameters
     double inner_tol = 5e-7;       // deepest relative accuracy asked of one fp32 inner solve (reading A2)
     double outer_target = 0;       // absolute residual norm the running outer pass has to reach

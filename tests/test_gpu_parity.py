@@ -645,6 +645,36 @@ def test_full_size_32_ras_apply():
         assert rel(want16, want) > 2e-5
     finally:
         cs.ctx.set_operand_precision(32)
+    # the named shapes of configs[3] on the cluster tier with fp16 operands staged by TMA (ras_cl16.cu), full size: 1024
+    # domains over 33 4-CTA clusters, 256 domains over 9 16-CTA clusters, chained cycles
+    cs.ctx.set_operand_precision(16)
+    try:
+        for block, nit, nras in (((8, 8, 4, 4), 2, 3), ((8, 8, 8, 8), 2, 2)):
+            cs.ctx.ras_precondition(block, 0, nit, nras)
+            got = cs.ras_apply(r32)
+            want16 = rounded_op(cs).ras_apply(block, 0, nit, nras, r32)
+            assert rel(got, want16) <= TOL_RAS
+            assert np.abs(got - want16).max() / np.abs(want16).max() <= 10 * TOL_RAS
+    finally:
+        cs.ctx.set_operand_precision(32)
+
+
+def test_generic_tier_many_domains():
+    """Forced generic tier with more than 65535 domains (2^4 blocks on 32^4 = 65536 domains: the domain index lives in
+    gridDim.x), per-domain dots summed in a fixed order: equal to the oracle and bit-identical run to run."""
+    cs = case(3)
+    r32 = I.spinor(cs.dims, 79).astype(np.complex64).astype(np.complex128)
+    cs.ctx.set_ras_tier(1)
+    try:
+        cs.ctx.ras_precondition((2, 2, 2, 2), 0, 2, 1)
+        got = cs.ras_apply(r32)
+        assert rel(got, cs.op.ras_apply((2, 2, 2, 2), 0, 2, 1, r32)) <= TOL_RAS
+        cs.ctx.ras_precondition((8, 4, 4, 4), 1, 2, 1)          # 2160-site extended domains: 17 CTAs per domain share the dots
+        a = cs.ras_apply(r32)
+        b = cs.ras_apply(r32)
+        assert np.array_equal(a, b)
+    finally:
+        cs.ctx.set_ras_tier(0)
 
 
 def test_full_size_32_sap_and_multi():
