@@ -304,7 +304,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
             for (int mu = 0; mu < 4; mu++) nface = rc.nloc / rc.ext[mu] > nface ? rc.nloc / rc.ext[mu] : nface;
             if (ctx->hb) { WC_CUDA(cudaStreamSynchronize(ctx->stream)); cudaFree(ctx->hb); ctx->hb = nullptr; }
             ctx->hb_nrhs = 0;
-            ctx->nface = (nface + 7) / 8 * 8;
+            ctx->nface = rc.cl16 ? fgeom.C * ctx->cl16_nfc : (nface + 7) / 8 * 8;  // ras_cl16: halo slots per CTA, [nd][C][8][3][nfc]
         }
     }
     ctx->ras = rc;

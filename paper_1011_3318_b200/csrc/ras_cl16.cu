@@ -8,8 +8,12 @@
 // Q9), restriction R_Omega, the disjoint sum, phi += v (line 9), chained cycles (reading A3) -- with
 // the data path of ras_cta16.cu carried over to the cluster:
 //   * Omega' is cut into C <= 16 sub-blocks of <= 256 sites, one CTA per sub-block, one thread per site; the CTAs of a
-//     domain form a cluster.  Half spinors cross sub-block faces with st.shared::cluster (DSMEM); two cluster barriers
-//     per MR iteration (exchange, dots); the clover term is applied between arrive and wait of the first one.
+//     domain form a cluster.  A half spinor whose receiver sits in the same CTA is a plain st.shared; one that crosses a
+//     sub-block face travels by st.async (DSMEM store that completes bytes on an mbarrier of the RECEIVING CTA), and the
+//     receiver waits on that mbarrier: no cluster barrier and no memory fence in the MR iteration.  (barrier.cluster
+//     arrive.release / wait.acquire twice per iteration cost 14 % of the warp time in MEMBAR stalls alone, ncu
+//     profiles/r2_kernels.md.)  The domain-local dots travel the same way: one float4 per warp to every CTA of the
+//     cluster, completing on a second pair of mbarriers; the table is double-buffered by sweep parity.
 //   * Operands: links and packed clover blocks ROUNDED TO fp16 (reading R1), domain-major per CTA,
 //     dm16 = uint4 [nd][C][18][nsp].  Each CTA stages its 18*nsp*16 bytes with two cp.async.bulk (TMA) copies onto
 //     mbarriers while the previous domain of its cluster is still being solved: the links half as soon as every thread
@@ -17,9 +21,11 @@
 //     fp32 operands synchronously at the start of every domain: 0.12-0.15 ms per launch at 32^4 against 0.04 here.)
 //   * Links pre-scaled by -kappa at conversion, so q accumulates the hops directly; packed fp32 arithmetic
 //     (site_math.cuh, FFMA2).
-//   * Chained cycles keep rho_fin domain-major (float4 [nd][C][6][nsp], one bulk copy per CTA); halo slots are read
-//     from global memory (a face of a large domain does not fit beside the rest).
-// Shared memory per CTA at nsp = 256: 96 KB half-spinor slots + 72 KB operands + 24 KB residual + 2 KB dot partials.
+//   * Chained cycles keep rho_fin domain-major (float4 [nd][C][6][nsp], one bulk copy per CTA) and the halo slots
+//     CTA-major ([nd][C][8][3][nfc], nfc = largest face of a sub-block), so that a CTA stages its own 24*nfc*16 bytes with
+//     one bulk copy as well.
+// Shared memory per CTA at nsp = 256: 96 KB half-spinor slots + 72 KB operands + 24 KB residual + 24 KB halo + 4 KB dot
+// partials.
 // Roofline: HBM; algorithmic bytes per extended site and launch 288 operands + 96 residual in, 96 per bulk site out
 // (+ 96 rho_fin, + halo in the chained cycles).
 #include <cuda_fp16.h>
@@ -40,19 +46,22 @@ __device__ __forceinline__ unsigned cl16_mapa(unsigned addr, unsigned rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
 }
-// predicated 16-byte store into the shared memory of any CTA of the cluster (dst == 0xffffffff: no receiver, Dirichlet)
-__device__ __forceinline__ void st_cl_pred_f4(unsigned addr, float a, float b, float c, float d) {
+// 16-byte store to a half-spinor slot: plain st.shared when the receiver is a site of this CTA (loc), st.async with
+// completion on the receiving CTA's mbarrier when it sits in another CTA of the cluster (rem); neither: no receiver
+// (Dirichlet).  addr is a shared::cta address in the first case and a shared::cluster address in the second.
+__device__ __forceinline__ void st_slot_f4(unsigned addr, unsigned mbar, bool loc, bool rem, float a, float b, float c, float d) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0xffffffff;\n\t@p st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};\n\t}" ::"r"(addr),
-        "f"(a), "f"(b), "f"(c), "f"(d)
+        "{\n\t.reg .pred pl, pr;\n\tsetp.ne.u32 pl, %6, 0;\n\tsetp.ne.u32 pr, %7, 0;\n\t"
+        "@pl st.shared.v4.f32 [%0], {%1, %2, %3, %4};\n\t"
+        "@pr st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];\n\t}" ::"r"(addr),
+        "f"(a), "f"(b), "f"(c), "f"(d), "r"(mbar), "r"((unsigned)loc), "r"((unsigned)rem)
         : "memory");
 }
-__device__ __forceinline__ void st_cl_half_pred(unsigned dst, unsigned chunk_bytes, const float* h) {
-    const unsigned d1 = dst == 0xffffffffu ? dst : dst + chunk_bytes;
-    const unsigned d2 = dst == 0xffffffffu ? dst : dst + 2 * chunk_bytes;
-    st_cl_pred_f4(dst, h[0], h[1], h[2], h[3]);
-    st_cl_pred_f4(d1, h[4], h[5], h[6], h[7]);
-    st_cl_pred_f4(d2, h[8], h[9], h[10], h[11]);
+__device__ __forceinline__ void st_slot_half(unsigned dst, unsigned mbar, bool remote, unsigned chunk_bytes, const float* h) {
+    const bool ok = dst != 0xffffffffu, loc = ok && !remote, rem = ok && remote;
+    st_slot_f4(dst, mbar, loc, rem, h[0], h[1], h[2], h[3]);
+    st_slot_f4(dst + chunk_bytes, mbar, loc, rem, h[4], h[5], h[6], h[7]);
+    st_slot_f4(dst + 2 * chunk_bytes, mbar, loc, rem, h[8], h[9], h[10], h[11]);
 }
 __device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
@@ -110,37 +119,41 @@ __global__ void pack_cl16_kernel(FusedGeom fg, int nd, Fields<float> f, uint4* _
 }
 
 struct Cl16Smem {  // offsets in float4 units
-    int hbuf, opbuf, rstage, red, bars, org;
+    int hbuf, opbuf, rstage, hstage, red, bars, org;
     size_t bytes;
 };
-__host__ __device__ inline Cl16Smem cl16_smem(int nsp, int C) {
+__host__ __device__ inline Cl16Smem cl16_smem(int nsp, int C, int nfc) {
     Cl16Smem s;
     s.hbuf = 0;
     s.opbuf = 24 * nsp;
     s.rstage = s.opbuf + 18 * nsp;
-    s.red = s.rstage + 6 * nsp;
-    s.bars = s.red + C * (nsp / 32);
-    s.org = s.bars + 2;
-    s.bytes = (size_t)(s.org + 2) * 16;
+    s.hstage = s.rstage + 6 * nsp;            // [8][3][nfc] halo slots of this CTA (chained cycles)
+    s.red = s.hstage + 24 * nfc;              // [2][C][nwarps] dot partials of the whole cluster, by sweep parity
+    s.bars = s.red + 2 * C * (nsp / 32);      // 6 mbarriers: links, clover, vectors, exchange, dots[2]
+    s.org = s.bars + 3;
+    s.bytes = (size_t)(s.org + 3) * 16;       // org[2] = {bytes expected on the exchange mbarrier per MR iteration, ...}
     return s;
 }
 
-// One K_RAS cycle (Alg.1 lines 3-9) for all domains; arguments as ras_cta16_kernel (no colouring, halo slots in global)
+// One K_RAS cycle (Alg.1 lines 3-9) for all domains; arguments as ras_cta16_kernel (no colouring); nfc = padded size of
+// the largest face of a sub-block, halo buffers CTA-major [nd][C][8][3][nfc]
 template <bool CHAIN>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
-ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __restrict__ dm16, const float4* __restrict__ r_lat,
+ras_cl16_kernel(FusedGeom fg, int nd, int nfc, float mkappa, const uint4* __restrict__ dm16, const float4* __restrict__ r_lat,
                 const float4* __restrict__ r_dm, const float4* __restrict__ hb_in, float4* __restrict__ hb_out, const float4* phi_in,
                 float4* phi_out, float4* __restrict__ rho_dm, const int4* __restrict__ dom_org, const unsigned* __restrict__ dom_bc) {
     if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
     extern __shared__ float4 smem[];
     const int nsp = fg.nsp, C = fg.C;
-    const Cl16Smem lay = cl16_smem(nsp, C);
+    const Cl16Smem lay = cl16_smem(nsp, C, nfc);
     float4* hbuf = smem + lay.hbuf;                                        // [8][3][nsp] half-spinor slots
     const uint4* opbuf = reinterpret_cast<const uint4*>(smem + lay.opbuf);  // [18][nsp] fp16 operands of the current domain
     float4* rstage = smem + lay.rstage;                                    // [6][nsp] residual of the current / next domain
-    float4* red = smem + lay.red;                                          // [C][nwarps] dot partials of the whole cluster
+    const float4* hstage = smem + lay.hstage;                              // [8][3][nfc] halo slots of this CTA (chained cycles)
+    float4* red = smem + lay.red;                                          // [2][C][nwarps] dot partials of the whole cluster
     int4* org_s = reinterpret_cast<int4*>(smem + lay.org);                 // [2] first site of the current / next domain (table dom_org)
     const unsigned bar_links = cta_smem_u32(smem + lay.bars), bar_clov = bar_links + 8, bar_vec = bar_links + 16;
+    const unsigned bar_x = bar_links + 24, bar_d = bar_links + 32;  // exchange (remote half spinors), dots [2] (by sweep parity)
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
     const unsigned rank = cl16_rank();
     const int cl = blockIdx.x / C, ncl = gridDim.x / C;
@@ -151,7 +164,9 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
     int ec[4];
     bool bulk = active;
     unsigned dst[8];  // slot 2mu: receiver x-mu (its forward hop); slot 2mu+1: receiver x+mu (its backward hop)
-    int fidx[4];      // index of the site within the mu-face of Omega' (coordinate mu removed), unique over the cluster
+    int fidx[4];      // index of the site within the mu-face of its sub-block (local index with coordinate mu removed)
+    unsigned remote = 0;          // bit n: the receiver of slot n sits in another CTA of the cluster
+    unsigned rk_pk = 0;           // 4 bits per direction: the rank of that CTA
     const unsigned chunk_bytes = (unsigned)nsp * 16u;
     {
         int lc[4], sc[4];
@@ -163,19 +178,11 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             ec[mu] = sc[mu] * fg.sb[mu] + lc[mu];
             if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
         }
-        int E = 0, es = 1;
-#pragma unroll
-        for (int mu = 0; mu < 4; mu++) { E += ec[mu] * es; es *= fg.ext[mu]; }
-        es = 1;
-#pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            fidx[mu] = (E % es) + (E / (es * fg.ext[mu])) * es;
-            es *= fg.ext[mu];
-        }
         const unsigned base = cta_smem_u32(hbuf);
         int lstride = 1, cstride = 1;
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
+            fidx[mu] = (k % lstride) + (k / (lstride * fg.sb[mu])) * lstride;
 #pragma unroll
             for (int sg = 0; sg < 2; sg++) {  // sg 0: receiver x-mu, sg 1: receiver x+mu
                 int kd = k, rk = (int)rank;
@@ -197,8 +204,13 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
                         else ok = false;
                     }
                 }
-                const unsigned a = cl16_mapa(base + (unsigned)((2 * mu + sg) * 3 * nsp + kd) * 16u, (unsigned)rk);
-                dst[2 * mu + sg] = ok ? a : 0xffffffffu;
+                const unsigned a_loc = base + (unsigned)((2 * mu + sg) * 3 * nsp + kd) * 16u;
+                const bool far = rk != (int)rank;
+                dst[2 * mu + sg] = ok ? (far ? cl16_mapa(a_loc, (unsigned)rk) : a_loc) : 0xffffffffu;
+                if (ok && far) {  // at most one remote receiver per direction (sub-blocks are at least two sites thick)
+                    remote |= 1u << (2 * mu + sg);
+                    rk_pk |= (unsigned)rk << (4 * mu);
+                }
             }
             lstride *= fg.sb[mu];
             cstride *= fg.c[mu];
@@ -214,15 +226,27 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         mbar_init(bar_links, 1);
         mbar_init(bar_clov, 1);
         mbar_init(bar_vec, 1);
+        mbar_init(bar_x, 1);
+        mbar_init(bar_d, 1);
+        mbar_init(bar_d + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // bytes of half spinors that arrive from other CTAs per MR iteration: slot 2mu of a site is written by x+mu and slot
+    // 2mu+1 by x-mu, so a slot is filled remotely exactly when this site's own store in the opposite sense is remote
+    {
+        unsigned xb = 0;
+#pragma unroll
+        for (int n = 0; n < 8; n++) xb += 48u * (unsigned)__syncthreads_count(0 != (remote & (1u << n)));
+        if (k == 0) org_s[2].x = (int)xb;  // read back by thread 0 at the top of every MR iteration
+    }
     cl_arrive();
-    cl_wait();  // every CTA of the cluster has zeroed its slots before anybody scatters into them
+    cl_wait();  // every CTA of the cluster has zeroed its slots and initialised its mbarriers before anybody stores into it
 
     const size_t V = fg.V;
     const unsigned half_bytes = 9u * chunk_bytes;  // links or clover part of one CTA's share of a domain
-    const unsigned vec_bytes = src_dm ? 6u * chunk_bytes : 0u;
-    const unsigned op_addr = cta_smem_u32(opbuf), rs_addr = cta_smem_u32(rstage);
+    const unsigned halo_bytes = CHAIN ? 24u * (unsigned)nfc * 16u : 0u;
+    const unsigned vec_bytes = (src_dm ? 6u * chunk_bytes : 0u) + halo_bytes;
+    const unsigned op_addr = cta_smem_u32(opbuf), rs_addr = cta_smem_u32(rstage), hs_addr = cta_smem_u32(hstage);
 
     auto request_links_vec = [&](int d) {
         if (k == 0) {
@@ -231,7 +255,8 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             bulk_g2s(op_addr, dm16 + chunk * 18 * nsp, half_bytes, bar_links);
             if (vec_bytes) {
                 mbar_expect_tx(bar_vec, vec_bytes);
-                bulk_g2s(rs_addr, r_dm + chunk * 6 * nsp, vec_bytes, bar_vec);
+                if (src_dm) bulk_g2s(rs_addr, r_dm + chunk * 6 * nsp, 6u * chunk_bytes, bar_vec);
+                if (CHAIN) bulk_g2s(hs_addr, hb_in + chunk * 24 * nfc, halo_bytes, bar_vec);
             }
         }
     };
@@ -268,6 +293,7 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
     }
 
     float U[72];
+    unsigned sw = 0;  // MR iterations done by this cluster so far: parity of the exchange mbarrier, index / parity of the dots pair
     for (int j = 0;; j++) {
         const int dom = cl + j * ncl;
         if (dom >= nd) break;
@@ -290,7 +316,7 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         // ---- projection P_Omega' r: the staged residual column of this thread ----
         float rho[24], v[24];
         cp_async_wait();  // own residual column (lattice-layout source); thread 0: the origin of this domain in org_s
-        if (src_dm) mbar_wait(bar_vec, par);
+        if (vec_bytes) mbar_wait(bar_vec, par);
 #pragma unroll
         for (int c = 0; c < 6; c++) {
             float4 t = rstage[c * nsp + k];
@@ -299,17 +325,17 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         }
         if (!src_dm && has_next) request_r_lat(org_nxt);  // own column: free as soon as it has been read
         if (CHAIN) {
-            // ---- boundary coupling: rho -= D-terms of v_{j-1} that cross the domain boundary (reading A3); the halo
-            // slots of this domain come straight from global memory (L2: written by the previous launch) ----
-            const float4* hin = hb_in + (size_t)dom * 24 * nface;
+            // ---- boundary coupling: rho -= D-terms of v_{j-1} that cross the domain boundary (reading A3), from the
+            // staged halo slots of this CTA ----
+            const float4* hin = hstage;
             float g[12], hh[12];
 #define WC_CROSS_LOAD(SL)                                                                         \
     {                                                                                             \
         const bool rcv = active && dst[(SL) ^ 1] == 0xffffffffu;                                  \
-        const float4* q4 = hin + (size_t)(SL) * 3 * nface + WC_FIDX((SL) >> 1);                      \
+        const float4* q4 = hin + (SL) * 3 * nfc + WC_FIDX((SL) >> 1);                             \
         _Pragma("unroll") for (int jj = 0; jj < 3; jj++) {                                        \
             float4 t = make_float4(0.f, 0.f, 0.f, 0.f);                                           \
-            if (rcv) t = __ldcs(q4 + (size_t)jj * nface);                                         \
+            if (rcv) t = q4[jj * nfc];                                                            \
             hh[4 * jj] = t.x; hh[4 * jj + 1] = t.y; hh[4 * jj + 2] = t.z; hh[4 * jj + 3] = t.w;   \
         }                                                                                         \
     }
@@ -327,27 +353,32 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
 #undef WC_CROSS
 #undef WC_CROSS_LOAD
         }
-        if (CHAIN && has_next && k == 32)
-            prefetch_l2_bulk(hb_in + (size_t)nxt * 24 * nface, 24u * (unsigned)nface * 16u);
 #pragma unroll
         for (int n = 0; n < 24; n++) v[n] = 0.f;
 
-        for (int it = 0; it < fg.niter; it++) {
+        for (int it = 0; it < fg.niter; it++, sw++) {
+            const unsigned bar_dk = bar_d + 8u * (sw & 1u);
+            if (k == 0) {  // this iteration's arrivals: the remote half spinors and the C * nwarps dot partials
+                mbar_expect_tx(bar_x, (unsigned)org_s[2].x);
+                mbar_expect_tx(bar_dk, 16u * (unsigned)(C * nwarps));
+            }
             {
                 float hs[12], g[12];
-#define WC_SCATTER(MU)                                       \
-    project<float, MU, -1>(rho, hs);                         \
-    st_cl_half_pred(dst[2 * MU], chunk_bytes, hs);           \
-    project<float, MU, +1>(rho, hs);                         \
-    su3_adj_mul<float>(U + 18 * MU, hs, g);                  \
-    st_cl_half_pred(dst[2 * MU + 1], chunk_bytes, g);
+#define WC_SCATTER(MU)                                                                                  \
+    {                                                                                                   \
+        const unsigned xb = cl16_mapa(bar_x, (rk_pk >> (4 * MU)) & 15u);                                \
+        project<float, MU, -1>(rho, hs);                                                                \
+        st_slot_half(dst[2 * MU], xb, (remote >> (2 * MU)) & 1u, chunk_bytes, hs);                      \
+        project<float, MU, +1>(rho, hs);                                                                \
+        su3_adj_mul<float>(U + 18 * MU, hs, g);                                                         \
+        st_slot_half(dst[2 * MU + 1], xb, (remote >> (2 * MU + 1)) & 1u, chunk_bytes, g);               \
+    }
                 WC_SCATTER(0) WC_SCATTER(1) WC_SCATTER(2) WC_SCATTER(3)
 #undef WC_SCATTER
             }
-            cl_arrive();
             float q[24];
             if (it == 0) mbar_wait(bar_clov, par);
-            // q = A rho from the staged fp16 clover blocks (independent of the exchange: overlaps the cluster barrier)
+            // q = A rho from the staged fp16 clover blocks (independent of the exchange: covers the flight of the stores)
 #pragma unroll
             for (int ch = 0; ch < 2; ch++) {
                 float Ab[40];
@@ -355,8 +386,9 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
                 for (int c = 0; c < 5; c++) half8_to_float(opbuf[(9 + 4 * ch + c) * nsp + k], Ab + 8 * c);
                 herm6_mul<float>(Ab + 4 * ch, rho + 12 * ch, q + 12 * ch);
             }
-            cl_wait();
-            // Every thread of the cluster is past its staging reads of this domain (links, residual: before the first
+            __syncthreads();                               // the half spinors stored by this CTA
+            mbar_wait(bar_x, sw & 1u);                     // those stored into it by the other CTAs of the cluster
+            // Every thread of this CTA is past its staging reads of this domain (links, residual, halo: before the first
             // barrier; clover: before this barrier of the last sweep): thread 0 requests the next domain's data.
             if (has_next && warp == 0) {
                 if (it == 0) {
@@ -395,16 +427,20 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
                 d1 += __shfl_xor_sync(0xffffffffu, d1, o);
                 d2 += __shfl_xor_sync(0xffffffffu, d2, o);
             }
-            // one float4 per warp, pushed by lane c into the partial table of CTA c: every CTA sums the same table
+            // one float4 per warp, pushed by lane c into the partial table of CTA c (its copy for this sweep parity) with
+            // completion on that CTA's dots mbarrier: every CTA sums the same table in the same order
+            float4* redk = red + (sw & 1u) * (unsigned)(C * nwarps);
             if (lane < C) {
-                const unsigned slot = cl16_mapa(cta_smem_u32(red + rank * nwarps + warp), (unsigned)lane);
-                asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(slot), "f"(d0), "f"(d1), "f"(d2), "f"(0.f) : "memory");
+                const unsigned slot = cl16_mapa(cta_smem_u32(redk + rank * nwarps + warp), (unsigned)lane);
+                const unsigned db = cl16_mapa(bar_dk, (unsigned)lane);
+                asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(slot),
+                             "f"(d0), "f"(d1), "f"(d2), "f"(0.f), "r"(db)
+                             : "memory");
             }
-            cl_arrive();
-            cl_wait();
+            mbar_wait(bar_dk, (sw >> 1) & 1u);
             float s0 = 0.f, s1 = 0.f, s2 = 0.f;
             for (int n = lane; n < C * nwarps; n += 32) {
-                const float4 p = red[n];
+                const float4 p = redk[n];
                 s0 += p.x; s1 += p.y; s2 += p.z;
             }
 #pragma unroll
@@ -436,26 +472,27 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
         // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
         if (hb_out) {
             unsigned dd = dom_bc_here;
-            int dstride = 1;
+            int dstride = 1, cstr = 1;
             float hs[12], g[12];
 #define WC_HALO(MU)                                                                                              \
     {                                                                                                            \
-        const int nb = fg.nblk[MU], bc = (int)(dd & 255u);                                                       \
+        const int nb = fg.nblk[MU], bc = (int)(dd & 255u), cspan = (fg.c[MU] - 1) * cstr;                        \
         dd >>= 8;                                                                                                \
-        if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the domain at -mu */            \
+        if (active && dst[2 * MU] == 0xffffffffu) { /* lower face -> slot 2mu of the last sub-block of the domain at -mu */ \
             const int nbd = bc == 0 ? dom + (nb - 1) * dstride : dom - dstride;                                  \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU) * 3 * nface + WC_FIDX(MU);                             \
+            float4* o = hb_out + (((size_t)nbd * C + rank + cspan) * 8 + 2 * MU) * 3 * nfc + WC_FIDX(MU);        \
             project<float, MU, -1>(v, hs);                                                                       \
-            for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(hs[4 * jj], hs[4 * jj + 1], hs[4 * jj + 2], hs[4 * jj + 3]); \
+            for (int jj = 0; jj < 3; jj++) o[jj * nfc] = make_float4(hs[4 * jj], hs[4 * jj + 1], hs[4 * jj + 2], hs[4 * jj + 3]); \
         }                                                                                                        \
-        if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the domain at +mu */      \
+        if (active && dst[2 * MU + 1] == 0xffffffffu) { /* upper face -> slot 2mu+1 of the first sub-block of the domain at +mu */ \
             const int nbd = bc + 1 == nb ? dom - (nb - 1) * dstride : dom + dstride;                             \
-            float4* o = hb_out + ((size_t)nbd * 8 + 2 * MU + 1) * 3 * nface + WC_FIDX(MU);                         \
+            float4* o = hb_out + (((size_t)nbd * C + rank - cspan) * 8 + 2 * MU + 1) * 3 * nfc + WC_FIDX(MU);    \
             project<float, MU, +1>(v, hs);                                                                       \
             su3_adj_mul<float>(U + 18 * MU, hs, g);                                                              \
-            for (int jj = 0; jj < 3; jj++) o[(size_t)jj * nface] = make_float4(g[4 * jj], g[4 * jj + 1], g[4 * jj + 2], g[4 * jj + 3]); \
+            for (int jj = 0; jj < 3; jj++) o[jj * nfc] = make_float4(g[4 * jj], g[4 * jj + 1], g[4 * jj + 2], g[4 * jj + 3]); \
         }                                                                                                        \
         dstride *= nb;                                                                                           \
+        cstr *= fg.c[MU];                                                                                        \
     }
             WC_HALO(0) WC_HALO(1) WC_HALO(2) WC_HALO(3)
 #undef WC_HALO
@@ -482,6 +519,9 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nface, float mkappa, const uint4* __re
             }
         }
     }
+    // no CTA leaves while a store from (or a read of its partials by) another CTA of the cluster could still be under way
+    cl_arrive();
+    cl_wait();
 }
 
 // ---- host side ----
@@ -507,7 +547,7 @@ static cudaError_t cl16_launch(wcras_ctx* ctx, const float4* r_lat, const float4
     cudaLaunchAttribute at[1];
     const int nclus = ctx->ras.nd < ctx->cl16_nclus ? ctx->ras.nd : ctx->cl16_nclus;
     cl16_config(fg, nclus, ctx->cta16_smem, ctx->stream, &cfg, at);
-    return cudaLaunchKernelEx(&cfg, ras_cl16_kernel<CHAIN>, fg, ctx->ras.nd, ctx->nface, -(float)ctx->kappa, (const uint4*)ctx->dm16, r_lat, r_dm,
+    return cudaLaunchKernelEx(&cfg, ras_cl16_kernel<CHAIN>, fg, ctx->ras.nd, ctx->cl16_nfc, -(float)ctx->kappa, (const uint4*)ctx->dm16, r_lat, r_dm,
                               hb_in, hb_out, phi_in, phi_out, rho_dm, (const int4*)ctx->dom_org, (const unsigned*)ctx->dom_bc);
 }
 
@@ -515,11 +555,17 @@ static cudaError_t cl16_launch(wcras_ctx* ctx, const float4* r_lat, const float4
 // kernel can run the configuration (2 <= C <= 16, the cluster is schedulable, memory), 0 otherwise (ras_fused.cu runs).
 int ras_cl16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f) {
     if (fg.C < 2 || fg.C > CL16_MAX_CLUSTER || fg.nsp > FUSED_CTA_MAX_THREADS) return 0;
-    for (int mu = 0; mu < 4; mu++) if (fg.nblk[mu] > 255) return 0;  // dom_bc packs the block coordinates into 8 bits each
+    int nfc = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        if (fg.nblk[mu] > 255) return 0;                // dom_bc packs the block coordinates into 8 bits each
+        if (fg.c[mu] > 1 && fg.sb[mu] < 2) return 0;    // a site has at most one receiver in another CTA per direction
+        nfc = fg.ns / fg.sb[mu] > nfc ? fg.ns / fg.sb[mu] : nfc;
+    }
+    nfc = (nfc + 7) / 8 * 8;
     int smem_max = 0, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const size_t smem = cl16_smem(fg.nsp, fg.C).bytes;
+    const size_t smem = cl16_smem(fg.nsp, fg.C, nfc).bytes;
     if (smem > (size_t)smem_max) return 0;
     int nclus = 0;
     for (int chain = 0; chain < 2; chain++) {
@@ -551,6 +597,7 @@ int ras_cl16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<f
     ctx->dom_bc = reinterpret_cast<unsigned*>(ctx->dom_org + nd);
     ctx->cta16_smem = smem;
     ctx->cl16_nclus = nclus;
+    ctx->cl16_nfc = nfc;
     pack_cl16_kernel<<<(unsigned)nchunk, fg.nsp, 0, ctx->stream>>>(fg, nd, f, ctx->dm16, ctx->dom_org, ctx->dom_bc);
     ctx->launches++;
     if (cudaGetLastError() != cudaSuccess) return 0;
@@ -568,7 +615,7 @@ int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu
 // v = K_RAS r with NRAS chained cycles (overlap 0): one launch per cycle, no full-lattice D in between (reading A3);
 // rho_fin travels domain-major through ctx->rf_dm, the halo buffer alternates between its two parities
 int ras_cl16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
-    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;
+    const int nras = ctx->ras.nras, nd = ctx->ras.nd, nface = ctx->nface;  // nface = C * nfc: CTA-major halo slots
     if (int rc = ensure_halo(ctx, 1)) return rc;
     float4* rf = ctx->rf_dm;
     const size_t hstride = (size_t)24 * nface * nd;

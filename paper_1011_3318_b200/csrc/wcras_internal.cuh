@@ -190,6 +190,7 @@ struct wcras_ctx {
     int dslash_rounded = 0;        // the next fp32 dslash applies the rounded operator (r -= D~ v inside K_RAS)
     int cta_grid = 0;              // its persistent grid size
     int cl16_nclus = 0;            // ras_cl16: clusters resident at once
+    int cl16_nfc = 0;              //           padded size of the largest face of a sub-block (halo slots are CTA-major)
     float4* hb = nullptr;          // halo buffers of the chained K_RAS cycles: [2][nd][8][3][nface]
     int nface = 0;
     int hb_nrhs = 0;               // stack depth the halo buffers are allocated for
