@@ -34,7 +34,7 @@ TOL = 1e-12
 # the paper's parameter survey (NRAS x N_dominv, here also over the domain shape and the operand
 # storage) as found by wcras_ras_autotune on B200: it is NOT one of the two shapes configs[3] names; those are timed
 # beside it (solve.named_shapes) and in the same interleaved loop as the unpreconditioned solve.
-RAS = dict(domain=(4, 4, 4, 4), overlap=0, block_iters=2, nras=3)
+RAS = dict(domain=(4, 4, 4, 4), overlap=0, block_iters=2, nras=4)
 OPERAND_BITS = 16   # block-solver operand storage of the timed step (reading R1); 32 is reported beside it
 # the domain shapes configs[3] names, each at a few (N_dominv, NRAS) points of the paper's survey; the
 # fastest point of every shape is what `ras_named_shapes_faster_than_no_prec` compares with the unpreconditioned solve
@@ -368,14 +368,15 @@ def main():
     # algorithmic HBM bytes per site of one block-solver launch: operands + residual in + v out,
     # chained cycles add rho_fin, the halo slots (96 B per site each way at 4^4: every face site) and the phi read-modify-write
     ob = 288 if OPERAND_BITS == 16 else 576
-    cyc_bytes = [ob + 96 + 96 + 96 + 96, ob + 96 + 96 + 96 + 96 + 192, ob + 96 + 96 + 192]   # cycle 0, middle, last (NRAS = 3)
+    nmid = max(0, RAS["nras"] - 2)
+    cyc_bytes = [ob + 96 + 96 + 96 + 96] + [ob + 96 + 96 + 96 + 96 + 192] * nmid + [ob + 96 + 96 + 192]   # cycle 0, middle, last
     blk_bytes_in_solve = float(np.mean(cyc_bytes))
     blk_bytes_plain = ob + 96 + 96
     # the same launches against the FP32 pipe: 648 packed-pair instructions (FFMA2 / FADD2 / FMUL2, two
     # lane-cycles each) per site and MR sweep, 108 more per site for the boundary coupling of a chained cycle (60 in, 48 out)
     sm_hz = 1e6 * float((clocks or {}).get("sm_mhz") or peaks_json.get("sm_max_mhz") or 1965.0)
     alu_peak = 148 * 128 * sm_hz                                      # FP32 lane-cycles per second
-    alu_cycles = [2.0 * (648 * RAS["block_iters"] + c) for c in (48, 108, 60)]   # cycle 0 (halo out), middle, last (halo in)
+    alu_cycles = [2.0 * (648 * RAS["block_iters"] + c) for c in [48] + [108] * nmid + [60]]   # cycle 0 (halo out), middle, last (halo in)
     alu_cycles_in_solve = float(np.mean(alu_cycles))
 
     if rank != 0:

@@ -56,6 +56,16 @@ __global__ void __launch_bounds__(RED_THREADS) k_init(size_t n, const Vec* __res
     }
 }
 
+// the same scalar reset when |b|^2 is already known (the outer solver: |eta|^2 and the true-residual norms are computed anyway)
+__global__ void k_init_known(Scalars* sc, double bb, double tol, double tiny, int half) {
+    sc->bb = bb; sc->rr = bb; sc->ss = bb;
+    sc->rho[0] = bb; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
+    sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+    sc->thresh = tol * tol; sc->tiny = tiny; sc->half = half;
+    sc->flag = bb > 0 ? 0 : 1;
+    sc->it_done = 0; sc->half_exit = 0;
+}
+
 // restart: rt = r, p = v = 0, rho = <r,r>, rho_old = alpha = omega = 1
 template <typename T, typename Vec>
 __global__ void __launch_bounds__(RED_THREADS) k_restart(size_t n, const Vec* __restrict__ r, Vec* rt, Vec* p, Vec* v, Scalars* sc,
@@ -81,25 +91,22 @@ __global__ void __launch_bounds__(RED_THREADS) k_restart(size_t n, const Vec* __
     }
 }
 
-// p = r + beta (p - omega v), beta = (rho/rho_old)(alpha/omega)
+// pout = r + beta (pin - omega v), beta = (rho/rho_old)(alpha/omega).  pin == pout in general; in the second iteration pin
+// is b: the first iteration has p = r = b and works on b itself instead of on a copy.
 template <typename T, typename Vec>
-__global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* __restrict__ r, Vec* __restrict__ p,
-                                                          const Vec* __restrict__ v, const Scalars* __restrict__ sc, int first) {
+__global__ void __launch_bounds__(RED_THREADS) k_update_p(size_t n, const Vec* __restrict__ r, const Vec* pin, Vec* pout,
+                                                          const Vec* __restrict__ v, const Scalars* __restrict__ sc) {
     constexpr int N = Cx<Vec>::N;
     if (sc->flag) return;
-    if (first) {  // p = v = 0 before the first iteration: p = r (= b), nothing else is read
-        GRID_STRIDE(k, n) p[k] = r[k];
-        return;
-    }
     const cd b = cmul(cdiv({sc->rho[0], sc->rho[1]}, {sc->rho_old[0], sc->rho_old[1]}),
                       cdiv({sc->alpha[0], sc->alpha[1]}, {sc->omega[0], sc->omega[1]}));
     const cpx<T> beta = {(T)b.r, (T)b.i}, omega = ld_scalar<T>(sc->omega);
     GRID_STRIDE(k, n) {
         cpx<T> rc[N], pc[N], vc[N];
-        unpack<T>(r[k], rc); unpack<T>(p[k], pc); unpack<T>(v[k], vc);
+        unpack<T>(r[k], rc); unpack<T>(pin[k], pc); unpack<T>(v[k], vc);
 #pragma unroll
         for (int j = 0; j < N; j++) pc[j] = rc[j] + beta * (pc[j] - omega * vc[j]);
-        p[k] = pack(pc, (Vec*)nullptr);
+        pout[k] = pack(pc, (Vec*)nullptr);
     }
 }
 
@@ -212,8 +219,8 @@ __global__ void __launch_bounds__(RED_THREADS) k_norm2_d(size_t n, const double2
 // out32 = in64 / sqrt(nrm).  fp32 SoA chunk c4 of site i (float4 [6][V]) holds the complex components 2*c4 and
 // 2*c4+1, which live in fp64 SoA chunks 2*c4 and 2*c4+1 of the same site (double2 [12][V]).
 __global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, int nr, const double2* __restrict__ in,
-                                                                float4* __restrict__ out, const Scalars* __restrict__ sc) {
-    const double inv = sc->nrm > 0 ? rsqrt(sc->nrm) : 0.0;
+                                                                float4* __restrict__ out, const double* __restrict__ nrm2) {
+    const double inv = *nrm2 > 0 ? rsqrt(*nrm2) : 0.0;
     GRID_STRIDE(k, 6 * V * nr) {
         const size_t r = k / (6 * V), kk = k - r * 6 * V, c4 = kk / V, i = kk - c4 * V;
         const double2* inr = in + r * 12 * V;
@@ -223,8 +230,8 @@ __global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, int nr
 }
 // out64 = in32 * sqrt(nrm)
 __global__ void __launch_bounds__(RED_THREADS) k_f2d_scaled(size_t V, int nr, const float4* __restrict__ in,
-                                                            double2* __restrict__ out, const Scalars* __restrict__ sc) {
-    const double sc_ = sqrt(sc->nrm);
+                                                            double2* __restrict__ out, const double* __restrict__ nrm2) {
+    const double sc_ = sqrt(*nrm2);
     GRID_STRIDE(k, 6 * V * nr) {
         const size_t r = k / (6 * V), kk = k - r * 6 * V, c4 = kk / V, i = kk - c4 * V;
         double2* outr = out + r * 12 * V;
@@ -284,7 +291,7 @@ template <typename T> struct Work {
 // half-step flag is read before K(s).
 template <typename T, typename KFunc>
 static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b, typename VecOf<T>::type* x, double tol, int maxit,
-                    bool half_exit, bool k_identity, KFunc K, int* iters, double* relres) {
+                    bool half_exit, bool k_identity, KFunc K, int* iters, double* relres, double bb_known = -1.0) {
     typedef typename VecOf<T>::type Vec;
     constexpr int RING = 4;
     const size_t n = w.n;
@@ -294,12 +301,17 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
     const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH((k_init<T, Vec>), n, b, w.sc, part, tk, tol, tiny, half_exit ? 1 : 0);
+        if (bb_known >= 0) {
+            k_init_known<<<1, 1, 0, ctx->stream>>>(w.sc, bb_known, tol, tiny, half_exit ? 1 : 0);
+            ctx->launches++;
+        } else {
+            LAUNCH((k_init<T, Vec>), n, b, w.sc, part, tk, tol, tiny, half_exit ? 1 : 0);
+        }
     }
     *iters = 0;
     *relres = 0;
-    Vec* ph = k_identity ? w.p : w.ph;
-    Vec* sh = k_identity ? w.s : w.sh;
+    const Vec* sh = k_identity ? w.s : w.sh;
+    const Vec* pprev = b;  // p of the previous iteration: b after the first one (p = r = b, never copied), then w.p
     const Vec* rt = b;    // shadow residual = initial residual = b (x0 = 0); a restart switches to the copy in w.rt
     const Vec* rcur = b;  // residual read by the first iteration; w.r from the first r = s - omega t on
     // the fp32 launches of this solver carry the device flag so that those enqueued past convergence are no-ops
@@ -326,11 +338,17 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
                 if (best < 0 || h.rr < best) { best = h.rr; it_best = j; }
                 else if (j - it_best >= 10) break;
             }
-            {
+            // K hints (outer solver): whose norm the device already holds -- 1: |p|^2 = |b|^2 (first iteration), 2: |s|^2, 0: none
+            const Vec* pcur = w.p;
+            if (first) {
+                pcur = rcur;  // p = r = b
+            } else {
                 TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_update_p<T, Vec>), n, rcur, w.p, w.v, w.sc, first ? 1 : 0);
+                LAUNCH((k_update_p<T, Vec>), n, rcur, pprev, w.p, w.v, w.sc);
+                pprev = w.p;
             }
-            if (!k_identity) if (int rc = K(w.p, ph)) return rc;
+            const Vec* ph = k_identity ? pcur : w.ph;
+            if (!k_identity) if (int rc = K(pcur, w.ph, first ? 1 : 0)) return rc;
             if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
             {
                 TimedRegion tr(ctx, TC_BLAS);
@@ -342,7 +360,7 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
                 half_now = ctx->sc_host->flag == 2;
             }
             if (!half_now) {
-                if (!k_identity) if (int rc = K(w.s, sh)) return rc;
+                if (!k_identity) if (int rc = K(w.s, w.sh, 2)) return rc;
                 if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
             }
             {
@@ -370,6 +388,7 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
             LAUNCH((k_restart<T, Vec>), n, rcur, w.rt, w.p, w.v, w.sc, part, tk);
             rt = w.rt;
             first = false;  // p = v = 0 are stored now: the general p update applies
+            pprev = w.p;
             enq = h.it_done;
             best = -1;
             continue;
@@ -454,14 +473,16 @@ static Work<double> work64(wcras_ctx* ctx) {
 }
 
 // inner solve as the outer preconditioner: out64 ~= D^-1 in64
-static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int* inner_iters, int* inner_solves) {
+// hint: which scalar of the outer solver already holds |in64|^2 (1: bb, 2: ss), or 0: compute it (nrm)
+static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int hint, int* inner_iters, int* inner_solves) {
     const size_t V = ctx->geom.V;
     float4* b32 = ctx->w32[8];
     float4* x32 = ctx->w32[9];
+    const double* nrm2 = hint == 1 ? &ctx->sc64->bb : hint == 2 ? &ctx->sc64->ss : &ctx->sc64->nrm;
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH(k_norm2_d, (size_t)12 * V * ctx->nrhs, in64, ctx->sc64, ctx->partials, ctx->ticket);
-        LAUNCH(k_d2f_normalised, V, ctx->nrhs, in64, b32, ctx->sc64);
+        if (hint == 0) LAUNCH(k_norm2_d, (size_t)12 * V * ctx->nrhs, in64, ctx->sc64, ctx->partials, ctx->ticket);
+        LAUNCH(k_d2f_normalised, V, ctx->nrhs, in64, b32, nrm2);
     }
     // Tolerance of this inner solve (reading A2): the outer residual after this preconditioner call is
     // about (inner accuracy) x |in|, so the reduction still missing is R = target/|in|.  It is spread evenly over
@@ -469,7 +490,7 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
     // accuracy fp32 can deliver), instead of solving every call to inner_tol and overshooting the target.
     if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
     double itol = ctx->inner_tol;
-    const double in_norm = std::sqrt(ctx->sc_host->nrm);
+    const double in_norm = std::sqrt(hint == 1 ? ctx->sc_host->bb : hint == 2 ? ctx->sc_host->ss : ctx->sc_host->nrm);
     if (ctx->outer_target > 0 && in_norm > 0) {
         const double R = 0.5 * ctx->outer_target / in_norm;
         if (R < 1.0) {
@@ -485,7 +506,7 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
     const bool use_ras = ctx->use_ras && ctx->ras.set;
     int it = 0;
     double rel = 0;
-    auto K = [ctx](const float4* in, float4* out) { return ras_apply(ctx, in, out); };
+    auto K = [ctx](const float4* in, float4* out, int) { return ras_apply(ctx, in, out); };
     int rc = bicgstab<float>(ctx, w, b32, x32, itol, ctx->inner_maxit, true, !use_ras, K, &it, &rel);
     *inner_iters += it;
     *inner_solves += 1;
@@ -493,7 +514,7 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int*
     // an unconverged or broken-down inner solve is still a usable (flexible) preconditioner
     {
         TimedRegion tr(ctx, TC_BLAS);
-        LAUNCH(k_f2d_scaled, V, ctx->nrhs, x32, out64, ctx->sc64);
+        LAUNCH(k_f2d_scaled, V, ctx->nrhs, x32, out64, nrm2);
     }
     return WCRAS_OK;
 }
@@ -535,7 +556,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         WC_CUDA(cudaMemsetAsync(phi, 0, sizeof(double2) * n64, ctx->stream));
     }
     Work<double> w = work64(ctx);
-    auto K = [&](const double2* in, double2* out) { return inner_solve(ctx, in, out, &inner_iters, &inner_solves); };
+    auto K = [&](const double2* in, double2* out, int hint) { return inner_solve(ctx, in, out, hint, &inner_iters, &inner_solves); };
     for (int pass = 0; pass < 10 && status != WCRAS_OK && outer < ctx->outer_maxit; pass++) {
         int it = 0;
         double rel = 0;
@@ -544,8 +565,11 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         ctx->outer_target = tol_pass * std::sqrt(rn2);  // absolute |r| this pass has to reach
         // pass 0: phi = 0 and res = eta, so the solver works on eta and writes phi directly; later passes solve
         // D dx = res for the correction and add it
-        int rc = pass == 0 ? bicgstab<double>(ctx, w, eta, phi, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel)
-                           : bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel);
+        // |b|^2 is known (|eta|^2, then the norm of the true residual): no reduction pass to start the solver.  (Stacked
+        // systems, pass 0: the unit norms of the scaled eta_k are exact only up to rounding, so it is computed.)
+        const double bb = pass == 0 ? (nr == 1 ? en2 : -1.0) : rn2;
+        int rc = pass == 0 ? bicgstab<double>(ctx, w, eta, phi, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel, bb)
+                           : bicgstab<double>(ctx, w, res, dx, tol_pass, ctx->outer_maxit - outer, true, false, K, &it, &rel, bb);
         if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
         outer += it;
         recur = rel * std::sqrt(rn2 / en2);

@@ -620,16 +620,16 @@ def test_full_size_32_sampled(prec):
 
 
 def test_full_size_32_ras_apply():
-    """K_RAS at full size in the launch configuration bench.py times (4^4 domains, overlap 0, N_dominv 2, NRAS 3:
+    """K_RAS at full size in the launch configuration bench.py times (4^4 domains, overlap 0, N_dominv 2, NRAS 4:
     persistent one-CTA-per-domain kernel, 4096 domains over 148 CTAs, chained cycles) against the oracle's Alg. 1 on
     every site; the same with the cycles not chained (full-lattice D between them)."""
     cs = case(3)
     r = I.spinor(cs.dims, 77)
     r32 = r.astype(np.complex64).astype(np.complex128)
-    want = cs.op.ras_apply((4, 4, 4, 4), 0, 2, 3, r32)
+    want = cs.op.ras_apply((4, 4, 4, 4), 0, 2, 4, r32)
     for tier in (0, 4):
         cs.ctx.set_ras_tier(tier)
-        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 4)
         got = cs.ras_apply(r32)
         assert rel(got, want) <= TOL_RAS
         assert np.abs(got - want).max() / np.abs(want).max() <= 10 * TOL_RAS
@@ -637,9 +637,9 @@ def test_full_size_32_ras_apply():
     # the same point with fp16 operand storage (the staged kernel bench.py times), against the oracle's own rounding
     cs.ctx.set_operand_precision(16)
     try:
-        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 3)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 2, 4)
         got = cs.ras_apply(r32)
-        want16 = rounded_op(cs).ras_apply((4, 4, 4, 4), 0, 2, 3, r32)
+        want16 = rounded_op(cs).ras_apply((4, 4, 4, 4), 0, 2, 4, r32)
         assert rel(got, want16) <= TOL_RAS
         assert np.abs(got - want16).max() / np.abs(want16).max() <= 10 * TOL_RAS
         assert rel(want16, want) > 2e-5
