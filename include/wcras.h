@@ -12,7 +12,8 @@
  *     returns (wcras_create copies the gauge field into its own layouts, so it may be freed afterwards).
  *   - Canonical layouts at the boundary: site index i = x + Lx*(y + Ly*(z + Lz*t)), mu = 0..3 = x,y,z,t.
  *       gauge  [V][4][3][3][2]  fp64, (U psi)_a = sum_b U[a][b] psi_b, {re,im} innermost
- *       spinor [V][4][3][2]     spin, colour, {re,im}; fp32 or fp64 as stated per call
+ *       spinor [V][4][3][2]     spin, colour, {re,im}; fp32 or fp64 as stated per call; 16-byte aligned
+ *                               (WCRAS_INVALID_ARG otherwise)
  *     The internal coalesced SoA layouts (north_star (a)) are private to the library.
  *   - All work is enqueued on the CUDA stream given to wcras_create.  wcras_solve* and wcras_time_kernel
  *     synchronise that stream before returning; the apply_* calls do not.

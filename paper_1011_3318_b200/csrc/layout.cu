@@ -124,29 +124,34 @@ __global__ void export_clover_kernel(int V, const double2* __restrict__ c64, dou
     }
 }
 
-// canonical [V][24] <-> SoA; one thread per (site, chunk)
+// canonical [V][24] <-> SoA [CH][V] through a shared-memory tile of LAYOUT_TS sites: both the canonical side (a site's 24
+// reals contiguous) and the SoA side (a chunk's sites contiguous) are then read and written as whole 16-byte rows
+constexpr int LAYOUT_TS = 64;
 template <typename T, typename Vec, int CH>
-__global__ void spinor_to_internal_kernel(int V, const T* __restrict__ canon, Vec* __restrict__ soa) {
-    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (size_t)V * CH) return;
-    const size_t i = t / CH, c = t % CH;
-    constexpr int W = 24 / CH;
-    const T* s = canon + i * 24 + c * W;
-    Vec v;
-    if constexpr (W == 4) { v.x = s[0]; v.y = s[1]; v.z = s[2]; v.w = s[3]; }
-    else { v.x = s[0]; v.y = s[1]; }
-    soa[c * V + i] = v;
+__global__ void __launch_bounds__(256) spinor_to_internal_kernel(int V, const T* __restrict__ canon, Vec* __restrict__ soa) {
+    __shared__ Vec tile[LAYOUT_TS * CH];
+    const size_t i0 = (size_t)blockIdx.x * LAYOUT_TS;
+    const int ns = (int)((size_t)V - i0 < (size_t)LAYOUT_TS ? (size_t)V - i0 : (size_t)LAYOUT_TS);
+    const Vec* src = reinterpret_cast<const Vec*>(canon) + i0 * CH;  // element e = local site * CH + chunk
+    for (int e = threadIdx.x; e < ns * CH; e += blockDim.x) tile[e] = src[e];
+    __syncthreads();
+    for (int e = threadIdx.x; e < LAYOUT_TS * CH; e += blockDim.x) {
+        const int c = e / LAYOUT_TS, sl = e % LAYOUT_TS;
+        if (sl < ns) soa[(size_t)c * V + i0 + sl] = tile[sl * CH + c];
+    }
 }
 template <typename T, typename Vec, int CH>
-__global__ void spinor_from_internal_kernel(int V, const Vec* __restrict__ soa, T* __restrict__ canon) {
-    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (size_t)V * CH) return;
-    const size_t i = t / CH, c = t % CH;
-    constexpr int W = 24 / CH;
-    T* s = canon + i * 24 + c * W;
-    const Vec v = soa[c * V + i];
-    if constexpr (W == 4) { s[0] = v.x; s[1] = v.y; s[2] = v.z; s[3] = v.w; }
-    else { s[0] = v.x; s[1] = v.y; }
+__global__ void __launch_bounds__(256) spinor_from_internal_kernel(int V, const Vec* __restrict__ soa, T* __restrict__ canon) {
+    __shared__ Vec tile[LAYOUT_TS * CH];
+    const size_t i0 = (size_t)blockIdx.x * LAYOUT_TS;
+    const int ns = (int)((size_t)V - i0 < (size_t)LAYOUT_TS ? (size_t)V - i0 : (size_t)LAYOUT_TS);
+    for (int e = threadIdx.x; e < LAYOUT_TS * CH; e += blockDim.x) {
+        const int c = e / LAYOUT_TS, sl = e % LAYOUT_TS;
+        if (sl < ns) tile[sl * CH + c] = soa[(size_t)c * V + i0 + sl];
+    }
+    __syncthreads();
+    Vec* dst = reinterpret_cast<Vec*>(canon) + i0 * CH;
+    for (int e = threadIdx.x; e < ns * CH; e += blockDim.x) dst[e] = tile[e];
 }
 
 int setup_fields(wcras_ctx* ctx, const double* gauge_dev) {
@@ -177,11 +182,12 @@ int setup_fields(wcras_ctx* ctx, const double* gauge_dev) {
 
 int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal) {
     const int V = ctx->geom.V, T = 256;
+    if ((uintptr_t)canonical & 15) { snprintf(ctx->err, sizeof ctx->err, "spinor buffers must be 16-byte aligned"); return WCRAS_INVALID_ARG; }
     if (prec == 32)
-        spinor_to_internal_kernel<float, float4, 6><<<(unsigned)(((size_t)V * 6 + T - 1) / T), T, 0, ctx->stream>>>(
+        spinor_to_internal_kernel<float, float4, 6><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
             V, (const float*)canonical, (float4*)internal);
     else
-        spinor_to_internal_kernel<double, double2, 12><<<(unsigned)(((size_t)V * 12 + T - 1) / T), T, 0, ctx->stream>>>(
+        spinor_to_internal_kernel<double, double2, 12><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
             V, (const double*)canonical, (double2*)internal);
     ctx->launches++;
     WC_CHECK_LAUNCH();
@@ -190,11 +196,12 @@ int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal)
 
 int from_internal(wcras_ctx* ctx, int prec, const void* internal, void* canonical) {
     const int V = ctx->geom.V, T = 256;
+    if ((uintptr_t)canonical & 15) { snprintf(ctx->err, sizeof ctx->err, "spinor buffers must be 16-byte aligned"); return WCRAS_INVALID_ARG; }
     if (prec == 32)
-        spinor_from_internal_kernel<float, float4, 6><<<(unsigned)(((size_t)V * 6 + T - 1) / T), T, 0, ctx->stream>>>(
+        spinor_from_internal_kernel<float, float4, 6><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
             V, (const float4*)internal, (float*)canonical);
     else
-        spinor_from_internal_kernel<double, double2, 12><<<(unsigned)(((size_t)V * 12 + T - 1) / T), T, 0, ctx->stream>>>(
+        spinor_from_internal_kernel<double, double2, 12><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
             V, (const double2*)internal, (double*)canonical);
     ctx->launches++;
     WC_CHECK_LAUNCH();

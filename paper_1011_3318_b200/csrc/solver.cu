@@ -216,17 +216,34 @@ __global__ void __launch_bounds__(RED_THREADS) k_norm2_d(size_t n, const double2
     if (grid_reduce<1>(acc, partials, ticket, tot)) sc->nrm = tot[0];
 }
 
-// out32 = in64 / sqrt(nrm).  fp32 SoA chunk c4 of site i (float4 [6][V]) holds the complex components 2*c4 and
-// 2*c4+1, which live in fp64 SoA chunks 2*c4 and 2*c4+1 of the same site (double2 [12][V]).
-__global__ void __launch_bounds__(RED_THREADS) k_d2f_normalised(size_t V, int nr, const double2* __restrict__ in,
-                                                                float4* __restrict__ out, const double* __restrict__ nrm2) {
+// out32 = in64 / sqrt(nrm2), and the start of the inner solver on out32 in the same pass: bb = |out32|^2 from the rounded fp32
+// values (what k_init would compute from them), scalars reset; the tolerance follows by k_set_tol once the host has it.
+// fp32 SoA chunk c4 of site i (float4 [6][V]) holds the complex components 2*c4 and 2*c4+1, which live in fp64 SoA chunks
+// 2*c4 and 2*c4+1 of the same site (double2 [12][V]).
+__global__ void __launch_bounds__(RED_THREADS) k_d2f_init(size_t V, int nr, const double2* __restrict__ in, float4* __restrict__ out,
+                                                          const double* __restrict__ nrm2, Scalars* sc, double* partials,
+                                                          unsigned* ticket) {
     const double inv = *nrm2 > 0 ? rsqrt(*nrm2) : 0.0;
+    double acc[1] = {0};
     GRID_STRIDE(k, 6 * V * nr) {
         const size_t r = k / (6 * V), kk = k - r * 6 * V, c4 = kk / V, i = kk - c4 * V;
         const double2* inr = in + r * 12 * V;
         const double2 a = inr[(2 * c4) * V + i], b = inr[(2 * c4 + 1) * V + i];
-        out[k] = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
+        const float4 o = make_float4((float)(a.x * inv), (float)(a.y * inv), (float)(b.x * inv), (float)(b.y * inv));
+        out[k] = o;
+        acc[0] += (double)o.x * o.x + (double)o.y * o.y + (double)o.z * o.z + (double)o.w * o.w;
     }
+    double tot[1];
+    if (grid_reduce<1>(acc, partials, ticket, tot)) {
+        sc->bb = tot[0]; sc->rr = tot[0]; sc->ss = tot[0];
+        sc->rho[0] = tot[0]; sc->rho[1] = 0; sc->rho_old[0] = 1; sc->rho_old[1] = 0;
+        sc->alpha[0] = 1; sc->alpha[1] = 0; sc->omega[0] = 1; sc->omega[1] = 0;
+        sc->flag = tot[0] > 0 ? 0 : 1;
+        sc->it_done = 0; sc->half_exit = 0;
+    }
+}
+__global__ void k_set_tol(Scalars* sc, double tol, double tiny, int half) {
+    sc->thresh = tol * tol; sc->tiny = tiny; sc->half = half;
 }
 // out64 = in32 * sqrt(nrm)
 __global__ void __launch_bounds__(RED_THREADS) k_f2d_scaled(size_t V, int nr, const float4* __restrict__ in,
@@ -301,7 +318,10 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
     const double tiny = sizeof(T) == 4 ? 1e-30 : 1e-290;
     {
         TimedRegion tr(ctx, TC_BLAS);
-        if (bb_known >= 0) {
+        if (bb_known == -2.0) {  // scalars already reset by the kernel that produced b (k_d2f_init)
+            k_set_tol<<<1, 1, 0, ctx->stream>>>(w.sc, tol, tiny, half_exit ? 1 : 0);
+            ctx->launches++;
+        } else if (bb_known >= 0) {
             k_init_known<<<1, 1, 0, ctx->stream>>>(w.sc, bb_known, tol, tiny, half_exit ? 1 : 0);
             ctx->launches++;
         } else {
@@ -482,7 +502,7 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int 
     {
         TimedRegion tr(ctx, TC_BLAS);
         if (hint == 0) LAUNCH(k_norm2_d, (size_t)12 * V * ctx->nrhs, in64, ctx->sc64, ctx->partials, ctx->ticket);
-        LAUNCH(k_d2f_normalised, V, ctx->nrhs, in64, b32, nrm2);
+        LAUNCH(k_d2f_init, V, ctx->nrhs, in64, b32, nrm2, ctx->sc32, ctx->partials, ctx->ticket);
     }
     // Tolerance of this inner solve (reading A2): the outer residual after this preconditioner call is
     // about (inner accuracy) x |in|, so the reduction still missing is R = target/|in|.  It is spread evenly over
@@ -507,7 +527,7 @@ static int inner_solve(wcras_ctx* ctx, const double2* in64, double2* out64, int 
     int it = 0;
     double rel = 0;
     auto K = [ctx](const float4* in, float4* out, int) { return ras_apply(ctx, in, out); };
-    int rc = bicgstab<float>(ctx, w, b32, x32, itol, ctx->inner_maxit, true, !use_ras, K, &it, &rel);
+    int rc = bicgstab<float>(ctx, w, b32, x32, itol, ctx->inner_maxit, true, !use_ras, K, &it, &rel, -2.0);
     *inner_iters += it;
     *inner_solves += 1;
     if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
