@@ -340,10 +340,14 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
 static int block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     TimedRegion tr(ctx, TC_BLOCK);
     ctx->block_dv += ctx->ras.niter;
-    if (ctx->ras.tier == 2 && ctx->ras.pair && ctx->nrhs == 1) return ras_pair_block_solve(ctx, r, vout, accum);
-    if (ctx->ras.tier == 2 && ctx->ras.cta16 && ctx->nrhs == 1) return ras_cta16_block_solve(ctx, r, vout, accum);
-    if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
     const size_t rstride = (size_t)6 * ctx->geom.V;
+    if (ctx->ras.tier == 2 && ctx->ras.pair && ctx->nrhs == 1) return ras_pair_block_solve(ctx, r, vout, accum);
+    if (ctx->ras.tier == 2 && ctx->ras.cta16) {  // fp16 operand storage: the staged kernel, one right-hand side of the stack at a time
+        for (int k = 0; k < ctx->nrhs; k++)
+            if (int e = ras_cta16_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)) return e;
+        return WCRAS_OK;
+    }
+    if (ctx->ras.tier == 2 && ctx->ras.cta) return ras_cta_block_solve(ctx, r, vout, accum);  // handles the whole stack
     for (int k = 0; k < ctx->nrhs; k++) {  // cluster and generic tiers: one right-hand side of the stack at a time
         const int e = ctx->ras.tier == 2 ? (ctx->ras.stream ? ras_stream_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
                                             : ctx->ras.cl16 ? ras_cl16_block_solve(ctx, r + k * rstride, vout + k * rstride, accum)
@@ -362,20 +366,34 @@ int ras_apply(wcras_ctx* ctx, const float4* r, float4* v) {
     const RasConfig& rc = ctx->ras;
     if (!rc.set) { snprintf(ctx->err, sizeof ctx->err, "ras_apply: call wcras_ras_precondition first"); return WCRAS_INVALID_ARG; }
     ctx->ras_applies++;
+    const size_t vstride = (size_t)6 * ctx->geom.V;  // stacked right-hand sides (wcras_solve_multi)
     if (ctx->schwarz == 1) {
         if (!(rc.tier == 2 && rc.cta && rc.s == 0 && ctx->fused.pdir >= 0)) {
             snprintf(ctx->err, sizeof ctx->err, "multiplicative Schwarz needs overlap 0, domains of <= 256 sites and an even number of blocks in every cut direction");
             return WCRAS_UNSUPPORTED;
         }
         if (rc.pair && ctx->nrhs == 1) return ras_pair_apply_sap(ctx, r, v);
-        return rc.cta16 && ctx->nrhs == 1 ? ras_cta16_apply_sap(ctx, r, v) : ras_cta_apply_sap(ctx, r, v);
+        if (rc.cta16) {
+            for (int k = 0; k < ctx->nrhs; k++)
+                if (int e = ras_cta16_apply_sap(ctx, r + k * vstride, v + k * vstride)) return e;
+            return WCRAS_OK;
+        }
+        return ras_cta_apply_sap(ctx, r, v);
     }
     if (rc.nras == 1) return block_solve(ctx, r, v, false);
     // overlap 0 on the persistent-CTA tier: chained cycles, the residual update is the boundary coupling only
     if (rc.tier == 2 && rc.pair && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_pair_apply_chained(ctx, r, v);
-    if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cta16_apply_chained(ctx, r, v);
+    if (rc.tier == 2 && rc.cta16 && rc.s == 0 && ctx->chain_cycles) {  // stacked right-hand sides: one after the other
+        for (int k = 0; k < ctx->nrhs; k++)
+            if (int e = ras_cta16_apply_chained(ctx, r + k * vstride, v + k * vstride)) return e;
+        return WCRAS_OK;
+    }
     if (rc.tier == 2 && rc.cta && rc.s == 0 && ctx->chain_cycles) return ras_cta_apply_chained(ctx, r, v);
-    if (rc.tier == 2 && rc.cl16 && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_cl16_apply_chained(ctx, r, v);
+    if (rc.tier == 2 && rc.cl16 && rc.s == 0 && ctx->chain_cycles) {
+        for (int k = 0; k < ctx->nrhs; k++)
+            if (int e = ras_cl16_apply_chained(ctx, r + k * vstride, v + k * vstride)) return e;
+        return WCRAS_OK;
+    }
     if (rc.tier == 2 && !rc.cta && !rc.stream && rc.s == 0 && ctx->chain_cycles && ctx->nrhs == 1) return ras_fused_apply_chained(ctx, r, v);
     float4* rw = ctx->ras32[0];
     float4* vj = ctx->ras32[1];
