@@ -44,8 +44,8 @@ SAP = dict(domain=(4, 4, 4, 4), block_iters=3, ncycle=2)
 INNER_TOL = 5e-7
 REFERENCE_BUDGET_S = 150.0   # wall-clock budget of the --impl reference arm
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
-# `ncu --set full` capture (profiles/r1j_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
-DSLASH_TRAFFIC_NCU_BYTES = 810.3e6
+# `ncu --set full` capture (profiles/r2_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
+DSLASH_TRAFFIC_NCU_BYTES = 812.2e6
 KEYS = ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies", "rel_resid_true",
         "ms_total")
 
@@ -512,6 +512,12 @@ def main():
                   "ras_faster_than_no_prec": float(np.median(pair["ras"])) < float(np.median(pair["no_prec"])),
                   "ras_named_shapes_faster_than_no_prec": named_faster,
                   "named_shapes": side},
+        # vector passes (96 B per site each) of one inner BiCGStab iteration in its right-preconditioned form (p^, s^ stored):
+        # SURVEY.md 8(d) budgets 10-12 for the fused form against ~19 unfused
+        "blas_vector_passes_per_inner_iteration": {"k_update_p": 4, "k_update_s": 3, "k_update_xr": 8, "dot_operands_read_by_the_two_dslash": 2,
+                                                   "total": 17, "unfused_same_recurrence": 24,
+                                                   "note": "r,p,v->p; r,v->s (+|s|^2); x,p^,s^,s,t,rt->x,r (+<rt,r>,|r|^2); <rt,v> and <t,s>,<t,t> "
+                                                           "ride on the Dslash that produces v and t; the first iteration skips k_update_p (p = b)"},
         "kernels": {"dslash_fp32_ms": ms_d32, "dslash_fp64_ms": ms_d64,
                     "dslash_fp64_gbs": 1536.0 * V / (ms_d64 * 1e-3) / 1e9,
                     "block_solve_ms": ms_blk,

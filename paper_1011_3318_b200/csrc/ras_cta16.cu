@@ -23,7 +23,6 @@
 //   * Shared memory at nsp = 256: 96 KB half-spinor slots + 72 KB operands + 24 KB residual + 24 KB halo = 216 KB.
 // Roofline: HBM; algorithmic bytes per site and launch 288 operands + 96 residual in + 96 out (+ 96 rho_fin, + halo).
 #include <cuda_fp16.h>
-#include <stdlib.h>
 
 #include "ras_cta_common.cuh"
 
@@ -499,17 +498,7 @@ int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<
             if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg.nsp), fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
             if (n > best) { best = n; stage_halo = sh; smem = b; }
         }
-        if (const char* e = getenv("WCRAS_CTA16_STAGE_HALO")) {  // experiment switch
-            const int sh = atoi(e);
-            const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
-            if (b <= (size_t)smem_max) {
-                int n = 0;
-                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg.nsp), fg.nsp, b);
-                if (n >= 1) { best = n; stage_halo = sh; smem = b; }
-            }
-        }
         per_sm = best;
-        if (getenv("WCRAS_DEBUG")) fprintf(stderr, "cta16: nsp %d nface %d stage_halo %d smem %zu per_sm %d\n", fg.nsp, nface, stage_halo, smem, per_sm);
         if (per_sm < 1) return 0;
         cudaFuncSetAttribute(cta16_kernel(false, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         cudaFuncSetAttribute(cta16_kernel(true, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
