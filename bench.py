@@ -203,6 +203,26 @@ def oracle_table(torch, binding, I, O, config4=False):
             if cid != 4:
                 a = p.cpu().numpy()
                 g[key]["oracle_rel_resid_true"] = float(op.true_residual(eta, (a[..., 0] + 1j * a[..., 1]).reshape(V, 4, 3)))
+        # every RAS point BASELINE.json:configs[cid] names (configs[1]: overlap 0 and 1; configs[2]: 4^4 vs 8x4x4x4, overlap
+        # 0/1/2, block iterations 2-8), GPU solves with the oracle's residual of every solution; NRAS 1, fp32 operands
+        if cid != 4:
+            sweep = {}
+            iters = (2, 4, 6, 8) if cid == 2 else (cfg["ras"][0]["block_iters"],)
+            ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+            for rr in cfg["ras"]:
+                for nit in iters:
+                    ctx.ras_precondition(rr["domain"], rr["overlap"], nit, 1)
+                    ctx.solve(e, p, TOL)
+                    ms = []
+                    for _ in range(3):
+                        i = ctx.solve(e, p, TOL)
+                        ms.append(i["ms_total"])
+                    a = p.cpu().numpy()
+                    sweep["ras_%s_s%d_it%d" % ("x".join(map(str, rr["domain"])), rr["overlap"], nit)] = {
+                        "ms_total": float(np.median(ms)), "inner_iters": i["inner_iters"], "ras_applies": i["ras_applies"],
+                        "rel_resid_true": i["rel_resid_true"],
+                        "oracle_rel_resid_true": float(op.true_residual(eta, (a[..., 0] + 1j * a[..., 1]).reshape(V, 4, 3)))}
+            g["named_points"] = sweep
         row["gpu"] = g
         out["config%d" % cid] = row
         del ctx, e, p

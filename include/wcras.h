@@ -141,6 +141,12 @@ int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int oute
  * the price of up to n no-op iterations after convergence.  Results are identical for every value. */
 int wcras_set_lookahead(wcras_ctx* ctx, int iterations);
 
+/* CUDA graphs for the inner solver (default on): one inner fp32 BiCGStab iteration (10-14 kernel launches, the
+ * inner solver "does most of arithmetics") is captured the second time it runs with the same vectors and configuration and
+ * replayed afterwards, which removes the host's launch cost from small lattices.  Results are identical either way; every
+ * call that changes the configuration discards the captured graphs.  Off while wcras_set_timing(1) is in force. */
+int wcras_set_graphs(wcras_ctx* ctx, int enable);
+
 /* Per-kernel-class CUDA-event timing inside wcras_solve (fills ms_dslash / ms_blocksolve / ms_blas). */
 int wcras_set_timing(wcras_ctx* ctx, int enable);
 

@@ -17,7 +17,7 @@ OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, 
 
 EXPORTS = [
     "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_ras_precondition", "wcras_set_ras_tier", "wcras_set_operand_precision", "wcras_set_schwarz", "wcras_set_traversal",
-    "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_lookahead", "wcras_set_timing", "wcras_solve",
+    "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_lookahead", "wcras_set_graphs", "wcras_set_timing", "wcras_solve",
     "wcras_solve_host", "wcras_solve_multi", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
 ]
 
@@ -148,6 +148,9 @@ class Context:
 
     def set_lookahead(self, iterations):
         self._chk(self._lib.wcras_set_lookahead(self._h, C.c_int(iterations)))
+
+    def set_graphs(self, enable):
+        self._chk(self._lib.wcras_set_graphs(self._h, C.c_int(1 if enable else 0)))
 
     def set_timing(self, enable):
         self._chk(self._lib.wcras_set_timing(self._h, C.c_int(1 if enable else 0)))

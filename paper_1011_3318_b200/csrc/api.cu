@@ -50,6 +50,8 @@ int wcras_create(wcras_ctx** out, const int dims[4], double kappa, double csw, c
 int wcras_destroy(wcras_ctx* ctx) {
     if (!ctx) return WCRAS_INVALID_ARG;
     cudaStreamSynchronize(ctx->stream);
+    drop_iter_graphs(ctx);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
     if (ctx->dm) cudaFree(ctx->dm);
@@ -83,6 +85,7 @@ int wcras_ras_precondition(wcras_ctx* ctx, const int domain[4], int overlap_s, i
 
 int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
     NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(tier >= 0 && tier <= 6, "set_ras_tier: tier must be 0..6");
     ctx->tier_request = tier == 4 ? 2 : tier;
     ctx->chain_cycles = tier != 4;
@@ -91,6 +94,7 @@ int wcras_set_ras_tier(wcras_ctx* ctx, int tier) {
 
 int wcras_set_operand_precision(wcras_ctx* ctx, int bits) {
     NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(bits == 32 || bits == 16, "set_operand_precision: bits must be 32 or 16");
     ctx->op_prec = bits;
     return WCRAS_OK;
@@ -98,6 +102,7 @@ int wcras_set_operand_precision(wcras_ctx* ctx, int bits) {
 
 int wcras_set_traversal(wcras_ctx* ctx, int ztile) {
     NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(ztile >= -1 && ztile < ctx->geom.L[2] && (ztile <= 0 || ctx->geom.L[2] % ztile == 0),
          "set_traversal: ztile must be -1 (automatic), 0 (off) or a proper divisor of Lz");
     ctx->ztile_request = ztile;
@@ -106,6 +111,7 @@ int wcras_set_traversal(wcras_ctx* ctx, int ztile) {
 
 int wcras_set_schwarz(wcras_ctx* ctx, int multiplicative) {
     NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(multiplicative == 0 || multiplicative == 1, "set_schwarz: 0 (additive, RAS) or 1 (multiplicative, SAP)");
     ctx->schwarz = multiplicative;
     return WCRAS_OK;
@@ -148,6 +154,7 @@ int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev) {
 
 int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int outer_maxit, int use_ras) {
     NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(inner_tol > 0 && inner_maxit >= 1 && outer_maxit >= 1, "set_solver: tolerances and caps must be positive");
     ctx->inner_tol = inner_tol;
     ctx->inner_maxit = inner_maxit;
@@ -160,6 +167,13 @@ int wcras_set_lookahead(wcras_ctx* ctx, int iterations) {
     NEED(ctx, "null ctx");
     NEED(iterations >= 0 && iterations <= 3, "set_lookahead: 0..3 iterations");
     ctx->lookahead = iterations;
+    return WCRAS_OK;
+}
+
+int wcras_set_graphs(wcras_ctx* ctx, int enable) {
+    NEED(ctx, "null ctx");
+    ctx->use_graphs = enable ? 1 : 0;
+    ctx->cfg_gen++;
     return WCRAS_OK;
 }
 
@@ -184,9 +198,11 @@ int wcras_solve_multi(wcras_ctx* ctx, int nrhs, const double* eta_dev, double* p
     NEED(nrhs >= 1 && nrhs <= 4, "solve_multi: nrhs must be 1..4");
     NEED(tol > 0, "solve_multi: tol must be positive");
     NEED(!ctx->use_ras || ctx->ras.set, "solve_multi: use_ras is set but wcras_ras_precondition was not called");
+    if (nrhs != 1) ctx->cfg_gen++;  // the stack depth changes what an inner iteration launches
     ctx->nrhs = nrhs;
     const int rc = solve(ctx, eta_dev, phi_dev, tol, info, rel_resid_host);
     ctx->nrhs = 1;
+    if (nrhs != 1) ctx->cfg_gen++;
     return rc;
 }
 

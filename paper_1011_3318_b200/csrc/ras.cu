@@ -244,6 +244,7 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     // from here on the buffers of the previous configuration are released: until the new one is complete the context has
     // no preconditioner (an allocation failure below leaves it that way, with the error message, instead of half of each)
     ctx->ras.set = false;
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     FusedGeom fgeom;
     // tier request 5: force the streamed-operand cluster kernel (tier 2c); automatic: 2a/2b when Omega' fits on chip with
     // its operands, else 2c when the spinors fit a cluster, else the generic tier

@@ -297,6 +297,15 @@ template <typename T> struct Work {
     size_t n;
 };
 
+void drop_iter_graphs(wcras_ctx* ctx) {
+    for (auto& g : ctx->iter_graph) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        g = wcras_ctx::IterGraph();
+    }
+    ctx->graph_b = ctx->graph_x = nullptr;
+    ctx->graph_kid = -1;
+}
+
 // BiCGStab driver.  K(in,out) applies the preconditioner (ignored when k_identity).  status: 0 converged,
 // WCRAS_NOT_CONVERGED, WCRAS_BREAKDOWN, or a CUDA error.
 //
@@ -358,35 +367,81 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
                 if (best < 0 || h.rr < best) { best = h.rr; it_best = j; }
                 else if (j - it_best >= 10) break;
             }
-            // K hints (outer solver): whose norm the device already holds -- 1: |p|^2 = |b|^2 (first iteration), 2: |s|^2, 0: none
-            const Vec* pcur = w.p;
-            if (first) {
-                pcur = rcur;  // p = r = b
+            // One iteration = 10-14 launches whose arguments depend only on its kind (0: first, p = r = b, x written; 1: second,
+            // p of the previous iteration is b; 2: every later one).  The fp32 inner solver replays it as a CUDA graph from the
+            // second time a kind runs with the same vectors and configuration (the first time runs eagerly, so that every
+            // lazily allocated buffer exists before a capture): below 16^4 the solve is bound by the host's launch rate.
+            const int kind = first ? 0 : (pprev == b ? 1 : 2);
+            auto body = [&]() -> int {
+                // K hints (outer solver): whose norm the device already holds -- 1: |p|^2 = |b|^2 (first iteration), 2: |s|^2, 0: none
+                const Vec* pcur = w.p;
+                if (kind == 0) {
+                    pcur = rcur;  // p = r = b
+                } else {
+                    TimedRegion tr(ctx, TC_BLAS);
+                    LAUNCH((k_update_p<T, Vec>), n, rcur, pprev, w.p, w.v, w.sc);
+                }
+                const Vec* ph = k_identity ? pcur : w.ph;
+                if (!k_identity) if (int rc = K(pcur, w.ph, kind == 0 ? 1 : 0)) return rc;
+                if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
+                {
+                    TimedRegion tr(ctx, TC_BLAS);
+                    LAUNCH((k_update_s<T, Vec>), n, rcur, w.v, w.s, w.sc, part, tk);
+                }
+                bool half_now = false;
+                if (la == 0 && half_exit) {  // the second half costs a whole inner solve: read the flag first
+                    if (int rc = read_scalars(ctx, w.sc)) return rc;
+                    half_now = ctx->sc_host->flag == 2;
+                }
+                if (!half_now) {
+                    if (!k_identity) if (int rc = K(w.s, w.sh, 2)) return rc;
+                    if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
+                }
+                {
+                    TimedRegion tr(ctx, TC_BLAS);
+                    LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, rt, w.r, w.sc, part, tk, x_written ? 0 : 1);
+                }
+                return WCRAS_OK;
+            };
+            const bool graphable = sizeof(T) == 4 && la > 0 && ctx->use_graphs && !ctx->timing && restarts == 0 && rt == b &&
+                                   (kind == 0) == !x_written;
+            if (graphable) {
+                if (ctx->graph_b != (const void*)b || ctx->graph_x != (const void*)x || ctx->graph_gen != ctx->cfg_gen ||
+                    ctx->graph_kid != (int)k_identity) {
+                    drop_iter_graphs(ctx);
+                    ctx->graph_b = b; ctx->graph_x = x; ctx->graph_gen = ctx->cfg_gen; ctx->graph_kid = (int)k_identity;
+                }
+                wcras_ctx::IterGraph& g = ctx->iter_graph[kind];
+                if (g.exec) {
+                    WC_CUDA(cudaGraphLaunch(g.exec, ctx->stream));
+                    ctx->launches += g.d_launches; ctx->dv32 += g.d_dv32; ctx->block_dv += g.d_blk; ctx->ras_applies += g.d_ras;
+                } else if (g.seen >= 1) {
+                    const long long l0 = ctx->launches;
+                    const int c1[3] = {ctx->dv32, ctx->block_dv, ctx->ras_applies};
+                    if (!ctx->cap_stream) WC_CUDA(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+                    cudaStream_t user = ctx->stream;
+                    WC_CUDA(cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+                    ctx->stream = ctx->cap_stream;  // every launch of the body goes to ctx->stream
+                    const int rc = body();
+                    ctx->stream = user;
+                    cudaGraph_t graph = nullptr;
+                    const cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &graph);
+                    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+                    WC_CUDA(ce);
+                    const cudaError_t ci = cudaGraphInstantiate(&g.exec, graph, 0);
+                    cudaGraphDestroy(graph);
+                    WC_CUDA(ci);
+                    g.d_launches = ctx->launches - l0;
+                    g.d_dv32 = ctx->dv32 - c1[0]; g.d_blk = ctx->block_dv - c1[1]; g.d_ras = ctx->ras_applies - c1[2];
+                    WC_CUDA(cudaGraphLaunch(g.exec, ctx->stream));  // a capture records, it does not execute
+                } else {
+                    g.seen++;
+                    if (int rc = body()) return rc;
+                }
             } else {
-                TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_update_p<T, Vec>), n, rcur, pprev, w.p, w.v, w.sc);
-                pprev = w.p;
+                if (int rc = body()) return rc;
             }
-            const Vec* ph = k_identity ? pcur : w.ph;
-            if (!k_identity) if (int rc = K(pcur, w.ph, first ? 1 : 0)) return rc;
-            if (int rc = dslash<T>(ctx, ph, w.v, nullptr, 1, rt, w.sc)) return rc;  // v = D ph; <rt,v>, alpha fused
-            {
-                TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_update_s<T, Vec>), n, rcur, w.v, w.s, w.sc, part, tk);
-            }
-            bool half_now = false;
-            if (la == 0 && half_exit) {  // the second half costs a whole inner solve: read the flag first
-                if (int rc = read_scalars(ctx, w.sc)) return rc;
-                half_now = ctx->sc_host->flag == 2;
-            }
-            if (!half_now) {
-                if (!k_identity) if (int rc = K(w.s, w.sh, 2)) return rc;
-                if (int rc = dslash<T>(ctx, sh, w.t, nullptr, 2, w.s, w.sc)) return rc;  // t = D sh; <t,s>, <t,t>, omega fused
-            }
-            {
-                TimedRegion tr(ctx, TC_BLAS);
-                LAUNCH((k_update_xr<T, Vec>), n, x, ph, sh, w.s, w.t, rt, w.r, w.sc, part, tk, x_written ? 0 : 1);
-            }
+            if (kind != 0) pprev = w.p;
             x_written = true;
             first = false;
             rcur = w.r;
@@ -461,6 +516,7 @@ int ensure_workspace(wcras_ctx* ctx) {
             for (int k = 0; k < 3; k++) { free_owned(ctx, ctx->ras32[k]); ctx->ras32[k] = nullptr; }
         };
         ctx->ws_nrhs = 0;
+        ctx->cfg_gen++;  // the work vectors move: captured inner-iteration graphs are stale
         release();
         const size_t nr = ctx->nrhs;
         bool ok = true;

@@ -213,6 +213,21 @@ struct wcras_ctx {
     wc::Scalars* sc_ring = nullptr;  // pinned [SC_RING]: per-iteration snapshots the host polls a few iterations late
     cudaEvent_t ev_ring[4] = {nullptr, nullptr, nullptr, nullptr};
     int lookahead = 1;             // inner iterations enqueued ahead of the host's convergence check (0 = check every one)
+    // CUDA graphs of one inner fp32 BiCGStab iteration (solver.cu): kind 0 = first iteration, 1 = second, 2 = every later
+    // one; captured the second time a kind runs with the same vectors and configuration, replayed afterwards
+    struct IterGraph {
+        cudaGraphExec_t exec = nullptr;
+        int seen = 0;
+        long long d_launches = 0;
+        int d_dv32 = 0, d_blk = 0, d_ras = 0;
+    } iter_graph[3];
+    const void* graph_b = nullptr;  // key of the captured graphs: right-hand side and solution vectors, configuration generation
+    const void* graph_x = nullptr;
+    unsigned graph_gen = 0;
+    int graph_kid = -1;            // ... and whether the iteration applies a preconditioner
+    unsigned cfg_gen = 1;          // bumped by every call that changes what an inner iteration launches
+    int use_graphs = 1;
+    cudaStream_t cap_stream = nullptr;  // captures run on this internal stream (the caller's may be the legacy default stream, which cannot capture)
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;
     double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][blocks], slice sums, ticket
@@ -293,6 +308,7 @@ constexpr int RED_THREADS = WC_RED_THREADS;
 
 int alloc_dev(wcras_ctx* ctx, void** p, size_t bytes);
 int ensure_workspace(wcras_ctx* ctx);
+void drop_iter_graphs(wcras_ctx* ctx);  // solver.cu
 
 // layout.cu
 int setup_fields(wcras_ctx* ctx, const double* gauge_dev);

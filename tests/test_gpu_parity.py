@@ -560,6 +560,48 @@ def test_ras_autotune_full_grid():
         cs.ctx.set_solver(use_ras=False)
 
 
+def test_inner_iteration_graphs():
+    """CUDA-graph replay of the inner iterations (wcras_set_graphs): bit-identical solutions and identical counters with and
+    without it, across repeated solves (first solve eager, second captures, later ones replay), for the unpreconditioned
+    solver, the persistent and cluster block solvers, SAP, fp16 operands, and after a reconfiguration in between."""
+    cs = case(2)
+    eta = I.spinor(cs.dims, 11)
+    x = dev(eta, torch.float64)
+
+    def run():
+        phi = torch.empty_like(x)
+        info = cs.ctx.solve(x, phi, 1e-12)
+        torch.cuda.synchronize()
+        return phi.cpu().numpy().copy(), info
+
+    keys = ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies", "status")
+    try:
+        for mode in ("none", "ras", "ras16", "cluster16", "sap", "overlap"):
+            cs.ctx.set_operand_precision(16 if mode.endswith("16") else 32)
+            cs.ctx.set_schwarz(mode == "sap")
+            if mode == "none":
+                cs.ctx.set_solver(use_ras=False)
+            else:
+                dom, s, it, nras = {"ras": ((4, 4, 4, 4), 0, 2, 3), "ras16": ((4, 4, 4, 4), 0, 2, 4), "cluster16": ((8, 8, 4, 4), 0, 2, 2),
+                                    "sap": ((4, 4, 4, 4), 0, 3, 2), "overlap": ((4, 4, 4, 4), 1, 3, 1)}[mode]
+                cs.ctx.ras_precondition(dom, s, it, nras)
+                cs.ctx.set_solver(use_ras=True)
+            cs.ctx.set_graphs(False)
+            ref, iref = run()
+            cs.ctx.set_graphs(True)
+            for rep in range(4):
+                got, info = run()
+                assert np.array_equal(got, ref), (mode, rep)
+                assert all(info[k] == iref[k] for k in keys), (mode, rep, info, iref)
+            a = got
+            assert cs.op.true_residual(eta, (a[..., 0] + 1j * a[..., 1]).reshape(cs.V, 4, 3)) <= 1e-12
+    finally:
+        cs.ctx.set_graphs(True)
+        cs.ctx.set_schwarz(False)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_solver(use_ras=False)
+
+
 def test_workspace_growth_failure():
     """A stacked solve whose workspace growth runs out of memory (injected: WCRAS_FAIL_ALLOC_ABOVE) returns an error and
     leaves a context that solves a single right-hand side again (ws_nrhs must not survive a failed growth)."""
