@@ -154,7 +154,6 @@ int wcras_ras_apply(wcras_ctx* ctx, const float* r_dev, float* v_dev) {
 
 int wcras_set_solver(wcras_ctx* ctx, double inner_tol, int inner_maxit, int outer_maxit, int use_ras) {
     NEED(ctx, "null ctx");
-    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
     NEED(inner_tol > 0 && inner_maxit >= 1 && outer_maxit >= 1, "set_solver: tolerances and caps must be positive");
     ctx->inner_tol = inner_tol;
     ctx->inner_maxit = inner_maxit;

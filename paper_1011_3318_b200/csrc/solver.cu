@@ -298,12 +298,12 @@ template <typename T> struct Work {
 };
 
 void drop_iter_graphs(wcras_ctx* ctx) {
-    for (auto& g : ctx->iter_graph) {
-        if (g.exec) cudaGraphExecDestroy(g.exec);
-        g = wcras_ctx::IterGraph();
-    }
+    for (auto& row : ctx->iter_graph)
+        for (auto& g : row) {
+            if (g.exec) cudaGraphExecDestroy(g.exec);
+            g = wcras_ctx::IterGraph();
+        }
     ctx->graph_b = ctx->graph_x = nullptr;
-    ctx->graph_kid = -1;
 }
 
 // BiCGStab driver.  K(in,out) applies the preconditioner (ignored when k_identity).  status: 0 converged,
@@ -406,12 +406,11 @@ static int bicgstab(wcras_ctx* ctx, Work<T>& w, const typename VecOf<T>::type* b
             const bool graphable = sizeof(T) == 4 && la > 0 && ctx->use_graphs && !ctx->timing && restarts == 0 && rt == b &&
                                    (kind == 0) == !x_written;
             if (graphable) {
-                if (ctx->graph_b != (const void*)b || ctx->graph_x != (const void*)x || ctx->graph_gen != ctx->cfg_gen ||
-                    ctx->graph_kid != (int)k_identity) {
+                if (ctx->graph_b != (const void*)b || ctx->graph_x != (const void*)x || ctx->graph_gen != ctx->cfg_gen) {
                     drop_iter_graphs(ctx);
-                    ctx->graph_b = b; ctx->graph_x = x; ctx->graph_gen = ctx->cfg_gen; ctx->graph_kid = (int)k_identity;
+                    ctx->graph_b = b; ctx->graph_x = x; ctx->graph_gen = ctx->cfg_gen;
                 }
-                wcras_ctx::IterGraph& g = ctx->iter_graph[kind];
+                wcras_ctx::IterGraph& g = ctx->iter_graph[k_identity ? 0 : 1][kind];
                 if (g.exec) {
                     WC_CUDA(cudaGraphLaunch(g.exec, ctx->stream));
                     ctx->launches += g.d_launches; ctx->dv32 += g.d_dv32; ctx->block_dv += g.d_blk; ctx->ras_applies += g.d_ras;

@@ -220,11 +220,10 @@ struct wcras_ctx {
         int seen = 0;
         long long d_launches = 0;
         int d_dv32 = 0, d_blk = 0, d_ras = 0;
-    } iter_graph[3];
+    } iter_graph[2][3];             // [no preconditioner / preconditioner][kind]
     const void* graph_b = nullptr;  // key of the captured graphs: right-hand side and solution vectors, configuration generation
     const void* graph_x = nullptr;
     unsigned graph_gen = 0;
-    int graph_kid = -1;            // ... and whether the iteration applies a preconditioner
     unsigned cfg_gen = 1;          // bumped by every call that changes what an inner iteration launches
     int use_graphs = 1;
     cudaStream_t cap_stream = nullptr;  // captures run on this internal stream (the caller's may be the legacy default stream, which cannot capture)
