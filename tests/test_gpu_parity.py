@@ -258,6 +258,9 @@ FP16_CASES = [
     # overlap 0 (the shapes configs[3] names), overlapping domains (6^4 = 1296 sites, 10x6x6x6, 8^4 from 4^4 + 2)
     (2, (8, 4, 4, 4), 0, 3, 2), (2, (8, 8, 4, 4), 0, 3, 3), (2, (8, 8, 8, 8), 0, 2, 2), (1, (4, 4, 4, 4), 1, 4, 1),
     (2, (8, 4, 4, 4), 1, 3, 2), (2, (4, 4, 4, 4), 2, 2, 1), (1, (8, 8, 4, 4), 0, 2, 2),
+    # clusters with padding lanes (240-site sub-blocks on 256 threads), wrap-around directions (block = L in x and y) and a
+    # 3-CTA cluster whose middle sub-block has remote neighbours on both sides
+    ("ragged", (6, 4, 10, 2), 0, 2, 3), ("ragged", (6, 4, 5, 4), 0, 3, 2), ("ragged", (6, 4, 10, 2), 1, 2, 2), ("ragged", (3, 4, 10, 4), 0, 2, 2),
 ]
 
 
