@@ -115,6 +115,10 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                  float4* __restrict__ hb_out, const float4* phi_in, float4* phi_out, float4* __restrict__ rho_dm,
                  const int4* __restrict__ dom_org, const unsigned* __restrict__ dom_bc) {
     if (fg.stop && __ldg(fg.stop)) return;  // the inner solver has converged (launch enqueued ahead of the host's check)
+    // Programmatic dependent launch: the next cycle of this K_RAS application (launched with the programmatic-serialization
+    // attribute) may be scheduled as SMs fall free while this grid is still running; its set-up and its first operand
+    // copies overlap our tail, and its griddepcontrol.wait below holds it until this grid has completed.
+    asm volatile("griddepcontrol.launch_dependents;");
     extern __shared__ float4 smem[];
     const int nsp = NSP ? NSP : fg.nsp;
     const Cta16Smem lay = cta16_smem(nsp, nface, stage_halo);
@@ -219,10 +223,22 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         cp_async_commit();
     };
 
+    // the operands do not depend on the previous kernel: their copies (and everything above) run ahead of it
+    if ((int)blockIdx.x < ndl && k == 0) {
+        const int dom0 = launch_dom(fg, blockIdx.x, colour);
+        mbar_expect_tx(bar_links, half_bytes);
+        bulk_g2s(op_addr, dm16 + (size_t)dom0 * 18 * nsp, half_bytes, bar_links);
+        mbar_expect_tx(bar_clov, half_bytes);
+        bulk_g2s(op_addr + half_bytes, dm16 + ((size_t)dom0 * 18 + 9) * nsp, half_bytes, bar_clov);
+    }
+    asm volatile("griddepcontrol.wait;" ::: "memory");  // residual, halo slots, phi: written by the kernels before this one
     if ((int)blockIdx.x < ndl) {
         const int dom0 = launch_dom(fg, blockIdx.x, colour);
-        request_links_vec(dom0);
-        request_clover(dom0);
+        if (k == 0 && vec_bytes) {
+            mbar_expect_tx(bar_vec, vec_bytes);
+            if (src_dm) bulk_g2s(rs_addr, r_dm + (size_t)dom0 * 6 * nsp, 6u * chunk_bytes, bar_vec);
+            if (CHAIN && stage_halo) bulk_g2s(hs_addr, hb_in + (size_t)dom0 * 24 * nface, 24u * (unsigned)nface * 16u, bar_vec);
+        }
         if (k == 0) cp_async16(org_s, dom_org + dom0);  // committed with (or as) the first group below, waited for at the loop top
         if (!src_dm) request_r_lat(dom_org[dom0]);
         else cp_async_commit();
@@ -467,6 +483,24 @@ static cta16_kernel_t cta16_kernel(bool chain, int nsp) {
 
 int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu
 
+// every launch carries the programmatic-stream-serialization attribute: behind another ras_cta16_kernel (which triggers its
+// dependents at once) it starts as SMs fall free and waits in griddepcontrol.wait; behind any other kernel the attribute
+// changes nothing
+template <typename... Args>
+static cudaError_t cta16_launch(wcras_ctx* ctx, bool chain, int grid, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)ctx->fused.nsp);
+    cfg.dynamicSmemBytes = ctx->cta16_smem;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, cta16_kernel(chain, ctx->fused.nsp), args...);
+}
+
 // Build the fp16 domain-major operand copy and the domain-major rho_fin buffer; returns 1 if this tier can run the
 // configuration (single CTA per domain, shared memory fits), 0 otherwise (the caller falls back to ras_cta.cu).
 int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<float>& f) {
@@ -547,11 +581,10 @@ int ras_round_fields(wcras_ctx* ctx) {
 
 int ras_cta16_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bool accum) {
     const FusedGeom& fg = ctx->fused;
-    cta16_kernel(false, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ctx->ras.nd, -1, ctx->nface, ctx->stage_halo,
-                                                                                -(float)ctx->kappa, ctx->dm16, r, nullptr, nullptr, nullptr,
-                                                                                accum ? vout : nullptr, vout, nullptr, ctx->dom_org, ctx->dom_bc);
+    WC_CUDA(cta16_launch(ctx, false, ctx->cta_grid, fg, ctx->ras.nd, -1, ctx->nface, ctx->stage_halo, -(float)ctx->kappa, (const uint4*)ctx->dm16,
+                         r, (const float4*)nullptr, (const float4*)nullptr, (float4*)nullptr, (const float4*)(accum ? vout : nullptr), vout,
+                         (float4*)nullptr, (const int4*)ctx->dom_org, (const unsigned*)ctx->dom_bc));
     ctx->launches++;
-    WC_CHECK_LAUNCH();
     return WCRAS_OK;
 }
 
@@ -571,13 +604,13 @@ int ras_cta16_apply_chained(wcras_ctx* ctx, const float4* r, float4* v) {
         TimedRegion tr(ctx, TC_BLOCK);
         ctx->block_dv += ctx->ras.niter;
         if (j == 0)
-            cta16_kernel(false, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
-                fg, nd, -1, nface, ctx->stage_halo, mk, ctx->dm16, r, nullptr, nullptr, last ? nullptr : hb[0], nullptr, v, last ? nullptr : rf,
-                ctx->dom_org, ctx->dom_bc);
+            WC_CUDA(cta16_launch(ctx, false, ctx->cta_grid, fg, nd, -1, nface, ctx->stage_halo, mk, (const uint4*)ctx->dm16, r, (const float4*)nullptr,
+                                 (const float4*)nullptr, last ? (float4*)nullptr : hb[0], (const float4*)nullptr, v, last ? (float4*)nullptr : rf,
+                                 (const int4*)ctx->dom_org, (const unsigned*)ctx->dom_bc));
         else
-            cta16_kernel(true, fg.nsp)<<<ctx->cta_grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(
-                fg, nd, -1, nface, ctx->stage_halo, mk, ctx->dm16, nullptr, rf, hb[(j - 1) & 1], last ? nullptr : hb[j & 1], v, v,
-                last ? nullptr : rf, ctx->dom_org, ctx->dom_bc);
+            WC_CUDA(cta16_launch(ctx, true, ctx->cta_grid, fg, nd, -1, nface, ctx->stage_halo, mk, (const uint4*)ctx->dm16, (const float4*)nullptr,
+                                 (const float4*)rf, (const float4*)hb[(j - 1) & 1], last ? (float4*)nullptr : hb[j & 1], (const float4*)v, v,
+                                 last ? (float4*)nullptr : rf, (const int4*)ctx->dom_org, (const unsigned*)ctx->dom_bc));
         ctx->launches++;
     }
     WC_CHECK_LAUNCH();
@@ -603,12 +636,12 @@ int ras_cta16_apply_sap(wcras_ctx* ctx, const float4* r, float4* v) {
         float4* rho_out = last_visit ? nullptr : rf;
         float4* halo_out = last_step ? nullptr : hb;
         if (step == 0)
-            cta16_kernel(false, fg.nsp)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm,
-                                                                               nullptr, halo_out, nullptr, v, rho_out, ctx->dom_org, ctx->dom_bc);
+            WC_CUDA(cta16_launch(ctx, false, grid, fg, ndl, colour, nface, ctx->stage_halo, mk, (const uint4*)ctx->dm16, r_lat, r_dm, (const float4*)nullptr,
+                                 halo_out, (const float4*)nullptr, v, rho_out, (const int4*)ctx->dom_org, (const unsigned*)ctx->dom_bc));
         else
-            cta16_kernel(true, fg.nsp)<<<grid, fg.nsp, ctx->cta16_smem, ctx->stream>>>(fg, ndl, colour, nface, ctx->stage_halo, mk, ctx->dm16, r_lat, r_dm, hb,
-                                                                              halo_out, first_visit ? nullptr : v, v, rho_out, ctx->dom_org,
-                                                                              ctx->dom_bc);
+            WC_CUDA(cta16_launch(ctx, true, grid, fg, ndl, colour, nface, ctx->stage_halo, mk, (const uint4*)ctx->dm16, r_lat, r_dm, (const float4*)hb,
+                                 halo_out, (const float4*)(first_visit ? nullptr : v), v, rho_out, (const int4*)ctx->dom_org,
+                                 (const unsigned*)ctx->dom_bc));
         ctx->launches++;
     }
     WC_CHECK_LAUNCH();
