@@ -205,7 +205,8 @@ int wcras_export_clover(wcras_ctx* ctx, double* out_dev);
 /* Time one kernel class in its native layout on internal scratch fields: reps back-to-back launches
  * bracketed by CUDA events on the library's stream; returns the mean milliseconds per launch.
  * which: 0 = fp32 D, 1 = fp64 D, 2 = one K_RAS block-solve launch (all domains, current RAS parameters),
- *        3 = fused BLAS update (x += a p + w s ; r = s - w t ; <rt,r>, |r|^2). */
+ *        3 = fused BLAS update (x += a p + w s ; r = s - w t ; <rt,r>, |r|^2),
+ *        4 = one whole K_RAS application (Alg. 1: NRAS cycles, as the inner solver issues it; ms per application). */
 int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch);
 
 /* How many kernels of this library have been launched on ctx since creation (for bench.py's gpu_launches). */

@@ -343,10 +343,10 @@ int wcras_export_clover(wcras_ctx* ctx, double* out_dev) {
 
 int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch) {
     NEED(ctx, "null ctx");
-    NEED(ms_per_launch && reps >= 1 && which >= 0 && which <= 3, "time_kernel: bad arguments");
+    NEED(ms_per_launch && reps >= 1 && which >= 0 && which <= 4, "time_kernel: bad arguments");
     if (int rc = ensure_workspace(ctx)) return rc;
     if (which == 3) return time_blas(ctx, reps, ms_per_launch);
-    NEED(which != 2 || ctx->ras.set, "time_kernel: call wcras_ras_precondition first");
+    NEED((which != 2 && which != 4) || ctx->ras.set, "time_kernel: call wcras_ras_precondition first");
     const size_t V = ctx->geom.V;
     // deterministic non-trivial scratch input: reuse the fp32 link array bytes as a spinor-sized pattern
     WC_CUDA(cudaMemcpyAsync(ctx->w32[0], ctx->g32a, sizeof(float4) * 6 * V, cudaMemcpyDeviceToDevice, ctx->stream));
@@ -361,7 +361,8 @@ int wcras_time_kernel(wcras_ctx* ctx, int which, int reps, double* ms_per_launch
         for (int k = 0; k < n && !rc; k++) {
             if (which == 0) rc = dslash<float>(ctx, ctx->w32[0], ctx->w32[1]);
             else if (which == 1) rc = dslash<double>(ctx, ctx->w64[0], ctx->w64[1]);
-            else rc = ras_block_solve(ctx, ctx->w32[0], ctx->w32[1]);
+            else if (which == 2) rc = ras_block_solve(ctx, ctx->w32[0], ctx->w32[1]);
+            else rc = ras_apply(ctx, ctx->w32[0], ctx->w32[1]);  // a whole K_RAS application: NRAS chained cycles
         }
         WC_CUDA(cudaEventRecord(e1, ctx->stream));
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
