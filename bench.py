@@ -229,6 +229,26 @@ def oracle_table(torch, binding, I, O, config4=False):
     return out
 
 
+def run_survey(torch, binding, I):
+    """The paper's parameter survey as the library runs it (wcras_ras_autotune): every row tried on the BASELINE field
+    (configs[3]) and on the near-critical field of `hard_regime`, with fp16 and fp32 operand storage as the starting point."""
+    cfg = I.CONFIGS[3]
+    dims = cfg["dims"]
+    out = {"survey": "wcras_ras_autotune, tol 1e-12, 32^4", "fields": {}}
+    for name, U, kappa, csw, seed in (("configs[3] (Haar links, kappa 0.1225)", I.make_gauge(cfg), cfg["kappa"], cfg["csw"], cfg["seed"]),
+                                      ("near-critical (links exp(i 0.2 H) seed 17, kappa 0.13)", I.gauge_exp(dims, 0.2, 17), 0.13, 1.0, 18)):
+        ctx = binding.Context(dims, kappa, csw, torch.view_as_real(torch.from_numpy(U)).contiguous().cuda())
+        eta = torch.view_as_real(torch.from_numpy(I.spinor(dims, seed))).contiguous().cuda()
+        ctx.set_solver(inner_tol=INNER_TOL, use_ras=True)
+        ctx.set_operand_precision(16)
+        t0 = time.time()
+        best, rows = ctx.ras_autotune(eta, TOL, max_rows=256)
+        out["fields"][name] = {"seconds": time.time() - t0, "best": best, "rows": rows}
+        del ctx, eta
+        torch.cuda.empty_cache()
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -239,6 +259,9 @@ def main():
     ap.add_argument("--no-hard", action="store_true", help="skip the near-critical side rows (a second gauge field)")
     ap.add_argument("--no-side", action="store_true", help="skip the side rows (named shapes, SAP, multi-RHS, configs 0-2)")
     ap.add_argument("--config4", action="store_true", help="add configs[4] (48^3 x 96, minutes of host time) to `configs`")
+    ap.add_argument("--survey", action="store_true",
+                    help="run the parameter survey (wcras_ras_autotune, PAPER.md:109) on configs[3] and on the near-critical field "
+                         "and print its rows as one JSON line instead of the benchmark (profiles/r2_survey.md)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -253,6 +276,9 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local)
+    if args.survey:
+        run_survey(torch, binding, I)
+        return
     if world > 1:
         R.init("nccl", torch.device("cuda", local))
     hbm_peak, peak_src, peaks_json = peaks()
