@@ -81,4 +81,6 @@ def test_config4_full_size():
     ctx.ras_precondition((4, 4, 4, 4), 0, 3, 2)
     solve("SAP 4^4 N_dominv 3, 2 cycles, fp16 operands", warm=True)
     ctx.set_schwarz(False)
+    ctx.ras_precondition(r["domain"], r["overlap"], r["block_iters"], 1)
+    solve("RAS 8^4 overlap 1 N_dominv 4 NRAS 1, fp16 operands", warm=True)
     ctx.set_operand_precision(32)
