@@ -88,7 +88,9 @@ __global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restric
     for (int j = 0; j < FIN_CTAS; j++)
 #pragma unroll
         for (int k = 0; k < 3; k++) tot[k] += __ldcg(&slice[j * 3 + k]);
-    if (DOT == 1) {
+    if (DOT == 3) {
+        sc->nrm = tot[2];
+    } else if (DOT == 1) {
         sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
         const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
         sc->alpha[0] = a.r; sc->alpha[1] = a.i;
@@ -102,6 +104,7 @@ __global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restric
 // DOT = 0: out = D in (XPAY: out = bsrc - D in).
 // DOT = 1: also rtv = <dotv, out> and alpha = rho / rtv          (BiCGStab: v = D ph, dotv = rt)
 // DOT = 2: also ts = <out, dotv>, tt = <out, out>, omega = ts/tt (BiCGStab: t = D sh, dotv = s)
+// DOT = 3: also nrm = <out, out>                                  (true residual: out = eta - D phi)
 template <typename T, bool XPAY, int TH, int MINB, int DOT>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
                                                      typename VecOf<T>::type* out,  // may be bsrc (r = r - D v in place)
@@ -127,7 +130,7 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
         const size_t ro = threadIdx.y * rstride;
         in += ro; out += ro;
         if (XPAY) bsrc += ro;
-        if (DOT) dotv += ro;
+        if (DOT == 1 || DOT == 2) dotv += ro;
     }
     const bool valid = i < g.V;
     if (!DOT && !valid) return;
@@ -159,7 +162,12 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
             for (int k = 0; k < 24; k++) acc[k] -= kappa * hop[k];
         }
         store_spinor(out, V, i, acc);
-        if (DOT) {
+        if (DOT == 3) {
+            T d2 = 0;
+#pragma unroll
+            for (int k = 0; k < 24; k++) d2 = wc_fma(acc[k], acc[k], d2);
+            dsum[2] = d2;
+        } else if (DOT) {
             load_spinor(dotv, V, i, s);
             T d0 = 0, d1 = 0, d2 = 0;  // per-site sums in T, accumulated over sites in fp64
 #pragma unroll
@@ -291,6 +299,9 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
         else if (dot == 2)                                                                                                         \
             dslash_kernel<T, false, TH, (sizeof(T) == 4 ? 384 / TH : 1), 2><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
+        else if (dot == 3)                                                                                                         \
+            dslash_kernel<T, true, TH, (sizeof(T) == 4 ? 384 / TH : 1), 3><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP,  \
+                                                                              BM, nullptr, ctx->dpart, nblk, POFF, rstride, ztile);  \
         else if (b_minus)                                                                                                          \
             dslash_kernel<T, true, TH, (sizeof(T) == 4 ? 384 / TH : 1), 0><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP,  \
                                                                               BM, nullptr, nullptr, 0, 0, rstride, ztile);         \
@@ -310,6 +321,7 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
 #undef WC_DSL
     if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
     if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
+    if (dot == 3) dot_finish_kernel<3><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, nullptr);
     if (dot) ctx->launches++;
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;
     WC_CHECK_LAUNCH();

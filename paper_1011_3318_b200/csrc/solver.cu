@@ -652,11 +652,12 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
             TimedRegion tr(ctx, TC_BLAS);
             LAUNCH(k_add_d, n64, phi, dx);
         }
-        if (int r2 = dslash<double>(ctx, phi, res, eta)) return r2;  // res = eta - D phi (true residual, fp64)
+        // res = eta - D phi (true residual, fp64); one system: its norm comes out of the same kernel (DOT = 3)
+        if (int r2 = dslash<double>(ctx, phi, res, eta, nr == 1 ? 3 : 0, nullptr, ctx->sc64)) return r2;
         rn2 = 0;
         double worst = 0;
         for (int k = 0; k < nr; k++) {  // the true residual of every system on its own
-            {
+            if (nr > 1) {
                 TimedRegion tr(ctx, TC_BLAS);
                 LAUNCH(k_norm2_d, n1, res + k * n1, ctx->sc64, ctx->partials, ctx->ticket);
             }
