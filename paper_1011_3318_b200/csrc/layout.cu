@@ -127,17 +127,54 @@ __global__ void export_clover_kernel(int V, const double2* __restrict__ c64, dou
 // canonical [V][24] <-> SoA [CH][V] through a shared-memory tile of LAYOUT_TS sites: both the canonical side (a site's 24
 // reals contiguous) and the SoA side (a chunk's sites contiguous) are then read and written as whole 16-byte rows
 constexpr int LAYOUT_TS = 64;
+// npart != nullptr: the block's sum of squares goes to npart[blockIdx.x] (|eta|^2 at the start of a solve without a pass of
+// its own); norm_finish_kernel sums the partials in a fixed order
 template <typename T, typename Vec, int CH>
-__global__ void __launch_bounds__(256) spinor_to_internal_kernel(int V, const T* __restrict__ canon, Vec* __restrict__ soa) {
+__global__ void __launch_bounds__(256) spinor_to_internal_kernel(int V, const T* __restrict__ canon, Vec* __restrict__ soa,
+                                                                 double* __restrict__ npart) {
     __shared__ Vec tile[LAYOUT_TS * CH];
+    __shared__ double wsum[8];
     const size_t i0 = (size_t)blockIdx.x * LAYOUT_TS;
     const int ns = (int)((size_t)V - i0 < (size_t)LAYOUT_TS ? (size_t)V - i0 : (size_t)LAYOUT_TS);
     const Vec* src = reinterpret_cast<const Vec*>(canon) + i0 * CH;  // element e = local site * CH + chunk
-    for (int e = threadIdx.x; e < ns * CH; e += blockDim.x) tile[e] = src[e];
+    double acc = 0;
+    for (int e = threadIdx.x; e < ns * CH; e += blockDim.x) {
+        const Vec t = src[e];
+        tile[e] = t;
+        if (npart) {
+            const T* c = reinterpret_cast<const T*>(&t);
+#pragma unroll
+            for (int j = 0; j < (int)(sizeof(Vec) / sizeof(T)); j++) acc = fma((double)c[j], (double)c[j], acc);
+        }
+    }
+    if (npart) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    }
     __syncthreads();
+    if (npart && threadIdx.x == 0) {
+        double t = 0;
+        for (int w = 0; w < 8; w++) t += wsum[w];
+        npart[blockIdx.x] = t;
+    }
     for (int e = threadIdx.x; e < LAYOUT_TS * CH; e += blockDim.x) {
         const int c = e / LAYOUT_TS, sl = e % LAYOUT_TS;
         if (sl < ns) soa[(size_t)c * V + i0 + sl] = tile[sl * CH + c];
+    }
+}
+__global__ void __launch_bounds__(1024) norm_finish_kernel(unsigned n, const double* __restrict__ npart, Scalars* sc) {
+    __shared__ double wsum[32];
+    double acc = 0;
+    for (unsigned j = threadIdx.x; j < n; j += 1024) acc += npart[j];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0;
+        for (int w = 0; w < 32; w++) t += wsum[w];
+        sc->nrm = t;
     }
 }
 template <typename T, typename Vec, int CH>
@@ -180,16 +217,28 @@ int setup_fields(wcras_ctx* ctx, const double* gauge_dev) {
     return WCRAS_OK;
 }
 
-int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal) {
+// norm_sc != nullptr: norm_sc->nrm = |canonical|^2 as well (one small kernel behind the conversion, no extra vector pass)
+int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal, Scalars* norm_sc) {
     const int V = ctx->geom.V, T = 256;
+    const unsigned nblk = (unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS);
     if ((uintptr_t)canonical & 15) { snprintf(ctx->err, sizeof ctx->err, "spinor buffers must be 16-byte aligned"); return WCRAS_INVALID_ARG; }
+    double* npart = nullptr;
+    if (norm_sc) {
+        if (!ctx->npart || ctx->npart_blocks < nblk) {
+            if (alloc_dev(ctx, (void**)&ctx->npart, sizeof(double) * nblk)) return WCRAS_CUDA_ERROR;
+            ctx->npart_blocks = nblk;
+        }
+        npart = ctx->npart;
+    }
     if (prec == 32)
-        spinor_to_internal_kernel<float, float4, 6><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
-            V, (const float*)canonical, (float4*)internal);
+        spinor_to_internal_kernel<float, float4, 6><<<nblk, T, 0, ctx->stream>>>(V, (const float*)canonical, (float4*)internal, npart);
     else
-        spinor_to_internal_kernel<double, double2, 12><<<(unsigned)((V + LAYOUT_TS - 1) / LAYOUT_TS), T, 0, ctx->stream>>>(
-            V, (const double*)canonical, (double2*)internal);
+        spinor_to_internal_kernel<double, double2, 12><<<nblk, T, 0, ctx->stream>>>(V, (const double*)canonical, (double2*)internal, npart);
     ctx->launches++;
+    if (norm_sc) {
+        norm_finish_kernel<<<1, 1024, 0, ctx->stream>>>(nblk, npart, norm_sc);
+        ctx->launches++;
+    }
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
 }

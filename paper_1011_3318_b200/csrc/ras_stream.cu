@@ -10,9 +10,9 @@
 //     site, the C CTAs of a domain form a cluster; the grid is persistent (as many clusters as the chip holds).
 //   * On chip, for the whole block solve: the MR vectors rho and v of the sub-block in shared memory (192 B per site,
 //     120 KB at 625 sites), q in registers.  q = D_Omega' rho is a GATHER: every site reads the full spinors of its (up to) 8
-//     neighbours from shared memory through a precomputed address: plain ld.shared for a neighbour in the same CTA,
-//     ld.shared::cluster (DSMEM) for one in another CTA of the cluster; a neighbour outside Omega' is skipped
-//     (Dirichlet), wrap-around inside Omega' (ext = L) is kept.
+//     neighbours from shared memory through a precomputed address: a shared::cta address for a neighbour in the same
+//     CTA, the mapa result (DSMEM) for one in another CTA of the cluster, both read by the same generic load; a
+//     neighbour outside Omega' is skipped (Dirichlet), wrap-around inside Omega' (ext = L) is kept.
 //   * Links and clover are NOT resident: every sweep streams a domain-major operand record per site from global memory
 //     -- 4 forward links, the 4 backward links U_mu(x-mu) already gathered to the site, the clover blocks; fp32 (58
 //     16-byte chunks) or, in 16-bit operand mode (reading R1), fp16 (33 chunks = 528 B).  The N_dominv sweeps of a
@@ -20,7 +20,11 @@
 //     the NEXT domain's record into L2 meanwhile (cp.async.bulk.prefetch.L2) was measured 5 % slower: it halves the L2
 //     room of the records in use (ncu: L2 hit rate 51 %), so it is not done.
 //   * Domain-local dots: warp shuffle -> one float4 per warp pushed to every CTA of the cluster -> fixed-order sum.
-//     Two cluster barriers per MR iteration (dots; rho updated before the neighbours read it again).
+//     Two cluster barriers per MR iteration (dots; rho updated before the neighbours read it again).  Measured and not
+//     kept (8^4 + overlap 1 at 32^4, fp16, 1.57 ms per launch of 4 sweeps): the partials by st.async onto an mbarrier and
+//     the "rho in place" sync as remote mbarrier arrivals, 1.66 ms (20 polling warps take issue slots from the ones still
+//     working; the barrier time is the wait for the slowest of 16 CTAs, not the barrier itself); the records through a
+//     3-slot cp.async ring in shared memory two links ahead, 1.75 ms; prefetch.global.L1 one link ahead, 1.80 ms.
 // Roofline: L2 operand stream, 528 (fp16) or 928 (fp32) B per site and sweep, against ~1.7 k fp32 instructions per site
 // and sweep; HBM floor per block solve: one record + 96 B in per extended site, 96 B out per bulk site.
 #include <cuda_fp16.h>
@@ -47,11 +51,6 @@ __device__ __forceinline__ unsigned st_mapa(unsigned addr, unsigned rank) {
     unsigned r;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
     return r;
-}
-__device__ __forceinline__ float4 ld_cluster_f4(unsigned addr) {
-    float4 v;
-    asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-    return v;
 }
 __device__ __forceinline__ void st_cluster_push(unsigned addr, float a, float b, float c, float d) {
     asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
@@ -103,6 +102,14 @@ __device__ __forceinline__ void load_clover_block(const uint4* __restrict__ p, s
 template <int CH>
 __device__ __forceinline__ void load_clover_block(const uint4* __restrict__ p, size_t stride, const float* t, float* Ab) {
     load_rec<9, 36, 0>(p + (size_t)(9 * CH) * stride, stride, t, Ab);
+}
+// One load for both kinds of neighbour: a generic address whose low word is a shared::cta address (own CTA) or the
+// result of mapa (another CTA of the cluster), the high word the shared window of the generic space.  A per-lane choice
+// between ld.shared and ld.shared::cluster instead costs two predicated loads and four moves per chunk.
+__device__ __forceinline__ float4 ld_window_f4(unsigned long long addr) {
+    float4 v;
+    asm volatile("ld.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(addr));
+    return v;
 }
 __device__ __forceinline__ float4 ld_shared_f4(unsigned addr) {
     float4 v;
@@ -211,7 +218,8 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
     for (int mu = 0; mu < 4; mu++)
         if (fg.split[mu]) bulk = bulk && ec[mu] >= fg.s && ec[mu] < fg.s + fg.b[mu];
     // cluster-space address of chunk 0 of rho at the neighbour in direction (mu, +) [index 2mu] and (mu, -) [2mu+1]
-    unsigned nbr[8], remote = 0;
+    unsigned nbr[8];
+    const unsigned long long win = (unsigned long long)(size_t)rho & 0xffffffff00000000ull;  // shared window of the generic space
     {
         const unsigned base = st_smem_u32(rho);
         int lstride = 1, cstride = 1;
@@ -238,10 +246,10 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
                         else ok = false;
                     }
                 }
-                // a neighbour in this CTA is read through the plain shared window (ld.shared at full shared-memory
-                // bandwidth); only a neighbour in another CTA goes through the cluster window (DSMEM, ~20 B/clk per SM)
+                // a neighbour in this CTA keeps its shared::cta address (served by the local shared memory at full
+                // bandwidth); only a neighbour in another CTA gets a cluster-window address (DSMEM, ~20 B/clk per SM)
                 unsigned a = base + (unsigned)kd * 16u;
-                if (CL && rk != (int)rank) { a = st_mapa(a, (unsigned)rk); remote |= 1u << (2 * mu + sg); }
+                if (CL && rk != (int)rank) a = st_mapa(a, (unsigned)rk);
                 nbr[2 * mu + sg] = ok ? a : ST_NONE;
             }
             lstride *= fg.sb[mu];
@@ -272,8 +280,7 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
         float u[18], sn[24];                                                                                  \
         load_rec<R::LINK, 18>(myrec + (size_t)(MU * R::LINK) * stride, stride, (const OP*)nullptr, u);        \
         _Pragma("unroll") for (int c = 0; c < 6; c++) {                                                       \
-            const float4 t = CL && (remote >> (2 * MU) & 1u) ? ld_cluster_f4(nbr[2 * MU] + c * chunk_bytes)       \
-                                                         : ld_shared_f4(nbr[2 * MU] + c * chunk_bytes);      \
+            const float4 t = CL ? ld_window_f4(win | (nbr[2 * MU] + c * chunk_bytes)) : ld_shared_f4(nbr[2 * MU] + c * chunk_bytes); \
             sn[4 * c] = t.x; sn[4 * c + 1] = t.y; sn[4 * c + 2] = t.z; sn[4 * c + 3] = t.w;                   \
         }                                                                                                     \
         hop_fwd<float, MU>(u, sn, hop);                                                                       \
@@ -282,8 +289,7 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
         float u[18], sn[24];                                                                                  \
         load_rec<R::LINK, 18>(myrec + (size_t)((4 + MU) * R::LINK) * stride, stride, (const OP*)nullptr, u);  \
         _Pragma("unroll") for (int c = 0; c < 6; c++) {                                                       \
-            const float4 t = CL && (remote >> (2 * MU + 1) & 1u) ? ld_cluster_f4(nbr[2 * MU + 1] + c * chunk_bytes)       \
-                                                         : ld_shared_f4(nbr[2 * MU + 1] + c * chunk_bytes);      \
+            const float4 t = CL ? ld_window_f4(win | (nbr[2 * MU + 1] + c * chunk_bytes)) : ld_shared_f4(nbr[2 * MU + 1] + c * chunk_bytes); \
             sn[4 * c] = t.x; sn[4 * c + 1] = t.y; sn[4 * c + 2] = t.z; sn[4 * c + 3] = t.w;                   \
         }                                                                                                     \
         hop_bwd<float, MU>(u, sn, hop);                                                                       \
@@ -304,6 +310,14 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
                 herm6_mul<float>(Ab, rs + 12, q + 12);
             }
             float d0 = 0.f, d1 = 0.f, d2 = 0.f;
+#ifdef WC_X2
+            {
+                const x2::c2 mk = x2::bc(-kappa);
+#pragma unroll
+                for (int n = 0; n < 12; n++) x2::st(q + 2 * n, x2::fma(mk, x2::ld(hop + 2 * n), x2::ld(q + 2 * n)));
+            }
+            x2::mr_dots(q, rs, d0, d1, d2);
+#else
 #pragma unroll
             for (int n = 0; n < 24; n++) q[n] = fmaf(-kappa, hop[n], q[n]);
 #pragma unroll
@@ -313,6 +327,7 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
                 d1 = fmaf(qr, ri, d1); d1 = fmaf(-qi, rr, d1);
                 d2 = fmaf(qr, qr, d2); d2 = fmaf(qi, qi, d2);
             }
+#endif
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 d0 += __shfl_xor_sync(0xffffffffu, d0, o);
@@ -346,6 +361,13 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
 #pragma unroll
             for (int c = 0; c < 6; c++) {
                 float4 t = vv[c * nsp + k];
+#ifdef WC_X2
+                float va[4] = {t.x, t.y, t.z, t.w};
+                if (!last) x2::mr_update<true, 2>(ar, ai, q + 4 * c, rs + 4 * c, va);
+                else x2::mr_update<false, 2>(ar, ai, q + 4 * c, rs + 4 * c, va);
+                vv[c * nsp + k] = make_float4(va[0], va[1], va[2], va[3]);
+                if (!last) rho[c * nsp + k] = make_float4(rs[4 * c], rs[4 * c + 1], rs[4 * c + 2], rs[4 * c + 3]);
+#else
                 const float r0 = rs[4 * c], r1 = rs[4 * c + 1], r2 = rs[4 * c + 2], r3 = rs[4 * c + 3];
                 t.x = fmaf(ar, r0, t.x); t.x = fmaf(-ai, r1, t.x);
                 t.y = fmaf(ar, r1, t.y); t.y = fmaf(ai, r0, t.y);
@@ -360,6 +382,7 @@ ras_stream_kernel(FusedGeom fg, int nd, float kappa, const uint4* __restrict__ r
                     n4.w = fmaf(-ar, q[4 * c + 3], r3); n4.w = fmaf(-ai, q[4 * c + 2], n4.w);
                     rho[c * nsp + k] = n4;
                 }
+#endif
             }
             if (!last) st_barrier<CL>();  // the new rho of every CTA is in place before the next sweep reads it
         }

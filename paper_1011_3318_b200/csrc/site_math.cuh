@@ -157,10 +157,10 @@ __device__ __forceinline__ void mr_dots(const float* __restrict__ q, const float
 }
 
 // v += alpha rho; rho -= alpha q (UPD_RHO), alpha = ar + i ai
-template <bool UPD_RHO>
+template <bool UPD_RHO, int NC = 12>
 __device__ __forceinline__ void mr_update(float ar, float ai, const float* __restrict__ q, float* __restrict__ rho, float* __restrict__ v) {
 #pragma unroll
-    for (int k = 0; k < 12; k++) {
+    for (int k = 0; k < NC; k++) {
         const c2 r = ld(rho + 2 * k);
         c2 vv = ld(v + 2 * k);
         vv = fma(r, bc(ar), vv);

@@ -615,8 +615,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
     double norm_k[8], rel_k[8];
     double en2 = 0;
     for (int k = 0; k < nr; k++) {
-        if (int rc = to_internal(ctx, 64, eta_dev + (size_t)k * 24 * V, eta + k * n1)) return rc;
-        LAUNCH(k_norm2_d, n1, eta + k * n1, ctx->sc64, ctx->partials, ctx->ticket);
+        if (int rc = to_internal(ctx, 64, eta_dev + (size_t)k * 24 * V, eta + k * n1, ctx->sc64)) return rc;  // and |eta_k|^2
         if (int rc = read_scalars(ctx, ctx->sc64)) return rc;
         norm_k[k] = std::sqrt(ctx->sc_host->nrm);
         rel_k[k] = norm_k[k] > 0 ? 1.0 : 0.0;

@@ -231,6 +231,8 @@ struct wcras_ctx {
     unsigned* ticket = nullptr;
     double* dpart = nullptr;       // per-CTA partials of the dots fused into the Dslash: [3][blocks], slice sums, ticket
     unsigned dpart_blocks = 0;
+    double* npart = nullptr;       // per-CTA partials of the norm fused into the layout conversion
+    unsigned npart_blocks = 0;
     int nrhs = 1;                  // right-hand sides stacked in every solver vector (wcras_solve_multi)
     int ws_nrhs = 0;               // stack depth the workspace is allocated for
     // timing
@@ -311,7 +313,7 @@ void drop_iter_graphs(wcras_ctx* ctx);  // solver.cu
 
 // layout.cu
 int setup_fields(wcras_ctx* ctx, const double* gauge_dev);
-int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal);
+int to_internal(wcras_ctx* ctx, int prec, const void* canonical, void* internal, Scalars* norm_sc = nullptr);
 int from_internal(wcras_ctx* ctx, int prec, const void* internal, void* canonical);
 int export_clover(wcras_ctx* ctx, double* out_dev);
 
