@@ -105,7 +105,7 @@ __device__ __forceinline__ void load_clover_block(const uint4* __restrict__ p, s
 }
 // One load for both kinds of neighbour: a generic address whose low word is a shared::cta address (own CTA) or the
 // result of mapa (another CTA of the cluster), the high word the shared window of the generic space.  A per-lane choice
-// between ld.shared and ld.shared::cluster instead costs two predicated loads and four moves per chunk.
+// between ld.shared and ld.shared::cluster instead costs two predicated loads per chunk and an S2R per cluster load.
 __device__ __forceinline__ float4 ld_window_f4(unsigned long long addr) {
     float4 v;
     asm volatile("ld.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(addr));

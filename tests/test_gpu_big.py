@@ -83,4 +83,9 @@ def test_config4_full_size():
     ctx.set_schwarz(False)
     ctx.ras_precondition(r["domain"], r["overlap"], r["block_iters"], 1)
     solve("RAS 8^4 overlap 1 N_dominv 4 NRAS 1, fp16 operands", warm=True)
+    ctx.set_timing(True)   # per-class CUDA-event split of the same solve (profiles/r2_stream.md)
+    i = solve("  the same with the class split on")
+    ctx.set_timing(False)
+    print("  class split: block solve %.1f ms (%d launches)  D fp32 %.1f  D fp64 %.1f  BLAS %.1f  of %.1f ms" % (
+        i["ms_blocksolve"], i["ras_applies"], i["ms_dslash"], i["ms_dslash64"], i["ms_blas"], i["ms_total"]))
     ctx.set_operand_precision(32)

@@ -704,6 +704,27 @@ def test_full_size_32_ras_apply():
         cs.ctx.set_operand_precision(32)
 
 
+def test_full_size_32_streamed_tier():
+    """Tier 2c (ras_stream.cu) at full size in the launch configuration of the point configs[4] names (8^4 domains, overlap
+    1, N_dominv 4, NRAS 1: 10^4-site extended domains over 16-CTA clusters, 256 domains on 32^4), fp32 and fp16 operand
+    records, against the oracle's Alg. 1 on every site."""
+    cs = case(3)
+    r32 = I.spinor(cs.dims, 81).astype(np.complex64).astype(np.complex128)
+    block, s, nit, nras = (8, 8, 8, 8), 1, 4, 1
+    cs.ctx.set_ras_tier(5)  # the streamed-operand kernel or WCRAS_UNSUPPORTED (tier 0 picks it for this shape as well)
+    try:
+        for bits in (32, 16):
+            cs.ctx.set_operand_precision(bits)
+            cs.ctx.ras_precondition(block, s, nit, nras)
+            got = cs.ras_apply(r32)
+            want = (rounded_op(cs) if bits == 16 else cs.op).ras_apply(block, s, nit, nras, r32)
+            assert rel(got, want) <= TOL_RAS
+            assert np.abs(got - want).max() / np.abs(want).max() <= 10 * TOL_RAS
+    finally:
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_ras_tier(0)
+
+
 def test_generic_tier_many_domains():
     """Forced generic tier with more than 65535 domains (2^4 blocks on 32^4 = 65536 domains: the domain index lives in
     gridDim.x), per-domain dots summed in a fixed order: equal to the oracle and bit-identical run to run."""
