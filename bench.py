@@ -46,6 +46,9 @@ REFERENCE_BUDGET_S = 150.0   # wall-clock budget of the --impl reference arm
 # dram__bytes_read.sum + dram__bytes_write.sum of one dslash_kernel<float> launch at 32^4 from the committed
 # `ncu --set full` capture (profiles/r2_kernels.md); algorithmic bytes are 768 B/site = 805.3 MB
 DSLASH_TRAFFIC_NCU_BYTES = 812.2e6
+# dram__bytes_read.sum + dram__bytes_write.sum of ras_cta16_kernel, mean over the four launches of one K_RAS application
+# (661 + 861 + 861 + 690 MB; profiles/r2_kernels.md): below the algorithmic 805 MB because L2 keeps part of the halo and rho_fin
+BLOCK_TRAFFIC_NCU_BYTES = 768.3e6
 KEYS = ("outer_iters", "inner_iters", "inner_solves", "dv_fp32", "dv_fp64", "block_dv", "ras_applies", "rel_resid_true",
         "ms_total")
 
@@ -533,6 +536,7 @@ def main():
                       "per launch)" % (OPERAND_BITS, RAS["block_iters"]),
             "bound": "hbm", "unit": "GB/s", "sites": V, "peak": hbm_peak,
             "bytes_per_site_in_solve": blk_bytes_in_solve, "bytes_per_site_by_cycle": cyc_bytes,
+            "traffic": BLOCK_TRAFFIC_NCU_BYTES, "algorithmic_bytes": blk_bytes_in_solve * V,
             "ms_per_launch_in_solve": ms_blk_chained, "ms_per_k_ras_application": ms_kras,
             "ms_per_launch_class_split": ms_blk_in_solve,
             "achieved": blk_bytes_in_solve * V / (ms_blk_chained * 1e-3) / 1e9,
