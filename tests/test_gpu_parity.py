@@ -420,6 +420,9 @@ def test_solve_true_residual(which, ras):
     true = cs.op.true_residual(eta, phi)
     assert true <= 1e-12
     assert abs(info["rel_resid_true"] - true) <= 1e-13
+    # the library's own figure (|eta|^2 from the layout conversion, |eta - D phi|^2 from the fp64 Dslash that forms the
+    # residual) is the oracle's up to the rounding of the two D applications
+    assert abs(info["rel_resid_true"] - true) <= 1e-2 * true
     assert info["dv_fp32"] > 0 and info["inner_iters"] > 0
     # nested scheme with inner_tol 1e-5: each outer half-step gains ~5 digits (catches a broken preconditioner path)
     assert info["outer_iters"] <= 3 and info["inner_solves"] <= 5
