@@ -89,16 +89,18 @@ struct Cta16Smem {  // offsets in float4 units
     int hbuf, opbuf, rstage, hstage, red, bars, org;
     size_t bytes;
 };
+// The small tables come first, at offsets that do not depend on the launch parameters: an address that needs nface or
+// stage_halo costs a constant-bank load wherever the compiler rematerialises it (measured ~300 cycles, once per domain).
 __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_halo) {
     Cta16Smem s;
-    s.hbuf = 0;
-    s.opbuf = 24 * nsp;
+    s.red = 0;
+    s.bars = 8;
+    s.org = 10;
+    s.hbuf = 16;  // 256-byte offset: bulk-copy destinations stay 128-byte aligned
+    s.opbuf = s.hbuf + 24 * nsp;
     s.rstage = s.opbuf + 18 * nsp;
     s.hstage = s.rstage + 6 * nsp;
-    s.red = s.hstage + (stage_halo ? 24 * nface : 0);
-    s.bars = s.red + 8;
-    s.org = s.bars + 2;
-    s.bytes = (size_t)(s.org + 2) * 16;
+    s.bytes = (size_t)(s.hstage + (stage_halo ? 24 * nface : 0)) * 16;
     return s;
 }
 
@@ -129,7 +131,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
     float4* red = smem + lay.red;                                         // [nwarps]
     int4* org_s = reinterpret_cast<int4*>(smem + lay.org);                // [2] first site of the current / next domain (table dom_org)
     const unsigned bar_links = cta_smem_u32(smem + lay.bars), bar_clov = bar_links + 8, bar_vec = bar_links + 16;
-    const int k = threadIdx.x, lane = k & 31, warp = k >> 5, nwarps = blockDim.x >> 5;
+    const int k = threadIdx.x, lane = k & 31, warp = k >> 5;
     const bool active = k < fg.ns;
     const bool src_dm = r_dm != nullptr;
 
@@ -247,16 +249,28 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #ifdef WC_CTA16_PROFILE
     long long prof[12] = {0}, tlast = clock64();
 #endif
+    // Per-launch uniforms the domain loop tests after its last stores, pinned in one register: rematerialised from the
+    // constant bank there, each is a load of a few hundred cycles that the ncu source page shows as a long-scoreboard stall
+    // of every warp at once (K_RAS application 0.769 -> 0.767 ms).  bit 0: halo out, bit 1: rho_fin out, bit 2: phi += v;
+    // bits 8..: ndl.
+    unsigned uni = (hb_out ? 1u : 0u) | (rho_dm ? 2u : 0u) | (phi_in ? 4u : 0u) | ((unsigned)ndl << 8);
+    asm volatile("" : "+r"(uni));
+#define WC_UNI_HALO (uni & 1u)
+#define WC_UNI_RHO (uni & 2u)
+#define WC_UNI_ACC (uni & 4u)
+#define WC_UNI_NDL ((int)(uni >> 8))
     float U[72];
-    for (int j = 0;; j++) {
-        const int h = blockIdx.x + j * gridDim.x;
-        if (h >= ndl) break;
+    // h (this domain) is carried and the exit test uses has_next from the top of the iteration: recomputed at the bottom, h
+    // and the test cost an S2R and two constant-bank loads with nothing left to hide them behind (with the fixed offsets
+    // of the small shared-memory tables: K_RAS application 0.784 -> 0.769 ms, plain launch 0.162 -> 0.158 ms)
+    for (int j = 0, h = blockIdx.x; h < WC_UNI_NDL; j++) {
         WC_T(0)
         const unsigned par = (unsigned)j & 1u;
-        const bool has_next = h + (int)gridDim.x < ndl;
+        const int hn = h + (int)gridDim.x;
+        const bool has_next = hn < WC_UNI_NDL;
         const int dom = launch_dom(fg, h, colour);
-        const int nxt = launch_dom(fg, has_next ? h + gridDim.x : h, colour);
-        const unsigned dom_bc_here = hb_out ? __ldg(dom_bc + dom) : 0u;  // consumed by the halo scatter after the sweeps
+        const int nxt = launch_dom(fg, has_next ? hn : h, colour);
+        const unsigned dom_bc_here = WC_UNI_HALO ? __ldg(dom_bc + dom) : 0u;  // consumed by the halo scatter after the sweeps
         int4 org_nxt = make_int4(0, 0, 0, 0);
         if (!src_dm) org_nxt = __ldg(dom_org + nxt);  // lattice-layout source: the next residual column is requested below
         // ---- operands: links from the staged fp16 block into registers, scaled by -kappa ----
@@ -398,7 +412,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
             // alpha = <q,rho>/<q,q>, 0 if <q,q> = 0 (Q9); v += alpha rho; rho -= alpha q
             const float inv = s2 > 0.f ? 1.f / s2 : 0.f;
             const float ar = s0 * inv, ai = s1 * inv;
-            const bool upd_rho = it + 1 < fg.niter || rho_dm != nullptr;
+            const bool upd_rho = it + 1 < fg.niter || WC_UNI_RHO;
 #ifdef WC_X2
             if (upd_rho) x2::mr_update<true>(ar, ai, q, rho, v);
             else x2::mr_update<false>(ar, ai, q, rho, v);
@@ -417,7 +431,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         }
         WC_T(11)
         // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
-        if (hb_out) {
+        if (WC_UNI_HALO) {
             unsigned dd = dom_bc_here;
             int dstride = 1;
             float hs[12], g[12];
@@ -444,14 +458,14 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #undef WC_HALO
         }
         // ---- rho_fin (domain-major, every site of the domain) and the restriction R_Omega (bulk sites only) ----
-        if (rho_dm && active) {
+        if (WC_UNI_RHO && active) {
             float4* o = rho_dm + (size_t)dom * 6 * nsp + k;
 #pragma unroll
             for (int c = 0; c < 6; c++) o[(size_t)c * nsp] = make_float4(rho[4 * c], rho[4 * c + 1], rho[4 * c + 2], rho[4 * c + 3]);
         }
         if (bulk) {
             const size_t gi = site_of(org_s[j & 1]);  // visible since the first barrier of this domain
-            if (phi_in) {
+            if (WC_UNI_ACC) {
                 // phi += v as a fire-and-forget vector reduction (phi_in == phi_out; one writer per site)
 #pragma unroll
                 for (int c = 0; c < 6; c++)
@@ -464,7 +478,13 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
+        if (!has_next) break;
+        h = hn;
     }
+#undef WC_UNI_HALO
+#undef WC_UNI_RHO
+#undef WC_UNI_ACC
+#undef WC_UNI_NDL
 #ifdef WC_CTA16_PROFILE
     if (k == 0 && blockIdx.x == 0)
         printf("cta16 prof chain %d niter %d: epi/loop %lld | links wait %lld cvt %lld | vec wait %lld rho %lld cross %lld | scatter %lld clov wait %lld "
