@@ -108,8 +108,8 @@ __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_ha
 //   r_lat   residual source in the lattice layout (cycle 0 / first visit), or nullptr
 //   r_dm    residual source domain-major [nd][6][nsp] (rho_fin of the previous cycle), or nullptr
 //   rho_dm  rho_fin of this cycle, domain-major, or nullptr (then the last MR residual update is skipped, Q12)
-//   NSP     threads per CTA = padded sites per domain as a compile-time constant (256: every slot, operand and staging
-//           offset becomes an immediate), or 0 = taken from fg.nsp at run time
+//   NSP     threads per CTA = sites per domain as a compile-time constant (256, no padding lanes: every slot, operand and
+//           staging offset becomes an immediate and every thread is active), or 0 = fg.nsp / fg.ns at run time
 template <bool CHAIN, int NSP>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
 ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, float mkappa, const uint4* __restrict__ dm16,
@@ -132,7 +132,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
     int4* org_s = reinterpret_cast<int4*>(smem + lay.org);                // [2] first site of the current / next domain (table dom_org)
     const unsigned bar_links = cta_smem_u32(smem + lay.bars), bar_clov = bar_links + 8, bar_vec = bar_links + 16;
     const int k = threadIdx.x, lane = k & 31, warp = k >> 5;
-    const bool active = k < fg.ns;
+    const bool active = NSP ? true : k < fg.ns;  // NSP = 256 is only launched for domains of exactly 256 sites
     const bool src_dm = r_dm != nullptr;
 
     // ---- domain-independent geometry: local coordinates, bulk flag, destination slots ----
@@ -280,8 +280,14 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         for (int c = 0; c < 9; c++) {
             float f[8];
             half8_to_float(opbuf[c * nsp + k], f);
+#ifdef WC_X2
+            const x2::c2 mk2 = x2::bc(mkappa);
+#pragma unroll
+            for (int n = 0; n < 4; n++) x2::st(U + 8 * c + 2 * n, x2::mul(x2::ld(f + 2 * n), mk2));
+#else
 #pragma unroll
             for (int n = 0; n < 8; n++) U[8 * c + n] = mkappa * f[n];
+#endif
         }
         // ---- projection P_Omega' r: the staged residual column of this thread ----
         float rho[24], v[24];
@@ -496,8 +502,9 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 // ---- host side ----
 typedef void (*cta16_kernel_t)(FusedGeom, int, int, int, int, float, const uint4*, const float4*, const float4*, const float4*, float4*,
                                const float4*, float4*, float4*, const int4*, const unsigned*);
-static cta16_kernel_t cta16_kernel(bool chain, int nsp) {
-    if (nsp == 256) return chain ? ras_cta16_kernel<true, 256> : ras_cta16_kernel<false, 256>;
+// the NSP = 256 instance: domains of exactly 256 sites (no padding lane: the kernel takes every thread as active)
+static cta16_kernel_t cta16_kernel(bool chain, const FusedGeom& fg) {
+    if (fg.nsp == 256 && fg.ns == 256) return chain ? ras_cta16_kernel<true, 256> : ras_cta16_kernel<false, 256>;
     return chain ? ras_cta16_kernel<true, 0> : ras_cta16_kernel<false, 0>;
 }
 
@@ -518,7 +525,7 @@ static cudaError_t cta16_launch(wcras_ctx* ctx, bool chain, int grid, Args... ar
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, cta16_kernel(chain, ctx->fused.nsp), args...);
+    return cudaLaunchKernelEx(&cfg, cta16_kernel(chain, ctx->fused), args...);
 }
 
 // Build the fp16 domain-major operand copy and the domain-major rho_fin buffer; returns 1 if this tier can run the
@@ -543,19 +550,19 @@ int ras_cta16_prepare(wcras_ctx* ctx, const FusedGeom& fg, int nd, const Fields<
         for (int sh = 1; sh >= 0; sh--) {
             const size_t b = cta16_smem(fg.nsp, nface, sh).bytes;
             if (b > (size_t)smem_max) continue;
-            if (cudaFuncSetAttribute(cta16_kernel(false, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess ||
-                cudaFuncSetAttribute(cta16_kernel(true, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) {
+            if (cudaFuncSetAttribute(cta16_kernel(false, fg), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess ||
+                cudaFuncSetAttribute(cta16_kernel(true, fg), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) {
                 cudaGetLastError();
                 continue;
             }
             int n = 0;
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg.nsp), fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cta16_kernel(true, fg), fg.nsp, b) != cudaSuccess) { cudaGetLastError(); n = 0; }
             if (n > best) { best = n; stage_halo = sh; smem = b; }
         }
         per_sm = best;
         if (per_sm < 1) return 0;
-        cudaFuncSetAttribute(cta16_kernel(false, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaFuncSetAttribute(cta16_kernel(true, fg.nsp), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(cta16_kernel(false, fg), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(cta16_kernel(true, fg), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     }
     if (ctx->dm16) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->dm16); ctx->dm16 = nullptr; }
     if (ctx->rf_dm) { cudaStreamSynchronize(ctx->stream); cudaFree(ctx->rf_dm); ctx->rf_dm = nullptr; }

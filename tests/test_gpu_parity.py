@@ -253,6 +253,8 @@ FP16_CASES = [
     (0, (2, 2, 2, 2), 0, 4, 3), (0, (2, 2, 2, 2), 1, 3, 2), (0, (4, 4, 4, 4), 0, 6, 1),
     (1, (4, 4, 4, 4), 0, 2, 3), (1, (4, 4, 4, 4), 0, 5, 1), (1, (8, 4, 4, 2), 0, 3, 3), (1, (4, 4, 4, 4), 1, 2, 2),
     ("ragged", (3, 4, 5, 2), 0, 2, 3), ("ragged", (2, 2, 5, 4), 1, 3, 2), ("ragged", (3, 2, 5, 2), 0, 1, 2),
+    # 240 sites on 256 threads: the run-time-size instance of the kernel at its largest block, 16 padding lanes
+    ("ragged", (3, 4, 5, 4), 0, 2, 3),
     (2, (4, 4, 4, 4), 0, 2, 3), (2, (8, 8, 4, 4), 0, 2, 2), (2, (8, 4, 4, 4), 2, 2, 2),
     # cluster tier with fp16 operand storage staged by TMA (ras_cl16.cu): 2-, 4- and 16-CTA clusters, chained cycles at
     # overlap 0 (the shapes configs[3] names), overlapping domains (6^4 = 1296 sites, 10x6x6x6, 8^4 from 4^4 + 2)
