@@ -294,12 +294,15 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nfc, float mkappa, const uint4* __rest
 
     float U[72];
     unsigned sw = 0;  // MR iterations done by this cluster so far: parity of the exchange mbarrier, index / parity of the dots pair
-    for (int j = 0;; j++) {
-        const int dom = cl + j * ncl;
-        if (dom >= nd) break;
+    // the domain index is carried and the exit test uses has_next from the top of the iteration: recomputed at the bottom
+    // they cost constant-bank loads with every warp waiting on them (see ras_cta16.cu; K_RAS application at 8^4, N_dominv 2,
+    // NRAS 4: 1.380 -> 1.341 ms).  The other two changes made there (small tables at fixed shared-memory offsets, per-launch
+    // uniforms pinned in a register) were measured slower here (1.349 with them, 1.41 with all three) and are not made.
+    for (int j = 0, dom = cl; dom < nd; j++) {
         const unsigned par = (unsigned)j & 1u;
-        const bool has_next = dom + ncl < nd;
-        const int nxt = has_next ? dom + ncl : dom;
+        const int dn = dom + ncl;
+        const bool has_next = dn < nd;
+        const int nxt = has_next ? dn : dom;
         const unsigned dom_bc_here = hb_out ? __ldg(dom_bc + dom) : 0u;
         int4 org_nxt = make_int4(0, 0, 0, 0);
         if (!src_dm) org_nxt = __ldg(dom_org + nxt);  // lattice-layout source: the next residual column is requested below
@@ -518,6 +521,8 @@ ras_cl16_kernel(FusedGeom fg, int nd, int nfc, float mkappa, const uint4* __rest
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
+        if (!has_next) break;
+        dom = dn;
     }
     // no CTA leaves while a store from (or a read of its partials by) another CTA of the cluster could still be under way
     cl_arrive();
