@@ -27,6 +27,14 @@
  * coefficient, taken literally from north_star) -- the implementation of the
  * literal formula is pinned by the closed-form clover matrix test.
  *
+ * Stronger block solver (reading R2):
+ * wco_mr2_block = restarted two-dimensional minimal residual (GMRES(2)): per
+ * pair of D applications the residual is minimised over span{rho, D rho}.
+ * wco_set_block_solver(1) makes wco_ras_apply / wco_sap_apply / the solvers use
+ * it in place of MR.  Pins (tests/test_oracle_mr2.py): dense least squares on a
+ * 2^4 box, exact solution in one cycle for a free-field plane wave (minimal
+ * polynomial of degree 2), never worse than two MR steps.
+ *
  * Reduced-precision operand storage (DESIGN.md reading
  * R1): the same algorithms applied to an operator whose links and site-diagonal
  * matrices A(x) were rounded entry by entry (fp64 -> fp32 -> fp16, round to
@@ -483,6 +491,78 @@ void wco_mr_block(const int L[4], const cplx* U, const cplx* F, double kappa, do
 }
 
 /* ------------------------------------------------------------------ */
+/* Stronger block solver (SURVEY.md 8(f) NEXT-4 "stronger block        */
+/* solvers"; reading R2; the paper only asks for "a fixed    */
+/* iteration solver"): restarted two-dimensional minimal  */
+/* residual = GMRES(2).  niter still counts D applications.            */
+/*   v = 0, rho = P r                                                  */
+/*   for every pair of D applications:                                 */
+/*     q1 = D rho ; q2 = D q1                                          */
+/*     (c1, c2) = argmin | rho - c1 q1 - c2 q2 | :                     */
+/*        a11 c1 + a12 c2 = b1 ; conj(a12) c1 + a22 c2 = b2,           */
+/*        a_ij = <q_i, q_j>, b_i = <q_i, rho>                          */
+/*        det = a11 a22 - |a12|^2 ; if not det > 0 (q2 parallel to q1, */
+/*        or rho = 0): the plain MR step c1 = b1 / a11 (0 if a11 = 0), */
+/*        c2 = 0                                                       */
+/*     v += c1 rho + c2 q1 ; rho -= c1 q1 + c2 q2                      */
+/*   odd niter: one plain MR iteration at the end                      */
+/* ------------------------------------------------------------------ */
+void wco_mr2_block(const int L[4], const cplx* U, const cplx* F, double kappa, double csw,
+                   const int start[4], const int ext[4], int niter, const cplx* r_full, cplx* v_local,
+                   cplx* rho_out) {
+    long n = box_volume(ext), n12 = n * 12;
+    cplx* rho = malloc(sizeof(cplx) * n12);
+    cplx* q1 = malloc(sizeof(cplx) * n12);
+    cplx* q2 = malloc(sizeof(cplx) * n12);
+    for (long k = 0; k < n; k++) { /* projection P_Omega' */
+        int x[4];
+        box_global_coords(L, start, ext, k, x);
+        long i = site_index(L, x);
+        for (int c = 0; c < 12; c++) rho[k * 12 + c] = r_full[i * 12 + c];
+    }
+    for (long k = 0; k < n12; k++) v_local[k] = 0;
+    int it = 0;
+    for (; it + 1 < niter; it += 2) {
+        box_apply_D_local(L, U, F, kappa, csw, start, ext, rho, q1);
+        box_apply_D_local(L, U, F, kappa, csw, start, ext, q1, q2);
+        double a11 = creal(sdot(n12, q1, q1)), a22 = creal(sdot(n12, q2, q2));
+        cplx a12 = sdot(n12, q1, q2), b1 = sdot(n12, q1, rho), b2 = sdot(n12, q2, rho);
+        double det = a11 * a22 - (creal(a12) * creal(a12) + cimag(a12) * cimag(a12));
+        cplx c1, c2;
+        if (det > 0) {
+            c1 = (b1 * a22 - a12 * b2) / det;
+            c2 = (a11 * b2 - conj(a12) * b1) / det;
+        } else {
+            c1 = a11 > 0 ? b1 / a11 : 0;
+            c2 = 0;
+        }
+        for (long k = 0; k < n12; k++) v_local[k] += c1 * rho[k] + c2 * q1[k];
+        for (long k = 0; k < n12; k++) rho[k] -= c1 * q1[k] + c2 * q2[k];
+    }
+    if (it < niter) { /* odd count: a last MR iteration */
+        box_apply_D_local(L, U, F, kappa, csw, start, ext, rho, q1);
+        cplx qr = sdot(n12, q1, rho);
+        double qq = creal(sdot(n12, q1, q1));
+        cplx alpha = qq > 0 ? qr / qq : 0;
+        for (long k = 0; k < n12; k++) v_local[k] += alpha * rho[k];
+        for (long k = 0; k < n12; k++) rho[k] -= alpha * q1[k];
+    }
+    if (rho_out) memcpy(rho_out, rho, sizeof(cplx) * n12);
+    free(rho);
+    free(q1);
+    free(q2);
+}
+
+/* which block solver Alg. 1, SAP and the solvers use: 0 = MR (the configs' "MR block iterations"), 1 = wco_mr2_block */
+static int g_block_solver = 0;
+void wco_set_block_solver(int kind) { g_block_solver = kind; }
+static void block_solve(const int L[4], const cplx* U, const cplx* F, double kappa, double csw, const int start[4],
+                        const int ext[4], int niter, const cplx* r_full, cplx* v_local) {
+    if (g_block_solver == 1) wco_mr2_block(L, U, F, kappa, csw, start, ext, niter, r_full, v_local, NULL);
+    else wco_mr_block(L, U, F, kappa, csw, start, ext, niter, r_full, v_local, NULL);
+}
+
+/* ------------------------------------------------------------------ */
 /* RAS iteration, Algorithm 1 (line numbering as read  */
 /* in Q11).  phi = K_RAS eta.                                          */
 /*  1: phi = 0, r = eta                                                */
@@ -517,7 +597,7 @@ int wco_ras_apply(const int L[4], const cplx* U, const cplx* F, double kappa, do
             wco_domain_box(L, b, s, i, origin, start, ext);
             long n = box_volume(ext);
             cplx* vl = malloc(sizeof(cplx) * n * 12);
-            wco_mr_block(L, U, F, kappa, csw, start, ext, niter, r, vl, NULL);
+            block_solve(L, U, F, kappa, csw, start, ext, niter, r, vl);
             for (long k = 0; k < n; k++) { /* restriction R_Omega_i: bulk sites only */
                 int x[4], bulk = 1;
                 box_global_coords(L, start, ext, k, x);
@@ -585,7 +665,7 @@ int wco_sap_apply(const int L[4], const cplx* U, const cplx* F, double kappa, do
                 wco_domain_box(L, b, 0, i, origin, start, ext);
                 long n = box_volume(ext);
                 cplx* vl = malloc(sizeof(cplx) * n * 12);
-                wco_mr_block(L, U, F, kappa, csw, start, ext, niter, r, vl, NULL);
+                block_solve(L, U, F, kappa, csw, start, ext, niter, r, vl);
                 for (long k = 0; k < n; k++) {
                     int x[4];
                     box_global_coords(L, start, ext, k, x);

@@ -151,6 +151,23 @@ class Operator:
         _load().wco_mr_block(*self._args(), _i4(start), _i4(ext), C.c_int(niter), _p(r_full), _p(v), _p(rho))
         return v, rho
 
+    def mr2_block(self, start, ext, niter, r_full):
+        """(v_local, rho_local) after niter D applications of the restarted two-dimensional minimal residual (GMRES(2),
+        DESIGN.md reading R2) on the box; local index x fastest."""
+        r_full = _c(r_full)
+        n = int(np.prod(ext))
+        v = np.empty((n, 4, 3), np.complex128)
+        rho = np.empty((n, 4, 3), np.complex128)
+        _load().wco_mr2_block(*self._args(), _i4(start), _i4(ext), C.c_int(niter), _p(r_full), _p(v), _p(rho))
+        return v, rho
+
+    def with_block_solver(self, kind):
+        """The same operator with Alg. 1 / SAP / the solvers using block solver `kind`: "mr" or "mr2" (reading R2)."""
+        import copy
+        o = copy.copy(self)
+        o._block_solver = {"mr": 0, "mr2": 1}[kind]
+        return o
+
     def ras_apply(self, block, s, niter, nras, eta):
         eta = _c(eta)
         out = np.empty((self.V, 4, 3), np.complex128)
@@ -230,6 +247,30 @@ def _wrap_explicit(name):
     return call
 
 
-for _n in ("apply_D", "apply_D_sites", "apply_D_box", "mr_block", "ras_apply", "sap_apply", "bicgstab",
+for _n in ("apply_D", "apply_D_sites", "apply_D_box", "mr_block", "mr2_block", "ras_apply", "sap_apply", "bicgstab",
            "nested_bicgstab", "true_residual"):
     setattr(ExplicitOperator, _n, _wrap_explicit(_n))
+
+
+def _wrap_block_solver(cls, name):
+    plain = getattr(cls, name)
+
+    def call(self, *a, **k):
+        kind = getattr(self, "_block_solver", 0)
+        if not kind:
+            return plain(self, *a, **k)
+        lib = _load()
+        lib.wco_set_block_solver(C.c_int(kind))
+        try:
+            return plain(self, *a, **k)
+        finally:
+            lib.wco_set_block_solver(C.c_int(0))
+
+    call.__name__ = name
+    call.__doc__ = plain.__doc__
+    return call
+
+
+for _cls in (Operator, ExplicitOperator):
+    for _n in ("ras_apply", "sap_apply", "bicgstab", "nested_bicgstab"):
+        setattr(_cls, _n, _wrap_block_solver(_cls, _n))
