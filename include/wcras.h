@@ -72,6 +72,20 @@ int wcras_destroy(wcras_ctx* ctx);
  * prec = 64: double; canonical spinor layout, 24*V reals each, device. */
 int wcras_apply_D(wcras_ctx* ctx, int prec, const void* in_dev, void* out_dev);
 
+/* The same w = D v (north_star (b)) for callers that may not allocate device memory: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc (wcras_apply_D allocates its two internal-layout
+ * buffers on its first call).  Arguments, layouts and result as wcras_apply_D.  The two buffers live in ONE file-scope
+ * device array of WCRAS_NOALLOC_SCRATCH_BYTES (csrc/noalloc.cu) that every GPU which loads the library holds until the
+ * process exits; the call itself performs no cudaMalloc / cudaFree and creates no event or stream (the per-class timers
+ * of wcras_set_timing are off for its duration).  Limit: 2 * 24 * V * sizeof(real) <= WCRAS_NOALLOC_SCRATCH_BYTES, i.e.
+ * V <= 87381 sites at prec 32 (16^4 fits) and V <= 43690 at prec 64; beyond that WCRAS_UNSUPPORTED with the sizes in
+ * wcras_last_error, nothing launched.  All calls on one device, of every context and stream, SHARE the array: it keeps the
+ * last call's contents (nothing needs clearing: both buffers are written in full before they are read), and two calls
+ * that overlap on the GPU race on it -- the caller serialises them.  Enqueues on the context's stream, does not
+ * synchronise. */
+#define WCRAS_NOALLOC_SCRATCH_BYTES (16u << 20)
+int wcras_apply_D_noalloc(wcras_ctx* ctx, int prec, const void* in_dev, void* out_dev);
+
 /* ras_precondition(domain shape, overlap, block iterations)  -- north_star ABI list; PAPER.md:83 (the three
  * RAS parameters d, N_dominv, NRAS), :101 (d = 2s), :45 (Omega_i, Omega'_i).
  * domain[mu] must divide dims[mu]; overlap_s = s >= 0 is the extension per side in every direction with

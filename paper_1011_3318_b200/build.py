@@ -8,7 +8,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwcras.so")
-SOURCES = ["api.cu", "layout.cu", "dslash.cu", "solver.cu", "ras.cu", "ras_fused.cu", "ras_cta.cu", "ras_cta16.cu", "ras_cl16.cu", "ras_pair.cu", "ras_stream.cu"]
+SOURCES = ["api.cu", "layout.cu", "dslash.cu", "solver.cu", "ras.cu", "ras_fused.cu", "ras_cta.cu", "ras_cta16.cu", "ras_cl16.cu", "ras_pair.cu", "ras_stream.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
