@@ -117,6 +117,16 @@ int wcras_set_ras_tier(wcras_ctx* ctx, int tier);
  * the other tiers compute with fp32 copies of the rounded fields.  Takes effect at the next wcras_ras_precondition. */
 int wcras_set_operand_precision(wcras_ctx* ctx, int bits);
 
+/* Block solver of the RAS / SAP domains (SURVEY.md 8(f) NEXT-4 "stronger block solvers"; reading R2; the paper
+ * asks only for "a fixed iteration solver", and `configs` name MR).  kind = 0 (default): N_dominv MR iterations
+ * (reading Q9).  kind = 1: restarted two-dimensional minimal residual (GMRES(2)): per PAIR of D_Omega' applications
+ * q1 = D rho, q2 = D q1 the residual is minimised over span{q1, q2} (2x2 normal equations; the plain MR step if their
+ * determinant is not positive); v += c1 rho + c2 q1, rho -= c1 q1 + c2 q2; an odd N_dominv ends with one MR iteration.
+ * N_dominv still counts D_Omega' applications.  Built into the persistent one-CTA-per-domain kernel with 16-bit operand
+ * storage (ras_cta16.cu): with kind = 1 the next wcras_ras_precondition returns WCRAS_UNSUPPORTED unless
+ * wcras_set_operand_precision(ctx, 16) is set and the extended domain has at most 256 sites on the automatic tier. */
+int wcras_set_block_solver(wcras_ctx* ctx, int kind);
+
 /* Order in which the full-lattice Dslash visits the sites (a traversal order only; no layout changes, results are
  * identical): ztile = -1 automatic (default: plain order x,y,z,t; above ~60 MB of operands per t-slice the order
  * x, y, z within a tile, t, z tile, with the largest tile whose slab stays under 30 MB, so that the t-neighbours are

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libwcras.so")
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = [
-    "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_apply_D_noalloc", "wcras_ras_precondition", "wcras_set_ras_tier", "wcras_set_operand_precision", "wcras_set_schwarz", "wcras_set_traversal",
+    "wcras_create", "wcras_destroy", "wcras_apply_D", "wcras_apply_D_noalloc", "wcras_ras_precondition", "wcras_set_ras_tier", "wcras_set_operand_precision", "wcras_set_block_solver", "wcras_set_schwarz", "wcras_set_traversal",
     "wcras_apply_D_restricted", "wcras_ras_apply", "wcras_set_solver", "wcras_set_lookahead", "wcras_set_graphs", "wcras_set_timing", "wcras_solve",
     "wcras_solve_host", "wcras_solve_multi", "wcras_ras_autotune", "wcras_export_clover", "wcras_time_kernel", "wcras_launch_count", "wcras_last_error",
 ]
@@ -125,6 +125,9 @@ class Context:
     def ras_precondition(self, domain, overlap, block_iters, nras=1):
         self._chk(self._lib.wcras_ras_precondition(self._h, _i4(domain), C.c_int(overlap), C.c_int(block_iters),
                                                    C.c_int(nras)))
+
+    def set_block_solver(self, kind):
+        self._chk(self._lib.wcras_set_block_solver(self._h, C.c_int(kind)))
 
     def set_ras_tier(self, tier):
         self._chk(self._lib.wcras_set_ras_tier(self._h, C.c_int(tier)))

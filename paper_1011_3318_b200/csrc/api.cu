@@ -100,6 +100,14 @@ int wcras_set_operand_precision(wcras_ctx* ctx, int bits) {
     return WCRAS_OK;
 }
 
+int wcras_set_block_solver(wcras_ctx* ctx, int kind) {
+    NEED(ctx, "null ctx");
+    ctx->cfg_gen++;  // captured inner-iteration graphs are stale
+    NEED(kind == 0 || kind == 1, "set_block_solver: kind must be 0 (MR) or 1 (two-dimensional minimal residual)");
+    ctx->block_solver = kind;
+    return WCRAS_OK;
+}
+
 int wcras_set_traversal(wcras_ctx* ctx, int ztile) {
     NEED(ctx, "null ctx");
     ctx->cfg_gen++;  // captured inner-iteration graphs are stale

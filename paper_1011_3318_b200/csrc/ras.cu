@@ -296,6 +296,8 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
         // and halo geometry are those of ras_cta_prepare: same CTA shape, one CTA per SM)
         // (tier request 6: the two-threads-per-site variant ras_pair.cu instead -- measured slower, kept for comparison)
         rc.pair = rc.cta && ctx->op_prec == 16 && ctx->tier_request == 6 && ras_pair_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
+        fgeom.mr2 = ctx->block_solver == 1 ? 1 : 0;
+        ctx->fused.mr2 = fgeom.mr2;
         rc.cta16 = rc.cta && ctx->op_prec == 16 && !rc.pair && ras_cta16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
         // 16-bit operand mode on the cluster tier: fp16 operands staged by TMA (ras_cl16.cu); otherwise ras_fused.cu
         rc.cl16 = !rc.cta && ctx->op_prec == 16 && fgeom.C > 1 && ras_cl16_prepare(ctx, fgeom, rc.nd, ras_fields(ctx)) != 0;
@@ -307,6 +309,14 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
             ctx->hb_nrhs = 0;
             ctx->nface = rc.cl16 ? fgeom.C * ctx->cl16_nfc : (nface + 7) / 8 * 8;  // ras_cl16: halo slots per CTA, [nd][C][8][3][nfc]
         }
+    }
+    if (ctx->block_solver == 1 && !rc.cta16) {
+        // the second block solver lives in the persistent one-CTA-per-domain kernel with 16-bit operand storage only
+        ctx->ras.set = false;
+        snprintf(ctx->err, sizeof ctx->err,
+                 "ras_precondition: block solver 1 (two-dimensional minimal residual) needs 16-bit operand storage and an "
+                 "extended domain of at most 256 sites on the automatic tier");
+        return WCRAS_UNSUPPORTED;
     }
     ctx->ras = rc;
     return WCRAS_OK;

@@ -93,10 +93,10 @@ struct Cta16Smem {  // offsets in float4 units
 // stage_halo costs a constant-bank load wherever the compiler rematerialises it (measured ~300 cycles, once per domain).
 __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_halo) {
     Cta16Smem s;
-    s.red = 0;
-    s.bars = 8;
-    s.org = 10;
-    s.hbuf = 16;  // 256-byte offset: bulk-copy destinations stay 128-byte aligned
+    s.red = 0;    // [2][8] warp partials (the second row for the five dots of the MR2 block solver)
+    s.bars = 16;
+    s.org = 18;
+    s.hbuf = 24;  // 384-byte offset: bulk-copy destinations stay 128-byte aligned
     s.opbuf = s.hbuf + 24 * nsp;
     s.rstage = s.opbuf + 18 * nsp;
     s.hstage = s.rstage + 6 * nsp;
@@ -108,9 +108,10 @@ __host__ __device__ inline Cta16Smem cta16_smem(int nsp, int nface, int stage_ha
 //   r_lat   residual source in the lattice layout (cycle 0 / first visit), or nullptr
 //   r_dm    residual source domain-major [nd][6][nsp] (rho_fin of the previous cycle), or nullptr
 //   rho_dm  rho_fin of this cycle, domain-major, or nullptr (then the last MR residual update is skipped, Q12)
+//   MR2     block solver: restarted two-dimensional minimal residual (reading R2) instead of MR
 //   NSP     threads per CTA = sites per domain as a compile-time constant (256, no padding lanes: every slot, operand and
 //           staging offset becomes an immediate and every thread is active), or 0 = fg.nsp / fg.ns at run time
-template <bool CHAIN, int NSP>
+template <bool CHAIN, int NSP, bool MR2>
 __global__ void __launch_bounds__(FUSED_CTA_MAX_THREADS, 1)
 ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, float mkappa, const uint4* __restrict__ dm16,
                  const float4* __restrict__ r_lat, const float4* __restrict__ r_dm, const float4* __restrict__ hb_in,
@@ -173,7 +174,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #define WC_FIDX(MU) ((int)((fidx_pk >> (8 * (MU))) & 255u))
 #pragma unroll
     for (int j = 0; j < 24; j++) hbuf[j * nsp + k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (k < FUSED_CTA_MAX_THREADS / 32) red[k] = make_float4(0.f, 0.f, 0.f, 0.f);  // warps that do not exist contribute zero
+    if (k < 2 * (FUSED_CTA_MAX_THREADS / 32)) red[k] = make_float4(0.f, 0.f, 0.f, 0.f);  // warps that do not exist contribute zero
     if (k == 0) {
         mbar_init(bar_links, 1);
         mbar_init(bar_clov, 1);
@@ -337,30 +338,31 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         for (int n = 0; n < 24; n++) v[n] = 0.f;
         WC_T(5)
 
-        for (int it = 0; it < fg.niter; it++) {
+        // q = D_Omega' in for sweep number it of this domain (the staging requests of the next domain hang on it): scatter
+        // of the projected half spinors, clover term, barrier, gather
+        auto apply_D = [&](const float (&in)[24], float (&q)[24], int it) {
             {
                 float hs[12], g[12];
 #define WC_SCATTER(MU)                                       \
-    project<float, MU, -1>(rho, hs);                         \
+    project<float, MU, -1>(in, hs);                          \
     st_half_pred(dst[2 * MU], chunk_bytes, hs);              \
-    project<float, MU, +1>(rho, hs);                         \
+    project<float, MU, +1>(in, hs);                          \
     su3_adj_mul<float>(U + 18 * MU, hs, g);                  \
     st_half_pred(dst[2 * MU + 1], chunk_bytes, g);
                 WC_SCATTER(0) WC_SCATTER(1) WC_SCATTER(2) WC_SCATTER(3)
 #undef WC_SCATTER
             }
-            float q[24];
             WC_T(6)
             if (it == 0) mbar_wait(bar_clov, par);
             WC_T(7)
-            // q = A rho from the staged fp16 clover blocks: block 0 = halfs 0..35 (chunks 9..13), block 1 = halfs
+            // q = A in from the staged fp16 clover blocks: block 0 = halfs 0..35 (chunks 9..13), block 1 = halfs
             // 36..71 (chunks 13..17, chunk 13 read twice)
 #pragma unroll
             for (int ch = 0; ch < 2; ch++) {
                 float Ab[40];
 #pragma unroll
                 for (int c = 0; c < 5; c++) half8_to_float(opbuf[(9 + 4 * ch + c) * nsp + k], Ab + 8 * c);
-                herm6_mul<float>(Ab + 4 * ch, rho + 12 * ch, q + 12 * ch);
+                herm6_mul<float>(Ab + 4 * ch, in + 12 * ch, q + 12 * ch);
             }
             WC_T(8)
             __syncthreads();
@@ -386,6 +388,76 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                 WC_GATHER(0) WC_GATHER(1) WC_GATHER(2) WC_GATHER(3)
 #undef WC_GATHER
             }
+        };
+        int it = 0;
+        if (MR2) {
+            // Restarted two-dimensional minimal residual (reading R2): per pair of sweeps q1 = D rho, q2 = D q1, then
+            // (c1, c2) = argmin |rho - c1 q1 - c2 q2| from the 2x2 normal equations; v += c1 rho + c2 q1; rho -= c1 q1 + c2 q2
+            for (; it + 1 < fg.niter; it += 2) {
+                float q1[24], q2[24];
+                apply_D(rho, q1, it);
+                __syncthreads();  // every thread is past its gather: the slots may be rewritten
+                apply_D(q1, q2, it + 1);
+                float e[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};  // b1 (re, im), a11, b2 (re, im), a22, a12 (re, im)
+#pragma unroll
+                for (int n = 0; n < 12; n++) {
+                    const float ar_ = q1[2 * n], ai_ = q1[2 * n + 1], br_ = q2[2 * n], bi_ = q2[2 * n + 1], rr = rho[2 * n], ri = rho[2 * n + 1];
+                    e[0] = fmaf(ar_, rr, e[0]); e[0] = fmaf(ai_, ri, e[0]); e[1] = fmaf(ar_, ri, e[1]); e[1] = fmaf(-ai_, rr, e[1]);
+                    e[2] = fmaf(ar_, ar_, e[2]); e[2] = fmaf(ai_, ai_, e[2]);
+                    e[3] = fmaf(br_, rr, e[3]); e[3] = fmaf(bi_, ri, e[3]); e[4] = fmaf(br_, ri, e[4]); e[4] = fmaf(-bi_, rr, e[4]);
+                    e[5] = fmaf(br_, br_, e[5]); e[5] = fmaf(bi_, bi_, e[5]);
+                    e[6] = fmaf(ar_, br_, e[6]); e[6] = fmaf(ai_, bi_, e[6]); e[7] = fmaf(ar_, bi_, e[7]); e[7] = fmaf(-ai_, br_, e[7]);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                    for (int n = 0; n < 8; n++) e[n] += __shfl_xor_sync(0xffffffffu, e[n], o);
+                if (lane == 0) {
+                    red[warp] = make_float4(e[0], e[1], e[2], e[3]);
+                    red[FUSED_CTA_MAX_THREADS / 32 + warp] = make_float4(e[4], e[5], e[6], e[7]);
+                }
+                __syncthreads();
+                float t[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int n = 0; n < FUSED_CTA_MAX_THREADS / 32; n++) {
+                    const float4 p = red[n], p2 = red[FUSED_CTA_MAX_THREADS / 32 + n];
+                    t[0] += p.x; t[1] += p.y; t[2] += p.z; t[3] += p.w; t[4] += p2.x; t[5] += p2.y; t[6] += p2.z; t[7] += p2.w;
+                }
+                const float b1r = t[0], b1i = t[1], a11 = t[2], b2r = t[3], b2i = t[4], a22 = t[5], a12r = t[6], a12i = t[7];
+                const float det = a11 * a22 - (a12r * a12r + a12i * a12i);
+                float c1r, c1i, c2r = 0.f, c2i = 0.f;
+                if (det > 0.f) {
+                    const float inv = 1.f / det;
+                    c1r = (b1r * a22 - (a12r * b2r - a12i * b2i)) * inv;  // c1 = (b1 a22 - a12 b2) / det
+                    c1i = (b1i * a22 - (a12r * b2i + a12i * b2r)) * inv;
+                    c2r = (a11 * b2r - (a12r * b1r + a12i * b1i)) * inv;  // c2 = (a11 b2 - conj(a12) b1) / det
+                    c2i = (a11 * b2i - (a12r * b1i - a12i * b1r)) * inv;
+                } else {  // q2 parallel to q1, or rho = 0: the plain MR step
+                    const float inv = a11 > 0.f ? 1.f / a11 : 0.f;
+                    c1r = b1r * inv; c1i = b1i * inv;
+                }
+                const bool upd_rho = it + 2 < fg.niter || WC_UNI_RHO;
+#pragma unroll
+                for (int n = 0; n < 12; n++) {
+                    const float rr = rho[2 * n], ri = rho[2 * n + 1], xr = q1[2 * n], xi = q1[2 * n + 1];
+                    float vr = v[2 * n], vi = v[2 * n + 1];
+                    vr = fmaf(c1r, rr, vr); vr = fmaf(-c1i, ri, vr); vr = fmaf(c2r, xr, vr); vr = fmaf(-c2i, xi, vr);
+                    vi = fmaf(c1r, ri, vi); vi = fmaf(c1i, rr, vi); vi = fmaf(c2r, xi, vi); vi = fmaf(c2i, xr, vi);
+                    v[2 * n] = vr; v[2 * n + 1] = vi;
+                    if (upd_rho) {
+                        const float yr = q2[2 * n], yi = q2[2 * n + 1];
+                        float nr = rr, ni = ri;
+                        nr = fmaf(-c1r, xr, nr); nr = fmaf(c1i, xi, nr); nr = fmaf(-c2r, yr, nr); nr = fmaf(c2i, yi, nr);
+                        ni = fmaf(-c1r, xi, ni); ni = fmaf(-c1i, xr, ni); ni = fmaf(-c2r, yi, ni); ni = fmaf(-c2i, yr, ni);
+                        rho[2 * n] = nr; rho[2 * n + 1] = ni;
+                    }
+                }
+                // (the barrier inside the next apply_D separates these reads of the partial table from its next writes)
+            }
+        }
+        for (; it < fg.niter; it++) {
+            float q[24];
+            apply_D(rho, q, it);
             float d0 = 0.f, d1 = 0.f, d2 = 0.f;
 #ifdef WC_X2
             x2::mr_dots(q, rho, d0, d1, d2);
@@ -504,8 +576,12 @@ typedef void (*cta16_kernel_t)(FusedGeom, int, int, int, int, float, const uint4
                                const float4*, float4*, float4*, const int4*, const unsigned*);
 // the NSP = 256 instance: domains of exactly 256 sites (no padding lane: the kernel takes every thread as active)
 static cta16_kernel_t cta16_kernel(bool chain, const FusedGeom& fg) {
-    if (fg.nsp == 256 && fg.ns == 256) return chain ? ras_cta16_kernel<true, 256> : ras_cta16_kernel<false, 256>;
-    return chain ? ras_cta16_kernel<true, 0> : ras_cta16_kernel<false, 0>;
+    if (fg.mr2) {
+        if (fg.nsp == 256 && fg.ns == 256) return chain ? ras_cta16_kernel<true, 256, true> : ras_cta16_kernel<false, 256, true>;
+        return chain ? ras_cta16_kernel<true, 0, true> : ras_cta16_kernel<false, 0, true>;
+    }
+    if (fg.nsp == 256 && fg.ns == 256) return chain ? ras_cta16_kernel<true, 256, false> : ras_cta16_kernel<false, 256, false>;
+    return chain ? ras_cta16_kernel<true, 0, false> : ras_cta16_kernel<false, 0, false>;
 }
 
 int ensure_halo(wcras_ctx* ctx, int nrhs);  // ras_cta.cu

@@ -135,6 +135,7 @@ struct FusedGeom {
     int V, s, ns, nsp, C, niter;
     int nclus;       // tier 2b: clusters (or CTAs) resident at once = persistent grid size in clusters
     int pdir;        // multiplicative Schwarz: pairing direction of the red-black domain enumeration, -1 = not colourable
+    int mr2 = 0;     // block solver: 1 = restarted two-dimensional minimal residual (reading R2; ras_cta16.cu only)
     const int* stop; // device flag of the running inner solver (see wc::Geom::stop), or nullptr
 };
 
@@ -183,6 +184,7 @@ struct wcras_ctx {
     unsigned* dom_bc = nullptr;    //            block coordinates of every domain, 8 bits each
     int stage_halo = 0;            // ras_cta16: halo slots staged in shared memory
     int stream_half = 0;           // ras_stream: operand records packed as fp16
+    int block_solver = 0;          // wcras_set_block_solver: 0 = MR, 1 = two-dimensional minimal residual (reading R2)
     size_t cta16_smem = 0;         // its dynamic shared memory
     float4* r16a = nullptr;        // fp32 copies of the fp16-rounded links and clover blocks (16-bit operand mode):
     float2* r16b = nullptr;        //   operands of every K_RAS path that does not read dm16

@@ -336,6 +336,81 @@ def test_fp16_operands_sap_and_solve():
         cs.ctx.set_solver(use_ras=False)
 
 
+MR2_CASES = [
+    # (case, block, overlap, N_dominv, NRAS): the second block solver (restarted two-dimensional minimal residual, reading
+    # R2) in the persistent fp16-operand kernel: pairs only, pairs + a last MR iteration (odd N_dominv), N_dominv 1 (MR
+    # alone), chained cycles, overlap with wrap-around, ragged domains with padding lanes
+    (0, (2, 2, 2, 2), 0, 4, 3), (0, (2, 2, 2, 2), 1, 3, 2), (1, (4, 4, 4, 4), 0, 2, 1), (1, (4, 4, 4, 4), 0, 2, 4),
+    (1, (4, 4, 4, 4), 0, 5, 2), (1, (4, 4, 4, 4), 0, 1, 2), (1, (8, 4, 4, 2), 0, 4, 3), ("ragged", (3, 4, 5, 2), 0, 4, 2),
+    ("ragged", (3, 4, 5, 4), 0, 2, 3), ("ragged", (2, 2, 2, 2), 1, 3, 2),
+]
+
+
+@pytest.mark.parametrize("tier", [0, 4])
+@pytest.mark.parametrize("which,block,s,nit,nras", MR2_CASES)
+def test_ras_apply_mr2_block_solver(which, block, s, nit, nras, tier):
+    """wcras_set_block_solver(1) (SURVEY 8(f) NEXT-4 stronger block solvers, reading R2) against the oracle's
+    Alg. 1 with wco_mr2_block on its own fp16 rounding of the operands; tier 4 = cycles not chained."""
+    cs = ragged_case() if which == "ragged" else case(which)
+    cs.ctx.set_ras_tier(tier)
+    cs.ctx.set_operand_precision(16)
+    cs.ctx.set_block_solver(1)
+    try:
+        cs.ctx.ras_precondition(block, s, nit, nras)
+        r32 = I.spinor(cs.dims, 61).astype(np.complex64).astype(np.complex128)
+        op2 = rounded_op(cs).with_block_solver("mr2")
+        want = op2.ras_apply(block, s, nit, nras, r32)
+        got = cs.ras_apply(r32)
+        assert rel(got, want) <= TOL_RAS
+        if nit >= 2:  # and it is not MR: the two block solvers differ by far more than the tolerance
+            assert rel(got, rounded_op(cs).ras_apply(block, s, nit, nras, r32)) > 2 * TOL_RAS
+    finally:
+        cs.ctx.set_block_solver(0)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_ras_tier(0)
+
+
+def test_mr2_block_solver_sap_solve_and_limits():
+    """The second block solver through multiplicative Schwarz and through the nested solve (true residual by the oracle on
+    the exact operator); UNSUPPORTED where the kernel that holds it does not run (fp32 operands, larger domains)."""
+    cs = case(1)
+    cs.ctx.set_ras_tier(0)
+    cs.ctx.set_operand_precision(16)
+    cs.ctx.set_block_solver(1)
+    try:
+        r32 = I.spinor(cs.dims, 62).astype(np.complex64).astype(np.complex128)
+        op2 = rounded_op(cs).with_block_solver("mr2")
+        for block, nit, ncyc in (((4, 4, 4, 4), 4, 2), ((8, 4, 4, 2), 3, 2)):
+            cs.ctx.ras_precondition(block, 0, nit, ncyc)
+            cs.ctx.set_schwarz(True)
+            assert rel(cs.ras_apply(r32), op2.sap_apply(block, nit, ncyc, r32)) <= TOL_RAS
+            cs.ctx.set_schwarz(False)
+        eta = I.spinor(cs.dims, 2)
+        cs.ctx.set_solver(use_ras=False)
+        _, i0 = cs.solve(eta)
+        for nit, nras in ((2, 3), (4, 2)):
+            cs.ctx.ras_precondition((4, 4, 4, 4), 0, nit, nras)
+            cs.ctx.set_solver(use_ras=True)
+            phi, info = cs.solve(eta, 1e-12)
+            assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
+            assert info["inner_iters"] < i0["inner_iters"]
+            # (a smaller block residual does not always make a better preconditioner: the iteration count may go either way
+            # against MR by one on this lattice, so it is reported by bench.py's survey rows, not asserted)
+        for bits, block, s in ((32, (4, 4, 4, 4), 0), (16, (4, 4, 4, 4), 1), (16, (8, 8, 4, 4), 0)):
+            cs.ctx.set_operand_precision(bits)
+            with pytest.raises(binding.WcrasError) as e:
+                cs.ctx.ras_precondition(block, s, 2, 1)
+            assert e.value.code == binding.UNSUPPORTED
+        with pytest.raises(binding.WcrasError) as e:
+            cs.ctx.set_block_solver(2)
+        assert e.value.code == binding.INVALID_ARG
+    finally:
+        cs.ctx.set_block_solver(0)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_solver(use_ras=False)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 4, 1)   # leave a valid configuration behind
+
+
 SAP_CASES = [
     (0, (2, 2, 2, 2), 4, 1), (0, (2, 2, 2, 2), 4, 3), (1, (4, 4, 4, 4), 3, 1), (1, (4, 4, 4, 4), 2, 2),
     (1, (8, 4, 4, 2), 2, 3), ("ragged", (3, 2, 5, 2), 3, 2),
