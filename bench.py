@@ -342,6 +342,15 @@ def main():
         for bits in (32, 16):
             configure(SAP, bits, sap=True)
             side["sap_%s_it%d_ncycle%d_op%d" % ("x".join(map(str, SAP["domain"])), SAP["block_iters"], SAP["ncycle"], bits)] = measure()
+        # the second block solver (wcras_set_block_solver(1), reading R2: restarted two-dimensional minimal
+        # residual) at the SAP point above and at the timed RAS point: same iteration counts on this well-conditioned field,
+        # so it only costs its three extra dots here; it pays on the near-critical field (hard_regime)
+        ctx.set_block_solver(1)
+        configure(SAP, 16, sap=True)
+        side["sap_%s_it%d_ncycle%d_op16_mr2" % ("x".join(map(str, SAP["domain"])), SAP["block_iters"], SAP["ncycle"])] = measure()
+        configure(RAS, 16)
+        side["ras_%s_op16_mr2" % ras_label(RAS)] = measure()
+        ctx.set_block_solver(0)
         ctx.set_schwarz(False)
         configure(RAS, 32)
         side["ras_%s_op32" % ras_label(RAS)] = measure()
@@ -472,6 +481,13 @@ def main():
         ch.ras_precondition((4, 4, 4, 4), 0, 5, 3)
         ch.set_schwarz(True)
         hrun("sap_4x4x4x4_it5_ncycle3_op16")
+        ch.set_block_solver(1)                       # second block solver (reading R2) at its best surveyed points here
+        ch.ras_precondition((4, 4, 4, 4), 0, 6, 3)
+        hrun("sap_4x4x4x4_it6_ncycle3_op16_mr2")
+        ch.set_schwarz(False)
+        ch.ras_precondition((4, 4, 4, 4), 0, 4, 3)
+        hrun("ras_4x4x4x4_it4_nras3_op16_mr2")
+        ch.set_block_solver(0)
         del ch, eh, ph
         torch.cuda.empty_cache()
 

@@ -200,6 +200,7 @@ typedef struct {
     int overlap_s, block_iters, nras;
     int schwarz;        /* 0 = additive (RAS, the paper's method), 1 = multiplicative (SAP; nras = red-black cycles) */
     int operand_bits;   /* block-solver operand storage, 32 or 16 (wcras_set_operand_precision); 0 in the no-preconditioner row */
+    int block_solver;   /* 0 = MR, 1 = two-dimensional minimal residual (wcras_set_block_solver) */
     int status;         /* status of the timed solve (WCRAS_OK, NOT_CONVERGED, BREAKDOWN) or WCRAS_UNSUPPORTED */
     int inner_iters, ras_applies;
     double ms;          /* device time of the timed solve */
@@ -214,9 +215,12 @@ typedef struct {
  *              8x4x4x4, 8x8x4x4 and 8^4, each at (N_dominv, NRAS) in {(2,3),(2,2),(2,4),(3,2),(3,3),(4,1),(4,2),(4,3),(5,3)}
  *              ((5,3) is the paper's best point), with the operand precision the context is set to;
  *   stage 2    around the fastest row so far: the rectangle N_dominv 1..8 x NRAS 1..5 on its shape; overlap s = 1, 2
- *              (the paper's d = 2, 4) and multiplicative Schwarz on the three fastest shapes; the other operand precision.
+ *              (the paper's d = 2, 4) and multiplicative Schwarz on the three fastest shapes; the other operand precision;
+ *   stage 3    if the fastest row so far has overlap 0 and blocks of <= 256 sites: the second block solver
+ *              (wcras_set_block_solver(1)) on its shape with 16-bit operands, N_dominv 2, 4, 6 x 2, 3 cycles, multiplicative
+ *              and additive.
  * The fastest converged candidate is left configured (wcras_ras_precondition, wcras_set_schwarz, wcras_set_operand_precision,
- * use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.  table_host (may be NULL, room for max_rows rows)
+ * wcras_set_block_solver, use_ras; use_ras = 0 if no preconditioner wins) and returned in *best.  table_host (may be NULL, room for max_rows rows)
  * receives the rows tried, *nrows their number.  On a CUDA error the previous configuration is put back.
  * eta_dev: device, canonical fp64.  Uses the workspace of wcras_solve plus one scratch solution vector. */
 int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int max_rows, wcras_tune_row* best,

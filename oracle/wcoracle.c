@@ -501,12 +501,18 @@ void wco_mr_block(const int L[4], const cplx* U, const cplx* F, double kappa, do
 /*     (c1, c2) = argmin | rho - c1 q1 - c2 q2 | :                     */
 /*        a11 c1 + a12 c2 = b1 ; conj(a12) c1 + a22 c2 = b2,           */
 /*        a_ij = <q_i, q_j>, b_i = <q_i, rho>                          */
-/*        det = a11 a22 - |a12|^2 ; if not det > 0 (q2 parallel to q1, */
-/*        or rho = 0): the plain MR step c1 = b1 / a11 (0 if a11 = 0), */
-/*        c2 = 0                                                       */
+/*        g = (a12/a11)(conj(a12)/a22) (cos^2 of the angle of q1, q2;  */
+/*        1 if a11 or a22 is 0).  If 1 - g <= 1e-4 (q2 numerically par. */
+/*        to q1, or rho = 0): the plain MR step c1 = b1 / a11 (0 if    */
+/*        a11 = 0), c2 = 0.  Otherwise, with the rows divided by a11   */
+/*        and a22 (no product of two squared norms: a tiny rho must    */
+/*        not underflow), u_i = b_i / a_ii, m1 = a12 / a11,            */
+/*        m2 = conj(a12) / a22: c1 = (u1 - m1 u2) / (1 - g),           */
+/*        c2 = (u2 - m2 u1) / (1 - g)                                  */
 /*     v += c1 rho + c2 q1 ; rho -= c1 q1 + c2 q2                      */
 /*   odd niter: one plain MR iteration at the end                      */
 /* ------------------------------------------------------------------ */
+#define WCO_MR2_DELTA 1e-4
 void wco_mr2_block(const int L[4], const cplx* U, const cplx* F, double kappa, double csw,
                    const int start[4], const int ext[4], int niter, const cplx* r_full, cplx* v_local,
                    cplx* rho_out) {
@@ -527,11 +533,13 @@ void wco_mr2_block(const int L[4], const cplx* U, const cplx* F, double kappa, d
         box_apply_D_local(L, U, F, kappa, csw, start, ext, q1, q2);
         double a11 = creal(sdot(n12, q1, q1)), a22 = creal(sdot(n12, q2, q2));
         cplx a12 = sdot(n12, q1, q2), b1 = sdot(n12, q1, rho), b2 = sdot(n12, q2, rho);
-        double det = a11 * a22 - (creal(a12) * creal(a12) + cimag(a12) * cimag(a12));
+        /* scale-free form of the 2x2 solve: rows divided by a11 and a22; g = cos^2 of the angle between q1 and q2 */
+        double g = (a11 > 0 && a22 > 0) ? creal((a12 / a11) * (conj(a12) / a22)) : 1.0; /* no product a11 a22: it may underflow */
         cplx c1, c2;
-        if (det > 0) {
-            c1 = (b1 * a22 - a12 * b2) / det;
-            c2 = (a11 * b2 - conj(a12) * b1) / det;
+        if (1.0 - g > WCO_MR2_DELTA) {
+            cplx u1 = b1 / a11, u2 = b2 / a22, m1 = a12 / a11, m2 = conj(a12) / a22;
+            c1 = (u1 - m1 * u2) / (1.0 - g);
+            c2 = (u2 - m2 * u1) / (1.0 - g);
         } else {
             c1 = a11 > 0 ? b1 / a11 : 0;
             c2 = 0;

@@ -35,7 +35,7 @@ class WcrasInfo(C.Structure):
 
 class WcrasTuneRow(C.Structure):
     _fields_ = [("domain", C.c_int * 4), ("overlap_s", C.c_int), ("block_iters", C.c_int), ("nras", C.c_int),
-                ("schwarz", C.c_int), ("operand_bits", C.c_int), ("status", C.c_int), ("inner_iters", C.c_int), ("ras_applies", C.c_int), ("ms", C.c_double),
+                ("schwarz", C.c_int), ("operand_bits", C.c_int), ("block_solver", C.c_int), ("status", C.c_int), ("inner_iters", C.c_int), ("ras_applies", C.c_int), ("ms", C.c_double),
                 ("rel_resid_true", C.c_double)]
 
     def asdict(self):

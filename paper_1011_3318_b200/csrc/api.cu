@@ -236,28 +236,32 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
     const int* L = ctx->geom.L;
     // what the caller had configured, put back if the survey dies on a CUDA error
     const RasConfig prev = ctx->ras;
-    const int prev_use = ctx->use_ras, prev_schwarz = ctx->schwarz, prev_bits = ctx->op_prec;
+    const int prev_use = ctx->use_ras, prev_schwarz = ctx->schwarz, prev_bits = ctx->op_prec, prev_solver = ctx->block_solver;
     auto restore = [&]() {
-        ctx->use_ras = prev_use; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits;
+        ctx->use_ras = prev_use; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits; ctx->block_solver = prev_solver;
         if (prev.set) ras_configure(ctx, prev.b, prev.s, prev.niter, prev.nras);
     };
     std::vector<wcras_tune_row> rows;
     double* phi = (double*)ctx->io_b;
     int ibest = -1;
+    int cur_solver = 0;  // block solver of the candidates being run (stages 0-2: MR, the block solver `configs` name)
     // run one candidate (untimed, then timed solve) and append its row; returns WCRAS_CUDA_ERROR or WCRAS_OK
     auto run = [&](const int b[4], int s, int it, int nras, int sap, int bits) -> int {
         if ((int)rows.size() >= max_rows) return WCRAS_OK;
         for (const wcras_tune_row& o : rows)  // already tried
             if (o.domain[0] == b[0] && o.domain[1] == b[1] && o.domain[2] == b[2] && o.domain[3] == b[3] && o.overlap_s == s &&
-                o.block_iters == it && o.nras == nras && o.schwarz == sap && (it == 0 || o.operand_bits == bits)) return WCRAS_OK;
+                o.block_iters == it && o.nras == nras && o.schwarz == sap && (it == 0 || (o.operand_bits == bits && o.block_solver == cur_solver)))
+                return WCRAS_OK;
         wcras_tune_row r = {};
         for (int mu = 0; mu < 4; mu++) r.domain[mu] = b[mu];
         r.overlap_s = s; r.block_iters = it; r.nras = nras; r.schwarz = sap; r.operand_bits = it ? bits : 0;
+        r.block_solver = it ? cur_solver : 0;
         if (it == 0) {
             ctx->use_ras = 0;
         } else {
             ctx->op_prec = bits;
             ctx->schwarz = sap;
+            ctx->block_solver = cur_solver;
             const int rc = ras_configure(ctx, b, s, it, nras);
             if (rc == WCRAS_CUDA_ERROR) return rc;
             if (rc) { r.status = WCRAS_UNSUPPORTED; rows.push_back(r); return WCRAS_OK; }
@@ -326,6 +330,19 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
         }
         const wcras_tune_row now = rows[ibest];
         if (now.block_iters) WC_RUN(now.domain, now.overlap_s, now.block_iters, now.nras, now.schwarz, bits0 == 16 ? 32 : 16);
+        // ---- stage 3: the second block solver (wcras_set_block_solver(1), reading R2) where its kernel runs: 16-bit
+        // operands, overlap 0, the fastest persistent-tier shape so far; N_dominv 2, 4, 6 x 2, 3 cycles, additive and
+        // multiplicative (its best points are not MR's: fewer, longer cycles) ----
+        const wcras_tune_row lead = rows[ibest];
+        long lead_sites = 1;
+        for (int mu = 0; mu < 4; mu++) lead_sites *= lead.domain[mu];
+        if (lead.block_iters && lead.overlap_s == 0 && lead_sites <= 256) {
+            cur_solver = 1;
+            for (int sap = 1; sap >= 0; sap--)
+                for (int it = 2; it <= 6; it += 2)
+                    for (int nras = 2; nras <= 3; nras++) WC_RUN(lead.domain, 0, it, nras, sap, 16);
+            cur_solver = 0;
+        }
     }
 #undef WC_RUN
     if (table_host) for (size_t k = 0; k < rows.size(); k++) table_host[k] = rows[k];
@@ -336,10 +353,14 @@ int wcras_ras_autotune(wcras_ctx* ctx, const double* eta_dev, double tol, int ma
         return WCRAS_NOT_CONVERGED;
     }
     *best = rows[ibest];
-    if (best->block_iters == 0) { ctx->use_ras = 0; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits; return WCRAS_OK; }
+    if (best->block_iters == 0) {
+        ctx->use_ras = 0; ctx->schwarz = prev_schwarz; ctx->op_prec = prev_bits; ctx->block_solver = prev_solver;
+        return WCRAS_OK;
+    }
     ctx->use_ras = 1;
     ctx->schwarz = best->schwarz;
     ctx->op_prec = best->operand_bits;
+    ctx->block_solver = best->block_solver;
     return ras_configure(ctx, best->domain, best->overlap_s, best->block_iters, best->nras);
 }
 

@@ -424,17 +424,20 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                     t[0] += p.x; t[1] += p.y; t[2] += p.z; t[3] += p.w; t[4] += p2.x; t[5] += p2.y; t[6] += p2.z; t[7] += p2.w;
                 }
                 const float b1r = t[0], b1i = t[1], a11 = t[2], b2r = t[3], b2i = t[4], a22 = t[5], a12r = t[6], a12i = t[7];
-                const float det = a11 * a22 - (a12r * a12r + a12i * a12i);
-                float c1r, c1i, c2r = 0.f, c2i = 0.f;
-                if (det > 0.f) {
-                    const float inv = 1.f / det;
-                    c1r = (b1r * a22 - (a12r * b2r - a12i * b2i)) * inv;  // c1 = (b1 a22 - a12 b2) / det
-                    c1i = (b1i * a22 - (a12r * b2i + a12i * b2r)) * inv;
-                    c2r = (a11 * b2r - (a12r * b1r + a12i * b1i)) * inv;  // c2 = (a11 b2 - conj(a12) b1) / det
-                    c2i = (a11 * b2i - (a12r * b1i - a12i * b1r)) * inv;
-                } else {  // q2 parallel to q1, or rho = 0: the plain MR step
-                    const float inv = a11 > 0.f ? 1.f / a11 : 0.f;
-                    c1r = b1r * inv; c1i = b1i * inv;
+                // scale-free 2x2 solve (reading R2): rows divided by a11 and a22, g = cos^2 of the angle between q1 and q2.  No
+                // product of two squared norms: late in an inner solve they are ~1e-25 each and a11 a22 would underflow (a
+                // denormal determinant turned into inf * 0 = NaN).  Squared norms below FLT_MIN count as zero.
+                const float s1 = a11 >= 1.17549435e-38f ? 1.f / a11 : 0.f, s2 = a22 >= 1.17549435e-38f ? 1.f / a22 : 0.f;
+                const float u1r = b1r * s1, u1i = b1i * s1, u2r = b2r * s2, u2i = b2i * s2;
+                const float m1r = a12r * s1, m1i = a12i * s1, m2r = a12r * s2, m2i = -a12i * s2;  // a12 / a11, conj(a12) / a22
+                const float g = s1 > 0.f && s2 > 0.f ? m1r * m2r - m1i * m2i : 1.f;              // m1 m2 = |a12|^2 / (a11 a22), real
+                float c1r = u1r, c1i = u1i, c2r = 0.f, c2i = 0.f;  // q2 numerically parallel to q1, or rho = 0: the plain MR step
+                if (1.f - g > 1e-4f) {
+                    const float inv = 1.f / (1.f - g);
+                    c1r = (u1r - (m1r * u2r - m1i * u2i)) * inv;  // c1 = (u1 - m1 u2) / (1 - g)
+                    c1i = (u1i - (m1r * u2i + m1i * u2r)) * inv;
+                    c2r = (u2r - (m2r * u1r - m2i * u1i)) * inv;  // c2 = (u2 - m2 u1) / (1 - g)
+                    c2i = (u2i - (m2r * u1i + m2i * u1r)) * inv;
                 }
                 const bool upd_rho = it + 2 < fg.niter || WC_UNI_RHO;
 #pragma unroll

@@ -655,6 +655,7 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         if (int r2 = dslash<double>(ctx, phi, res, eta, nr == 1 ? 3 : 0, nullptr, ctx->sc64)) return r2;
         rn2 = 0;
         double worst = 0;
+        bool nonfinite = false;
         for (int k = 0; k < nr; k++) {  // the true residual of every system on its own
             if (nr > 1) {
                 TimedRegion tr(ctx, TC_BLAS);
@@ -666,7 +667,9 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
             const double ek = nr > 1 ? 1.0 : en2;  // |eta_k|^2 (unit after scaling)
             rel_k[k] = norm_k[k] > 0 ? std::sqrt(nk / ek) : 0.0;
             worst = rel_k[k] > worst ? rel_k[k] : worst;
+            nonfinite = nonfinite || !std::isfinite(rel_k[k]);
         }
+        if (nonfinite) { status = WCRAS_BREAKDOWN; break; }  // NaN / inf in the solution: never "converged" (a NaN compares false)
         if (worst <= tol) status = WCRAS_OK;
         else if (rc == WCRAS_BREAKDOWN) { status = WCRAS_BREAKDOWN; break; }
     }
@@ -675,7 +678,8 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         if (nr > 1 && norm_k[k] > 0) LAUNCH(k_scale_d, n1, phi + k * n1, norm_k[k]);
         if (int rc = from_internal(ctx, 64, phi + k * n1, phi_dev + (size_t)k * 24 * V)) return rc;
         if (resid_per_rhs) resid_per_rhs[k] = rel_k[k];
-        worst = rel_k[k] > worst ? rel_k[k] : worst;
+        worst = rel_k[k] > worst || !std::isfinite(rel_k[k]) ? rel_k[k] : worst;
+        if (!std::isfinite(rel_k[k])) break;  // reported as it is: a non-finite residual is never hidden behind a finite one
     }
     WC_CUDA(cudaEventRecord(e1, ctx->stream));
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -698,7 +702,8 @@ int solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double tol, wc
         info->ms_blocksolve = ctx->ms_class[TC_BLOCK]; info->ms_blas = ctx->ms_class[TC_BLAS];
     }
     if (status == WCRAS_NOT_CONVERGED) snprintf(ctx->err, sizeof ctx->err, "solve: not converged after %d outer iterations", outer);
-    if (status == WCRAS_BREAKDOWN) snprintf(ctx->err, sizeof ctx->err, "solve: BiCGStab breakdown");
+    if (status == WCRAS_BREAKDOWN)
+        snprintf(ctx->err, sizeof ctx->err, std::isfinite(worst) ? "solve: BiCGStab breakdown" : "solve: BiCGStab breakdown (non-finite residual)");
     return status;
 }
 

@@ -634,13 +634,23 @@ def test_ras_autotune_full_grid():
         assert {r["operand_bits"] for r in rows[1:]} == {16, 32}
         rect = {(r["block_iters"], r["nras"]) for r in rows if r["overlap_s"] == 0 and r["schwarz"] == 0 and r["block_iters"]}
         assert {(a, b) for a in range(1, 9) for b in range(1, 6)} <= rect          # the 1..8 x 1..5 rectangle was walked
+        # stage 3: the second block solver (reading R2) was tried where its kernel runs, additive and multiplicative
+        lead_sites = int(np.prod([r for r in rows if r["block_solver"] == 1][0]["domain"])) if any(r["block_solver"] for r in rows) else 0
+        if lead_sites:
+            mr2 = [r for r in rows if r["block_solver"] == 1]
+            assert len(mr2) == 12 and {r["schwarz"] for r in mr2} == {0, 1} and all(r["operand_bits"] == 16 and r["overlap_s"] == 0 for r in mr2)
+            assert all(r["status"] == 0 for r in mr2)
+        else:  # the fastest MR row was on a cluster-tier shape or overlapped: nothing to try
+            assert int(np.prod(best["domain"])) > 256 or best["overlap_s"] > 0 or best["block_iters"] == 0
         phi, info = cs.solve(eta, 1e-12)
         assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12
         assert (info["ras_applies"] > 0) == (best["block_iters"] > 0)
     finally:
         cs.ctx.set_schwarz(False)
+        cs.ctx.set_block_solver(0)
         cs.ctx.set_operand_precision(32)
         cs.ctx.set_solver(use_ras=False)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 0, 4, 1)   # a configuration that is valid with the defaults restored
 
 
 def test_inner_iteration_graphs():

@@ -104,6 +104,20 @@ def test_mr2_solves_free_field_plane_wave_in_one_cycle():
     assert np.abs(v1 - r1 / lam[0]).max() < 1e-12
 
 
+def test_mr2_is_scale_invariant(small):
+    """The block solve is linear in the scale of its input: a residual of norm 1e-120 (squared norms 1e-240, whose PRODUCT
+    would underflow) gives the scaled result, not the degenerate-pair fallback (reading R2: the 2x2 solve is
+    written without a product of two squared norms)."""
+    dims, op, D = small
+    origin, start, ext = op.domain_box((2, 2, 2, 2), 1, 3)
+    r = I.spinor(dims, 13)
+    v, rho = op.mr2_block(start, ext, 4, r)
+    v2, rho2 = op.mr2_block(start, ext, 4, 1e-120 * r)
+    assert np.abs(v2 * 1e120 - v).max() < 1e-12 * np.abs(v).max()
+    assert np.abs(rho2 * 1e120 - rho).max() < 1e-12 * np.abs(rho).max()
+    assert np.abs(v - op.mr_block(start, ext, 4, r)[0]).max() > 1e-3   # and it is not the MR fallback
+
+
 @pytest.mark.parametrize("s,nras", [(0, 1), (0, 3), (1, 2)])
 def test_alg1_with_mr2_blocks(small, s, nras):
     """Alg. 1 with the block solver switched (wco_set_block_solver through Operator.with_block_solver): every cycle is the
