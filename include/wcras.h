@@ -123,8 +123,11 @@ int wcras_set_operand_precision(wcras_ctx* ctx, int bits);
  * q1 = D rho, q2 = D q1 the residual is minimised over span{q1, q2} (2x2 normal equations; the plain MR step if their
  * determinant is not positive); v += c1 rho + c2 q1, rho -= c1 q1 + c2 q2; an odd N_dominv ends with one MR iteration.
  * N_dominv still counts D_Omega' applications.  Built into the persistent one-CTA-per-domain kernel with 16-bit operand
- * storage (ras_cta16.cu): with kind = 1 the next wcras_ras_precondition returns WCRAS_UNSUPPORTED unless
- * wcras_set_operand_precision(ctx, 16) is set and the extended domain has at most 256 sites on the automatic tier. */
+ * storage (ras_cta16.cu) and into the generic tier (ras.cu).  On the automatic tier (wcras_set_ras_tier 0) a configuration the
+ * first cannot run -- fp32 operands, an extended domain above 256 sites -- goes to the generic tier, as does tier 1; with a
+ * forced fused tier (2..6) the next wcras_ras_precondition returns WCRAS_UNSUPPORTED unless
+ * wcras_set_operand_precision(ctx, 16) is set and the extended domain has at most 256 sites.  Multiplicative Schwarz
+ * (wcras_set_schwarz) needs the persistent kernel. */
 int wcras_set_block_solver(wcras_ctx* ctx, int kind);
 
 /* Order in which the full-lattice Dslash visits the sites (a traversal order only; no layout changes, results are

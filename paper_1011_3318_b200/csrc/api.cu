@@ -54,6 +54,7 @@ int wcras_destroy(wcras_ctx* ctx) {
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
+    if (ctx->mr_q2) cudaFree(ctx->mr_q2);
     if (ctx->dm) cudaFree(ctx->dm);
     if (ctx->dm16) { cudaFree(ctx->dm16); cudaFree(ctx->rf_dm); }
     if (ctx->hb) cudaFree(ctx->hb);

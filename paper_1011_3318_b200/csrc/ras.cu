@@ -32,13 +32,21 @@ __device__ __forceinline__ void domain_start(const Geom& g, const DomGeom& dg, i
     }
 }
 
-// q = D_Omega' rho for local site k of domain d; FIRST: rho is the full-lattice r (projection fused)
-template <bool FIRST>
+// q = D_Omega' rho for local site k of domain d; FIRST: rho is the full-lattice r (projection fused).
+// Partial dots of CTA (d, chunk) go to scal[(d * nchunk + chunk) * sstride + 0..2] = <q,rho> (re, im), <q,q>.
+// SECOND != 0 (second block solver, reading R2): the second application of a pair, q2 = D_Omega' q1 -- `rho` is
+// then the q1 buffer, `q` the q2 buffer, and the partials go to slots 3..7 = <q2,q1> (re, im) = conj(a12), a22 = <q2,q2>,
+// b2 = <q2,rho> (re, im) with the residual rho read from rho2 (SECOND = 1, domain-local) or from the full-lattice r
+// (SECOND = 2, first pair: projection fused).
+template <bool FIRST, int SECOND = 0>
 __global__ void __launch_bounds__(128) mr_dslash_kernel(Geom g, DomGeom dg, Fields<float> f, float kappa, const float4* __restrict__ rglob,
-                                                        const float4* __restrict__ rho, float4* __restrict__ q, double* __restrict__ scal) {
+                                                        const float4* __restrict__ rho, float4* __restrict__ q, double* __restrict__ scal,
+                                                        int sstride, const float4* __restrict__ rho2) {
+    static_assert(!(FIRST && SECOND), "the second application of a pair reads the domain-local q1");
+    constexpr int NACC = SECOND ? 5 : 3;
     const int d = blockIdx.x;  // domain in gridDim.x (no 65535 limit), chunk of the domain in gridDim.y
     const int k = blockIdx.y * blockDim.x + threadIdx.x;
-    double acc[3] = {0, 0, 0};
+    double acc[NACC] = {};
     if (k < dg.nloc) {
         int start[4], c[4], x[4];
         domain_start(g, dg, d, start);
@@ -103,19 +111,30 @@ __global__ void __launch_bounds__(128) mr_dslash_kernel(Geom g, DomGeom dg, Fiel
             acc[1] += (double)(qr * ri - qi * rr);
             acc[2] += (double)(qr * qr + qi * qi);
         }
+        if (SECOND) {  // b2 = <q2,rho>
+            float rt[24];
+            if (SECOND == 2) load_spinor(rglob, V, i, rt);
+            else load_spinor(rho2 + (size_t)d * 6 * dg.nloc, dg.nloc, k, rt);
+#pragma unroll
+            for (int n = 0; n < 12; n++) {
+                const float qr = out[2 * n], qi = out[2 * n + 1], rr = rt[2 * n], ri = rt[2 * n + 1];
+                acc[NACC - 2] += (double)(qr * rr + qi * ri);
+                acc[NACC - 1] += (double)(qr * ri - qi * rr);
+            }
+        }
     }
-    __shared__ double sm[3][4];
+    __shared__ double sm[NACC][4];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll
-    for (int n = 0; n < 3; n++) {
+    for (int n = 0; n < NACC; n++) {
         const double s = warp_sum(acc[n]);
         if (lane == 0) sm[n][w] = s;
     }
     __syncthreads();
-    if (threadIdx.x < 3) {  // one partial per CTA, summed in a fixed order by mr_update_kernel (deterministic)
+    if (threadIdx.x < NACC) {  // one partial per CTA, summed in a fixed order by the update kernel (deterministic)
         double s = 0;
         for (int ww = 0; ww < (int)(blockDim.x >> 5); ww++) s += sm[threadIdx.x][ww];
-        scal[((size_t)d * gridDim.y + blockIdx.y) * 4 + threadIdx.x] = s;
+        scal[((size_t)d * gridDim.y + blockIdx.y) * sstride + (SECOND ? 3 : 0) + threadIdx.x] = s;
     }
 }
 
@@ -165,6 +184,82 @@ __global__ void __launch_bounds__(128) mr_update_kernel(Geom g, DomGeom dg, cons
             float4 rn;
             rn.x = rv.x - (ar * qv.x - ai * qv.y); rn.y = rv.y - (ar * qv.y + ai * qv.x);
             rn.z = rv.z - (ar * qv.z - ai * qv.w); rn.w = rv.w - (ar * qv.w + ai * qv.z);
+            rho[li] = rn;
+            v[li] = vv;
+        } else if (bulk) {
+            const size_t gi = (size_t)ch * g.V + i;
+            if (ACCUM) {
+                const float4 o = vout[gi];
+                vv.x += o.x; vv.y += o.y; vv.z += o.z; vv.w += o.w;
+            }
+            vout[gi] = vv;
+        }
+    }
+}
+
+// Second block solver on the generic tier (reading R2; wcras_set_block_solver(1)): the update that closes a pair
+// q1 = D_Omega' rho, q2 = D_Omega' q1.  (c1, c2) minimise |rho - c1 q1 - c2 q2| (2x2 normal equations in scale-free form:
+// rows divided by a11 = <q1,q1> and a22 = <q2,q2>, g = |a12|^2 / (a11 a22); the plain MR step if 1 - g <= 1e-4 or a
+// squared norm is 0); v += c1 rho + c2 q1, rho -= c1 q1 + c2 q2.  FIRST / LAST / ACCUM as in mr_update_kernel.  The dots
+// arrive as per-CTA partials of 8 doubles: <q1,rho> (re, im), a11, <q2,q1> (re, im), a22, <q2,rho> (re, im).
+template <bool FIRST, bool LAST, bool ACCUM>
+__global__ void __launch_bounds__(128) mr2_update_kernel(Geom g, DomGeom dg, const float4* __restrict__ rglob, float4* __restrict__ rho,
+                                                         const float4* __restrict__ q1, const float4* __restrict__ q2, float4* __restrict__ v,
+                                                         float4* __restrict__ vout, const double* __restrict__ scal) {
+    const int d = blockIdx.x;
+    const int k = blockIdx.y * blockDim.x + threadIdx.x;
+    if (k >= dg.nloc) return;
+    double t[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (unsigned c = 0; c < gridDim.y; c++) {  // the per-CTA partials of this domain, in order
+        const double* p = scal + ((size_t)d * gridDim.y + c) * 8;
+#pragma unroll
+        for (int n = 0; n < 8; n++) t[n] += p[n];
+    }
+    const double b1r = t[0], b1i = t[1], a11 = t[2], a12r = t[3], a12i = -t[4], a22 = t[5], b2r = t[6], b2i = t[7];  // a12 = conj(<q2,q1>)
+    const double s1 = a11 > 0 ? 1.0 / a11 : 0.0, s2 = a22 > 0 ? 1.0 / a22 : 0.0;
+    const double u1r = b1r * s1, u1i = b1i * s1, u2r = b2r * s2, u2i = b2i * s2;
+    const double m1r = a12r * s1, m1i = a12i * s1, m2r = a12r * s2, m2i = -a12i * s2;  // a12 / a11, conj(a12) / a22
+    const double gg = a11 > 0 && a22 > 0 ? m1r * m2r - m1i * m2i : 1.0;
+    double c1r = u1r, c1i = u1i, c2r = 0, c2i = 0;  // q2 numerically parallel to q1, or rho = 0: the plain MR step
+    if (1.0 - gg > 1e-4) {
+        const double inv = 1.0 / (1.0 - gg);
+        c1r = (u1r - (m1r * u2r - m1i * u2i)) * inv;
+        c1i = (u1i - (m1r * u2i + m1i * u2r)) * inv;
+        c2r = (u2r - (m2r * u1r - m2i * u1i)) * inv;
+        c2i = (u2i - (m2r * u1i + m2i * u1r)) * inv;
+    }
+    const float ar = (float)c1r, ai = (float)c1i, br = (float)c2r, bi = (float)c2i;
+    int start[4], c[4], x[4];
+    domain_start(g, dg, d, start);
+    {
+        int kk = k;
+        c[0] = kk % dg.ext[0]; kk /= dg.ext[0];
+        c[1] = kk % dg.ext[1]; kk /= dg.ext[1];
+        c[2] = kk % dg.ext[2];
+        c[3] = kk / dg.ext[2];
+    }
+    bool bulk = true;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        x[mu] = start[mu] + c[mu];
+        if (x[mu] >= g.L[mu]) x[mu] -= g.L[mu];
+        if (dg.split[mu]) bulk = bulk && c[mu] >= dg.s && c[mu] < dg.s + dg.b[mu];
+    }
+    const size_t i = x[0] + g.L[0] * (x[1] + g.L[1] * (x[2] + (size_t)g.L[2] * x[3]));
+    const size_t base = (size_t)d * 6 * dg.nloc + k;
+#pragma unroll
+    for (int ch = 0; ch < 6; ch++) {
+        const size_t li = base + (size_t)ch * dg.nloc;
+        const float4 rv = FIRST ? rglob[(size_t)ch * g.V + i] : rho[li];
+        const float4 xv = q1[li];
+        float4 vv = FIRST ? make_float4(0.f, 0.f, 0.f, 0.f) : v[li];
+        vv.x += ar * rv.x - ai * rv.y + br * xv.x - bi * xv.y; vv.y += ar * rv.y + ai * rv.x + br * xv.y + bi * xv.x;
+        vv.z += ar * rv.z - ai * rv.w + br * xv.z - bi * xv.w; vv.w += ar * rv.w + ai * rv.z + br * xv.w + bi * xv.z;
+        if (!LAST) {
+            const float4 yv = q2[li];
+            float4 rn;
+            rn.x = rv.x - (ar * xv.x - ai * xv.y) - (br * yv.x - bi * yv.y); rn.y = rv.y - (ar * xv.y + ai * xv.x) - (br * yv.y + bi * yv.x);
+            rn.z = rv.z - (ar * xv.z - ai * xv.w) - (br * yv.z - bi * yv.w); rn.w = rv.w - (ar * xv.w + ai * xv.z) - (br * yv.w + bi * yv.z);
             rho[li] = rn;
             v[li] = vv;
         } else if (bulk) {
@@ -249,7 +344,13 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     // tier request 5: force the streamed-operand cluster kernel (tier 2c); automatic: 2a/2b when Omega' fits on chip with
     // its operands, else 2c when the spinors fit a cluster, else the generic tier
     bool fused_ok = ctx->tier_request != 1 && ctx->tier_request != 5 && ras_fused_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0;
-    if (!fused_ok && (ctx->tier_request == 0 || ctx->tier_request == 5 || ctx->tier_request == 6) &&
+    // The second block solver (reading R2) lives in the persistent one-CTA-per-domain kernel with 16-bit operand storage and
+    // on the generic tier.  On the automatic tier a configuration the first cannot run (fp32 operands, an extended domain
+    // above 256 sites) goes to the generic tier; a forced fused tier (requests 2..6) returns WCRAS_UNSUPPORTED below.
+    if (ctx->block_solver == 1 && ctx->tier_request == 0 && !(fused_ok && ctx->op_prec == 16 && fgeom.C == 1 && fgeom.nsp <= FUSED_CTA_MAX_THREADS))
+        fused_ok = false;
+    const bool mr2_generic = ctx->block_solver == 1 && !fused_ok && ctx->tier_request <= 1;
+    if (!fused_ok && !mr2_generic && (ctx->tier_request == 0 || ctx->tier_request == 5 || ctx->tier_request == 6) &&
         ras_stream_prepare(ctx, rc.b, rc.ext, s, niter, &fgeom) != 0) {
         fused_ok = true;
         rc.stream = true;
@@ -263,14 +364,17 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
     if (ctx->mr_rho) {
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
         cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal);
-        ctx->mr_rho = ctx->mr_q = ctx->mr_v = nullptr; ctx->mr_scal = nullptr;
+        if (ctx->mr_q2) cudaFree(ctx->mr_q2);
+        ctx->mr_rho = ctx->mr_q = ctx->mr_v = ctx->mr_q2 = nullptr; ctx->mr_scal = nullptr;
     }
     if (rc.tier == 1) {
         const size_t nb = sizeof(float4) * 6 * (size_t)rc.nd * rc.nloc;
         WC_CUDA(cudaMalloc((void**)&ctx->mr_rho, nb));
         WC_CUDA(cudaMalloc((void**)&ctx->mr_q, nb));
         WC_CUDA(cudaMalloc((void**)&ctx->mr_v, nb));
-        WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * ((rc.nloc + 127) / 128) * niter));
+        // [niter][nd][nchunk][4] per-CTA partial dots; the second block solver uses two iterations' worth per pair ([..][8])
+        WC_CUDA(cudaMalloc((void**)&ctx->mr_scal, sizeof(double) * 4 * (size_t)rc.nd * ((rc.nloc + 127) / 128) * (niter + 1)));
+        if (ctx->block_solver == 1) WC_CUDA(cudaMalloc((void**)&ctx->mr_q2, nb));
     }
     if (ctx->dm) {
         WC_CUDA(cudaStreamSynchronize(ctx->stream));
@@ -310,12 +414,13 @@ int ras_configure(wcras_ctx* ctx, const int domain[4], int s, int niter, int nra
             ctx->nface = rc.cl16 ? fgeom.C * ctx->cl16_nfc : (nface + 7) / 8 * 8;  // ras_cl16: halo slots per CTA, [nd][C][8][3][nfc]
         }
     }
-    if (ctx->block_solver == 1 && !rc.cta16) {
-        // the second block solver lives in the persistent one-CTA-per-domain kernel with 16-bit operand storage only
+    if (ctx->block_solver == 1 && !rc.cta16 && rc.tier != 1) {
+        // among the fused tiers the second block solver lives in the persistent one-CTA-per-domain kernel with 16-bit
+        // operand storage only
         ctx->ras.set = false;
         snprintf(ctx->err, sizeof ctx->err,
-                 "ras_precondition: block solver 1 (two-dimensional minimal residual) needs 16-bit operand storage and an "
-                 "extended domain of at most 256 sites on the automatic tier");
+                 "ras_precondition: on a forced fused tier block solver 1 (two-dimensional minimal residual) needs 16-bit operand "
+                 "storage and an extended domain of at most 256 sites; the automatic and the generic tier take every shape");
         return WCRAS_UNSUPPORTED;
     }
     ctx->ras = rc;
@@ -331,11 +436,34 @@ static int generic_block_solve(wcras_ctx* ctx, const float4* r, float4* vout, bo
     const dim3 grid(rc.nd, nchunk);
     const Fields<float> f = ras_fields(ctx);
     const float kappa = (float)ctx->kappa;
-    for (int it = 0; it < rc.niter; it++) {
+    int it = 0;
+    if (ctx->block_solver == 1) {
+        // second block solver (reading R2): pairs of D_Omega' applications closed by the two-dimensional minimisation; an odd
+        // N_dominv ends with one MR iteration (the loop below).  Partial dots: 8 doubles per (pair, domain, chunk).
+        for (; it + 1 < rc.niter; it += 2) {
+            double* scal = ctx->mr_scal + (size_t)it * rc.nd * nchunk * 4;  // [pair][nd][nchunk][8]
+            const bool first = it == 0, last = it + 2 == rc.niter;
+            if (first) {
+                mr_dslash_kernel<true, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal, 8, nullptr);
+                mr_dslash_kernel<false, 2><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_q, ctx->mr_q2, scal, 8, nullptr);
+            } else {
+                mr_dslash_kernel<false, 0><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal, 8, nullptr);
+                mr_dslash_kernel<false, 1><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_q, ctx->mr_q2, scal, 8, ctx->mr_rho);
+            }
+#define WC_UPD2(F, L, A) mr2_update_kernel<F, L, A><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, r, ctx->mr_rho, ctx->mr_q, ctx->mr_q2, ctx->mr_v, vout, scal)
+            if (first && last) { if (accum) WC_UPD2(true, true, true); else WC_UPD2(true, true, false); }
+            else if (first) WC_UPD2(true, false, false);
+            else if (last) { if (accum) WC_UPD2(false, true, true); else WC_UPD2(false, true, false); }
+            else WC_UPD2(false, false, false);
+#undef WC_UPD2
+            ctx->launches += 3;
+        }
+    }
+    for (; it < rc.niter; it++) {
         double* scal = ctx->mr_scal + (size_t)it * rc.nd * nchunk * 4;  // [niter][nd][nchunk][4] per-CTA partial dots
         const bool first = it == 0, last = it == rc.niter - 1;
-        if (first) mr_dslash_kernel<true><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);
-        else mr_dslash_kernel<false><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal);
+        if (first) mr_dslash_kernel<true><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal, 4, nullptr);
+        else mr_dslash_kernel<false><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, f, kappa, r, ctx->mr_rho, ctx->mr_q, scal, 4, nullptr);
 #define WC_UPD(F, L, A) mr_update_kernel<F, L, A><<<grid, TH, 0, ctx->stream>>>(ctx->geom, dg, r, ctx->mr_rho, ctx->mr_q, ctx->mr_v, vout, scal)
         if (first && last) { if (accum) WC_UPD(true, true, true); else WC_UPD(true, true, false); }
         else if (first) WC_UPD(true, false, false);

@@ -8,7 +8,7 @@
 // issues at ~55-65 % of the slots (ncu: stalls on fixed-latency dependencies and shared-memory loads).  Here a site is
 // shared by the lanes l and l + 16 of one warp ("halves" p = 0, 1); each half owns two of the four directions and one of
 // the two chiralities, needs <= 128 registers, and the SM holds 16 warps = 4 per scheduler.
-// RESULT (profiles/r2_block_solver.md): correct (same parity tests), but SLOWER than ras_cta16.cu -- 410 against 337 us for
+// RESULT (profiles/r2_kernels.md): correct (same parity tests), but SLOWER than ras_cta16.cu -- 410 against 337 us for
 // four sweeps at 32^4: the issue rate rises only from 64 % to 69 % of the slots (1.9 eligible warps per cycle, the rest
 // are dispatch and math-pipe stalls: the fp32 pipe and its register-file ports are the limit, not latency) while the
 // instruction count grows by 32 % (exchange shuffles, selections, FFMA with sign registers instead of FADD, replicated

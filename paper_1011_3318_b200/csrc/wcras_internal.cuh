@@ -135,7 +135,7 @@ struct FusedGeom {
     int V, s, ns, nsp, C, niter;
     int nclus;       // tier 2b: clusters (or CTAs) resident at once = persistent grid size in clusters
     int pdir;        // multiplicative Schwarz: pairing direction of the red-black domain enumeration, -1 = not colourable
-    int mr2 = 0;     // block solver: 1 = restarted two-dimensional minimal residual (reading R2; ras_cta16.cu only)
+    int mr2 = 0;     // block solver: 1 = restarted two-dimensional minimal residual (reading R2; ras_cta16.cu; the generic tier reads ctx->block_solver)
     const int* stop; // device flag of the running inner solver (see wc::Geom::stop), or nullptr
 };
 
@@ -197,6 +197,7 @@ struct wcras_ctx {
     int nface = 0;
     int hb_nrhs = 0;               // stack depth the halo buffers are allocated for
     float4 *mr_rho = nullptr, *mr_q = nullptr, *mr_v = nullptr;  // [nd][6][nloc]
+    float4* mr_q2 = nullptr;                                        // second block solver on the generic tier: q2 = D q1
     double* mr_scal = nullptr;                                     // [niter][nd][nchunk][4] per-CTA partial dots
     // solver parameters
     double inner_tol = 5e-7;       // deepest relative accuracy asked of one fp32 inner solve (reading A2)

@@ -370,6 +370,40 @@ def test_ras_apply_mr2_block_solver(which, block, s, nit, nras, tier):
         cs.ctx.set_ras_tier(0)
 
 
+MR2_GENERIC_CASES = [
+    # (case, block, overlap, N_dominv, NRAS, operand bits, tier): the second block solver on the generic tier -- forced
+    # (tier 1), and chosen by the automatic tier (0) where the persistent fp16-operand kernel does not apply: fp32 operands,
+    # overlap that pushes the extended domain above 256 sites, shapes of the cluster and streamed tiers, ragged domains
+    (0, (2, 2, 2, 2), 0, 4, 3, 32, 1), (0, (2, 2, 2, 2), 1, 3, 2, 16, 1), (1, (4, 4, 4, 4), 0, 2, 1, 32, 0),
+    (1, (4, 4, 4, 4), 0, 5, 2, 32, 0), (1, (4, 4, 4, 4), 0, 4, 2, 16, 1), (1, (4, 4, 4, 4), 1, 4, 2, 16, 0),
+    (1, (4, 4, 4, 4), 1, 3, 1, 32, 0), (1, (8, 8, 4, 4), 0, 6, 2, 16, 0), (1, (8, 4, 8, 8), 0, 2, 2, 32, 0),
+    ("ragged", (3, 4, 5, 2), 1, 4, 2, 32, 0), ("ragged", (6, 4, 10, 4), 0, 3, 1, 16, 0), (1, (4, 4, 4, 4), 0, 1, 2, 32, 1),
+]
+
+
+@pytest.mark.parametrize("which,block,s,nit,nras,bits,tier", MR2_GENERIC_CASES)
+def test_ras_apply_mr2_generic_tier(which, block, s, nit, nras, bits, tier):
+    """wcras_set_block_solver(1) on the generic tier (every shape, overlap and operand precision; reading R2)
+    against the oracle's Alg. 1 with wco_mr2_block."""
+    cs = ragged_case() if which == "ragged" else case(which)
+    cs.ctx.set_ras_tier(tier)
+    cs.ctx.set_operand_precision(bits)
+    cs.ctx.set_block_solver(1)
+    try:
+        cs.ctx.ras_precondition(block, s, nit, nras)
+        r32 = I.spinor(cs.dims, 63).astype(np.complex64).astype(np.complex128)
+        op = rounded_op(cs) if bits == 16 else cs.op
+        want = op.with_block_solver("mr2").ras_apply(block, s, nit, nras, r32)
+        got = cs.ras_apply(r32)
+        assert rel(got, want) <= TOL_RAS
+        if nit >= 2:
+            assert rel(got, op.ras_apply(block, s, nit, nras, r32)) > 2 * TOL_RAS
+    finally:
+        cs.ctx.set_block_solver(0)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.set_ras_tier(0)
+
+
 def test_mr2_block_solver_sap_solve_and_limits():
     """The second block solver through multiplicative Schwarz and through the nested solve (true residual by the oracle on
     the exact operator); UNSUPPORTED where the kernel that holds it does not run (fp32 operands, larger domains)."""
@@ -396,15 +430,26 @@ def test_mr2_block_solver_sap_solve_and_limits():
             assert info["inner_iters"] < i0["inner_iters"]
             # (a smaller block residual does not always make a better preconditioner: the iteration count may go either way
             # against MR by one on this lattice, so it is reported by bench.py's survey rows, not asserted)
-        for bits, block, s in ((32, (4, 4, 4, 4), 0), (16, (4, 4, 4, 4), 1), (16, (8, 8, 4, 4), 0)):
+        # a forced fused tier that is not the persistent fp16-operand kernel cannot run it (the automatic tier sends these
+        # configurations to the generic tier: test_ras_apply_mr2_generic_tier)
+        for tier, bits, block, s in ((2, 32, (4, 4, 4, 4), 0), (2, 16, (4, 4, 4, 4), 1), (2, 16, (8, 8, 4, 4), 0), (3, 16, (8, 8, 4, 4), 0)):
+            cs.ctx.set_ras_tier(tier)
             cs.ctx.set_operand_precision(bits)
             with pytest.raises(binding.WcrasError) as e:
                 cs.ctx.ras_precondition(block, s, 2, 1)
             assert e.value.code == binding.UNSUPPORTED
+        cs.ctx.set_ras_tier(0)
+        # the nested solve through the generic tier (fp32 operands, overlap 1)
+        cs.ctx.set_operand_precision(32)
+        cs.ctx.ras_precondition((4, 4, 4, 4), 1, 4, 1)
+        cs.ctx.set_solver(use_ras=True)
+        phi, info = cs.solve(eta, 1e-12)
+        assert info["status"] == 0 and cs.op.true_residual(eta, phi) <= 1e-12 and info["inner_iters"] < i0["inner_iters"]
         with pytest.raises(binding.WcrasError) as e:
             cs.ctx.set_block_solver(2)
         assert e.value.code == binding.INVALID_ARG
     finally:
+        cs.ctx.set_ras_tier(0)
         cs.ctx.set_block_solver(0)
         cs.ctx.set_operand_precision(32)
         cs.ctx.set_solver(use_ras=False)
