@@ -11,7 +11,9 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libwcras.so")
+# WCRAS_LIB: another build of the same library (e.g. the phase-profile build of `python -m paper_1011_3318_b200.build
+# --phase-profile`); still a CUDA library behind the same C ABI, never a fallback
+LIB_PATH = os.environ.get("WCRAS_LIB") or os.path.join(_HERE, "libwcras.so")
 
 OK, INVALID_ARG, UNSUPPORTED, CUDA_ERROR, BREAKDOWN, NOT_CONVERGED = 0, -1, -2, -3, -4, -5
 

@@ -63,9 +63,27 @@ def build_microbench() -> str:
     return out
 
 
+def build_phase_profile() -> str:
+    """A copy of the library whose persistent block solver (csrc/ras_cta16.cu, -DWC_CTA16_PROFILE) prints the cycles thread 0
+    of CTA 0 spends in each phase of the domain loop; load it with WCRAS_LIB=<path> (results: profiles/r2_kernels.md)."""
+    build()
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    objdir = os.path.join(HERE, "build")
+    obj = os.path.join(objdir, "ras_cta16_phase.o")
+    out = os.path.join(objdir, "libwcras_phase.so")
+    for cmd in ([nvcc] + NVCC_FLAGS + ["-DWC_CTA16_PROFILE", "-c", os.path.join(CSRC, "ras_cta16.cu"), "-o", obj],
+                [nvcc, "-shared", "-o", out] + [os.path.join(objdir, s.replace(".cu", ".o")) for s in SOURCES if s != "ras_cta16.cu"] + [obj, "-lcudart"]):
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode:
+            raise RuntimeError("nvcc failed:\n%s\n%s" % (r.stdout, r.stderr))
+    return out
+
+
 if __name__ == "__main__":
     import sys
     if "--microbench" in sys.argv:
         print(build_microbench())
+    elif "--phase-profile" in sys.argv:
+        print(build_phase_profile())
     else:
         print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -81,8 +81,17 @@ __global__ void round_half_kernel(size_t n, const float* __restrict__ in, float*
 // cycle-level phase profile of CTA 0 (debug builds only: -DWC_CTA16_PROFILE prints the totals of thread 0)
 #ifdef WC_CTA16_PROFILE
 #define WC_T(n) { const long long t_ = clock64(); if (k == 0) prof[n] += t_ - tlast; tlast = t_; }
+// has the link half of the NEXT domain landed?  (non-blocking test of the next phase of bar_links, thread 0)
+#define WC_LANDED(n)                                                                                                          \
+    if (k == 0) {                                                                                                             \
+        unsigned ok_;                                                                                                         \
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"  \
+                     : "=r"(ok_) : "r"(bar_links), "r"(par ^ 1u) : "memory");                                                 \
+        landed[n] += ok_;                                                                                                     \
+    }
 #else
 #define WC_T(n)
+#define WC_LANDED(n)
 #endif
 
 struct Cta16Smem {  // offsets in float4 units
@@ -249,6 +258,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 
 #ifdef WC_CTA16_PROFILE
     long long prof[12] = {0}, tlast = clock64();
+    int landed[3] = {0, 0, 0};
 #endif
     // Per-launch uniforms the domain loop tests after its last stores, pinned in one register: rematerialised from the
     // constant bank there, each is a load of a few hundred cycles that the ncu source page shows as a long-scoreboard stall
@@ -353,6 +363,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #undef WC_SCATTER
             }
             WC_T(6)
+            if (it == 1) WC_LANDED(0)
             if (it == 0) mbar_wait(bar_clov, par);
             WC_T(7)
             // q = A in from the staged fp16 clover blocks: block 0 = halfs 0..35 (chunks 9..13), block 1 = halfs
@@ -511,6 +522,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #endif
         }
         WC_T(11)
+        WC_LANDED(1)
         // ---- halo scatter for the next cycle: the hops of v that leave the domain, as projected half spinors ----
         if (WC_UNI_HALO) {
             unsigned dd = dom_bc_here;
@@ -559,6 +571,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
                     phi_out[(size_t)c * V + gi] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
             }
         }
+        WC_LANDED(2)
         if (!has_next) break;
         h = hn;
     }
@@ -571,6 +584,9 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
         printf("cta16 prof chain %d niter %d: epi/loop %lld | links wait %lld cvt %lld | vec wait %lld rho %lld cross %lld | scatter %lld clov wait %lld "
                "clover %lld | barriers %lld gather+dots %lld update %lld\n", (int)CHAIN, fg.niter, prof[0], prof[1], prof[2], prof[3], prof[4], prof[5],
                prof[6], prof[7], prof[8], prof[9], prof[10], prof[11]);
+    if (k == 0 && blockIdx.x == 0)
+        printf("cta16 next links landed (of %d next domains) chain %d: after the scatter of sweep 1 %d, after the last update %d, after the epilogue %d\n",
+               (ndl - 1 - (int)blockIdx.x) / (int)gridDim.x, (int)CHAIN, landed[0], landed[1], landed[2]);
 #endif
 }
 
