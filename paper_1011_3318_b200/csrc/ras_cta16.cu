@@ -91,7 +91,7 @@ __global__ void round_half_kernel(size_t n, const float* __restrict__ in, float*
     }
 #else
 #define WC_T(n)
-#define WC_LANDED(n)
+#define WC_LANDED(n) {}
 #endif
 
 struct Cta16Smem {  // offsets in float4 units
@@ -363,7 +363,7 @@ ras_cta16_kernel(FusedGeom fg, int ndl, int colour, int nface, int stage_halo, f
 #undef WC_SCATTER
             }
             WC_T(6)
-            if (it == 1) WC_LANDED(0)
+            if (it == 1) { WC_LANDED(0) }
             if (it == 0) mbar_wait(bar_clov, par);
             WC_T(7)
             // q = A in from the staged fp16 clover blocks: block 0 = halfs 0..35 (chunks 9..13), block 1 = halfs
