@@ -194,7 +194,12 @@ int wcras_solve(wcras_ctx* ctx, const double* eta_dev, double* phi_dev, double t
 int wcras_solve_multi(wcras_ctx* ctx, int nrhs, const double* eta_dev, double* phi_dev, double tol, wcras_info* info,
                       double* rel_resid_host);
 
-/* Same, with HOST buffers: copies eta to the device, solves, copies phi back (end-to-end entry point). */
+/* wcras_solve with HOST buffers (24*V doubles each, pinned or pageable; the end-to-end entry point): copies eta to the
+ * device, solves, copies phi back; returns after phi_host is complete.  The copy of phi runs on an internal stream beside
+ * the fp64 true-residual check of the same phi and is repeated if a later pass corrects phi, so phi_host
+ * may be written more than once during the call; on return it holds bit for bit what wcras_solve would have left in
+ * phi_dev.  info->ms_total is the device time of the solve without the two copies.  On an error code other than
+ * WCRAS_NOT_CONVERGED / WCRAS_BREAKDOWN the contents of phi_host are unspecified. */
 int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, double tol, wcras_info* info);
 
 /* One row of the parameter survey of wcras_ras_autotune. */

@@ -52,6 +52,9 @@ int wcras_destroy(wcras_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     drop_iter_graphs(ctx);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_copy_ready) cudaEventDestroy(ctx->ev_copy_ready);
+    if (ctx->ev_copy_done) cudaEventDestroy(ctx->ev_copy_done);
     for (void* p : ctx->owned) cudaFree(p);
     if (ctx->mr_rho) { cudaFree(ctx->mr_rho); cudaFree(ctx->mr_q); cudaFree(ctx->mr_v); cudaFree(ctx->mr_scal); }
     if (ctx->mr_q2) cudaFree(ctx->mr_q2);
@@ -221,10 +224,23 @@ int wcras_solve_host(wcras_ctx* ctx, const double* eta_host, double* phi_host, d
     NEED(!ctx->use_ras || ctx->ras.set, "solve_host: use_ras is set but wcras_ras_precondition was not called");
     if (int rc = ensure_io(ctx)) return rc;
     const size_t bytes = sizeof(double) * 24 * (size_t)ctx->geom.V;
+    if (!ctx->copy_stream) {
+        WC_CUDA(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        WC_CUDA(cudaEventCreateWithFlags(&ctx->ev_copy_ready, cudaEventDisableTiming));
+        WC_CUDA(cudaEventCreateWithFlags(&ctx->ev_copy_done, cudaEventDisableTiming));
+    }
     WC_CUDA(cudaMemcpyAsync(ctx->io_a, eta_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    // solve() sends every candidate phi to phi_host on the copy stream while its fp64 true residual is still being checked;
+    // the copy that belongs to the final phi is the last one, and solve() returns after it has completed
+    ctx->host_out = phi_host;
+    ctx->host_copied = false;
     int rc = solve(ctx, (const double*)ctx->io_a, (double*)ctx->io_b, tol, info);
-    if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) return rc;
-    WC_CUDA(cudaMemcpyAsync(phi_host, ctx->io_b, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->host_out = nullptr;
+    if (rc != WCRAS_OK && rc != WCRAS_NOT_CONVERGED && rc != WCRAS_BREAKDOWN) {
+        cudaStreamSynchronize(ctx->copy_stream);  // nothing may still write the caller's buffer after an error return
+        return rc;
+    }
+    if (!ctx->host_copied) WC_CUDA(cudaMemcpyAsync(phi_host, ctx->io_b, bytes, cudaMemcpyDeviceToHost, ctx->stream));
     WC_CUDA(cudaStreamSynchronize(ctx->stream));
     return rc;
 }

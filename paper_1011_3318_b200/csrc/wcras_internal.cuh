@@ -229,6 +229,12 @@ struct wcras_ctx {
     unsigned graph_gen = 0;
     unsigned cfg_gen = 1;          // bumped by every call that changes what an inner iteration launches
     int use_graphs = 1;
+    // wcras_solve_host: the device->host copy of phi starts before the fp64 true-residual check of the same phi and runs beside
+    // it on this stream (solve() in solver.cu); host_out != nullptr only while wcras_solve_host is inside solve()
+    double* host_out = nullptr;
+    bool host_copied = false;           // solve() has delivered the final phi to host_out
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copy_ready = nullptr, ev_copy_done = nullptr;
     cudaStream_t cap_stream = nullptr;  // captures run on this internal stream (the caller's may be the legacy default stream, which cannot capture)
     double* partials = nullptr;    // reduction scratch [RED_BLOCKS][8]
     unsigned* ticket = nullptr;

@@ -571,6 +571,44 @@ def test_solve_host_buffers_and_zero_source():
     assert info["status"] == 0 and np.abs(p).max() == 0.0
 
 
+def test_solve_host_equals_device_solve_also_over_several_passes():
+    """wcras_solve_host sends phi to the host beside the fp64 true-residual check of the same phi (copy stream); what arrives
+    is bit for bit the phi of wcras_solve, with pinned and with pageable buffers, also when the check fails and later
+    passes correct phi (tolerance below what fp64 reaches: several passes, status NOT_CONVERGED, the last phi delivered)."""
+    cs = case(1)
+    eta = I.spinor(cs.dims, 5)
+    cs.ctx.ras_precondition((4, 4, 4, 4), 0, 4, 1)
+    cs.ctx.set_solver(use_ras=True)
+    try:
+        for tol, strict in ((1e-12, True), (1e-17, False)):
+            x = dev(eta, torch.float64)
+            y = torch.empty_like(x)
+            info_d = cs.ctx.solve(x, y, tol, strict=strict)
+            want = y.cpu().numpy()
+            e_pin = torch.view_as_real(torch.from_numpy(np.ascontiguousarray(eta))).contiguous().pin_memory()
+            p_pin = torch.full_like(e_pin, float("nan")).pin_memory()
+            e_pag = np.ascontiguousarray(eta).view(np.float64).copy()
+            p_pag = np.full_like(e_pag, np.nan)
+            for e_ptr, p_ptr, got in ((e_pin.data_ptr(), p_pin.data_ptr(), lambda: p_pin.numpy()),
+                                      (e_pag.ctypes.data, p_pag.ctypes.data, lambda: p_pag)):
+                info_h = cs.ctx.solve_host(e_ptr, p_ptr, tol, strict=strict)
+                assert info_h["status"] == info_d["status"] and info_h["outer_iters"] == info_d["outer_iters"]
+                assert info_h["rel_resid_true"] == info_d["rel_resid_true"]
+                assert np.array_equal(got().reshape(want.shape), want)
+            if strict:
+                assert info_d["status"] == 0
+            else:
+                assert info_d["status"] != 0 and info_d["dv_fp64"] >= 5   # several true-residual checks = several passes
+            phi = p_pag.view(np.complex128).reshape(cs.V, 4, 3)
+            true = cs.op.true_residual(eta, phi)
+            if strict:
+                assert true <= 1e-12 and abs(true - info_d["rel_resid_true"]) <= 1e-2 * true
+            else:
+                assert true <= 1e-14   # at the rounding level of fp64 the two sums differ in the first digit
+    finally:
+        cs.ctx.set_solver(use_ras=False)
+
+
 def test_ras_reduces_iterations():
     """the RAS preconditioner reduces the Dv count of the GPU solver."""
     cs = case(1)
