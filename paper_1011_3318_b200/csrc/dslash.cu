@@ -49,6 +49,60 @@ __device__ __forceinline__ void dslash_block_partial(double (&v)[3], double* __r
     }
 }
 
+// what the totals of the fused dots mean for the solver's scalars (one thread)
+template <int DOT>
+__device__ __forceinline__ void dot_finish_scalars(const double (&tot)[3], Scalars* sc) {
+    if (DOT == 3) {
+        sc->nrm = tot[2];
+    } else if (DOT == 1) {
+        sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
+        const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
+        sc->alpha[0] = a.r; sc->alpha[1] = a.i;
+    } else {
+        sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
+        sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
+        sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
+    }
+}
+
+// Small lattices (at most FIN_INLINE_MAX partials; one right-hand side): the Dslash finishes its dots itself -- the last
+// CTA to arrive (fence + atomic ticket) sums the partials of all CTAs in a fixed order and applies dot_finish_scalars.
+// One kernel node less per Dslash where a solve is bound by the latency of its dependent launches (reading A1);
+// at 32^4 the fence per 64-thread CTA costs ~15 % of the kernel, so large lattices keep the separate finish kernel.
+constexpr unsigned FIN_INLINE_MAX = 512;  // measured: -16..18 % per solve at 4^4 and 8^4 (64 CTAs), no gain at 16^4 (1024 CTAs)
+template <int TH, int DOT>
+__device__ __forceinline__ void dslash_finish_inline(const double* part, unsigned nblk, unsigned* ticket, Scalars* sc) {
+    constexpr int NW = TH / 32;
+    __shared__ bool last_s;
+    __shared__ double fs[3][NW];
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x, lane = tid & 31, w = tid >> 5;
+    __syncthreads();  // the partial of this CTA has been written (threads 0..2)
+    if (tid == 0) {
+        __threadfence();
+        last_s = atomicInc(ticket, nblk - 1) == nblk - 1;  // wraps back to 0: ready for the next launch
+    }
+    __syncthreads();
+    if (!last_s) return;
+    __threadfence();
+    double t[3] = {0, 0, 0};
+    for (unsigned j = tid; j < nblk; j += TH)
+#pragma unroll
+        for (int k = 0; k < 3; k++) t[k] += __ldcg(&part[(size_t)k * nblk + j]);
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const double u = warp_sum(t[k]);
+        if (lane == 0) fs[k][w] = u;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double tot[3] = {0, 0, 0};
+        for (int j = 0; j < NW; j++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) tot[k] += fs[k][j];
+        dot_finish_scalars<DOT>(tot, sc);
+    }
+}
+
 // FIN_CTAS CTAs each sum a contiguous slice of the partials in a fixed order; the last one to finish (atomic ticket)
 // sums the FIN_CTAS slice sums in a fixed order and finishes the scalar recurrence.
 constexpr int FIN_CTAS = 16;
@@ -88,29 +142,21 @@ __global__ void __launch_bounds__(512) dot_finish_kernel(const double* __restric
     for (int j = 0; j < FIN_CTAS; j++)
 #pragma unroll
         for (int k = 0; k < 3; k++) tot[k] += __ldcg(&slice[j * 3 + k]);
-    if (DOT == 3) {
-        sc->nrm = tot[2];
-    } else if (DOT == 1) {
-        sc->rtv[0] = tot[0]; sc->rtv[1] = tot[1];
-        const cd a = cdiv({sc->rho[0], sc->rho[1]}, {tot[0], tot[1]});
-        sc->alpha[0] = a.r; sc->alpha[1] = a.i;
-    } else {
-        sc->ts[0] = tot[0]; sc->ts[1] = tot[1]; sc->tt = tot[2];
-        sc->omega[0] = tot[2] > 0 ? tot[0] / tot[2] : 0.0;
-        sc->omega[1] = tot[2] > 0 ? tot[1] / tot[2] : 0.0;
-    }
+    dot_finish_scalars<DOT>(tot, sc);
 }
 
 // DOT = 0: out = D in (XPAY: out = bsrc - D in).
 // DOT = 1: also rtv = <dotv, out> and alpha = rho / rtv          (BiCGStab: v = D ph, dotv = rt)
 // DOT = 2: also ts = <out, dotv>, tt = <out, out>, omega = ts/tt (BiCGStab: t = D sh, dotv = s)
 // DOT = 3: also nrm = <out, out>                                  (true residual: out = eta - D phi)
-template <typename T, bool XPAY, int TH, int MINB, int DOT>
+// FIN: the kernel finishes its dots itself (dslash_finish_inline; fticket, sc), no dot_finish_kernel behind it.
+template <typename T, bool XPAY, int TH, int MINB, int DOT, bool FIN = false>
 __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T kappa, const typename VecOf<T>::type* __restrict__ in,
                                                      typename VecOf<T>::type* out,  // may be bsrc (r = r - D v in place)
                                                      const typename VecOf<T>::type* bsrc,
                                                      const typename VecOf<T>::type* __restrict__ dotv, double* part,
-                                                     unsigned pstride, unsigned poff, size_t rstride, int ztile) {
+                                                     unsigned pstride, unsigned poff, size_t rstride, int ztile,
+                                                     unsigned* fticket = nullptr, Scalars* fsc = nullptr) {
     // blockDim = (sites, right-hand sides): the threads threadIdx.y = 0..nrhs-1 of a site work on the vectors of a
     // stack rstride apart and load the same links and clover term, which L1 serves after the first warp has
     // fetched them (576/nrhs + 192 bytes of DRAM traffic per site and right-hand side)
@@ -182,6 +228,7 @@ __global__ void __launch_bounds__(TH, MINB) dslash_kernel(Geom g, Fields<T> f, T
         }
     }
     if (DOT) dslash_block_partial<TH>(dsum, part, pstride, poff);
+    if (DOT && FIN) dslash_finish_inline<TH, DOT>(part, pstride, fticket, fsc);
 }
 
 struct Box {
@@ -291,9 +338,20 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
         slice = ctx->dpart + 3 * (size_t)ctx->dpart_blocks;
         fticket = (unsigned*)(slice + 3 * FIN_CTAS);
     }
+    // small lattices, one right-hand side: the Dslash finishes its dots itself (dslash_finish_inline)
+    const bool fin = dot && nr == 1 && nblk <= FIN_INLINE_MAX;
 #define WC_DSL(TH, BLOCK, INP, OUTP, BM, DV, POFF)                                                                                    \
     {                                                                                                                              \
-        if (dot == 1)                                                                                                              \
+        if (fin && dot == 1)                                                                                                       \
+            dslash_kernel<T, false, 64, (sizeof(T) == 4 ? 6 : 1), 1, true><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                               nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile, fticket, sc); \
+        else if (fin && dot == 2)                                                                                                  \
+            dslash_kernel<T, false, 64, (sizeof(T) == 4 ? 6 : 1), 2, true><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                               nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile, fticket, sc); \
+        else if (fin && dot == 3)                                                                                                  \
+            dslash_kernel<T, true, 64, (sizeof(T) == 4 ? 6 : 1), 3, true><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
+                                                                              BM, nullptr, ctx->dpart, nblk, POFF, rstride, ztile, fticket, sc); \
+        else if (dot == 1)                                                                                                              \
             dslash_kernel<T, false, TH, (sizeof(T) == 4 ? 384 / TH : 1), 1><<<grid, BLOCK, 0, ctx->stream>>>(ctx->geom, ctx->dslash_fields<T>(), (T)ctx->kappa, INP, OUTP, \
                                                                                nullptr, DV, ctx->dpart, nblk, POFF, rstride, ztile); \
         else if (dot == 2)                                                                                                         \
@@ -319,10 +377,12 @@ int dslash(wcras_ctx* ctx, const typename VecOf<T>::type* in, typename VecOf<T>:
             WC_DSL(64, dim3(64, 1), in + r * rstride, out + r * rstride, b_minus + r * rstride, dotv + r * rstride, r * grid)
     }
 #undef WC_DSL
-    if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
-    if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
-    if (dot == 3) dot_finish_kernel<3><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, nullptr);
-    if (dot) ctx->launches++;
+    if (!fin) {
+        if (dot == 1) dot_finish_kernel<1><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
+        if (dot == 2) dot_finish_kernel<2><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, ctx->geom.stop);
+        if (dot == 3) dot_finish_kernel<3><<<FIN_CTAS, 512, 0, ctx->stream>>>(ctx->dpart, nblk, slice, fticket, sc, nullptr);
+        if (dot) ctx->launches++;
+    }
     if (sizeof(T) == 4) ctx->dv32++; else ctx->dv64++;
     WC_CHECK_LAUNCH();
     return WCRAS_OK;
